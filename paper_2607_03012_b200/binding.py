@@ -1,0 +1,308 @@
+"""Thin ctypes binding of libhva.so (include/hva.h).  Argument marshalling only: every step of
+the path runs in the CUDA kernels behind the C ABI.  PyTorch is used for device memory and the
+current stream.  There is no CPU fallback: importing works without a GPU (symbols load), any
+compute call without a CUDA device raises."""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+
+import torch
+
+from .inputs import Workload
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhva.so")
+
+HVA_F32, HVA_BF16 = 0, 1
+HVA_ANCHOR, HVA_INTERMEDIATE, HVA_DENSE = 0, 1, 2
+
+EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes",
+           "hva_plan_describe", "hva_cluster", "hva_select_subset", "hva_cluster_update", "hva_build_mask", "hva_merge",
+           "hva_build_plan", "hva_permute", "hva_unpermute", "hva_sparse_attention", "hva_forward", "hva_forward_host"]
+
+
+class hva_shape(C.Structure):
+    _fields_ = [(k, C.c_int32) for k in ("B", "heads", "T", "H", "W", "D", "dtype")]
+
+
+class hva_config(C.Structure):
+    _fields_ = [("cell_q", C.c_int32 * 3), ("cell_k", C.c_int32 * 3), ("win_q", C.c_int32 * 3), ("win_k", C.c_int32 * 3),
+                ("iters", C.c_int32), ("tile_q", C.c_int32), ("tile_k", C.c_int32), ("top_p", C.c_float),
+                ("min_kc", C.c_float), ("merge_rounds", C.c_int32), ("max_q_tiles", C.c_int32), ("seed", C.c_uint32),
+                ("subset_frac", C.c_float), ("hybrid_refresh_all", C.c_int32), ("softmax_scale", C.c_float)]
+
+
+class hva_stats(C.Structure):
+    _fields_ = [("n_groups", C.c_int32), ("q_tiles", C.c_int32), ("q_rows_valid", C.c_int64),
+                ("q_rows_padded", C.c_int64), ("k_cols_valid", C.c_int64), ("k_cols_padded", C.c_int64),
+                ("tiles_executed", C.c_int64), ("pairs_valid", C.c_int64)]
+
+
+class hva_plan_layout(C.Structure):
+    _fields_ = [(k, C.c_size_t) for k in ("perm_q", "inv_perm_q", "perm_k", "koff", "n_groups", "gid", "goff", "kappa",
+                                          "run_cnt", "runs", "run_stride", "work_cnt", "work", "work_cap", "stats", "total")]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libhva.so (raises if it has not been built: `python -m paper_2607_03012_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} missing: build it with `python paper_2607_03012_b200/build.py`")
+        L = C.CDLL(LIB_PATH)
+        L.hva_strerror.restype = C.c_char_p
+        L.hva_workspace_bytes.restype = C.c_size_t
+        L.hva_state_bytes.restype = C.c_size_t
+        _lib = L
+    return _lib
+
+
+class HvaError(RuntimeError):
+    pass
+
+
+def _check(rc):
+    if rc != 0:
+        raise HvaError(f"hva error {rc}: {lib().hva_strerror(rc).decode()}")
+
+
+def _p(t):
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    if not torch.cuda.is_available():
+        raise HvaError("no CUDA device: the hva path has no CPU fallback")
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _i3(v):
+    return (C.c_int32 * 3)(*[int(x) for x in v])
+
+
+def make_shape(wl_or_dims, heads=None, dtype=None) -> hva_shape:
+    if isinstance(wl_or_dims, Workload):
+        w = wl_or_dims
+        return hva_shape(w.B, w.heads if heads is None else heads, w.T, w.H, w.W, w.D,
+                         HVA_F32 if w.dtype == "f32" else HVA_BF16)
+    B, h, T, H, W, D = wl_or_dims
+    return hva_shape(B, h, T, H, W, D, HVA_F32 if dtype in ("f32", torch.float32) else HVA_BF16)
+
+
+def make_config(wl: Workload, top_p=None, merge_rounds=None, subset_frac=0.0, refresh_all=0, min_kc=0.0,
+                max_q_tiles=0) -> hva_config:
+    c = hva_config()
+    c.cell_q = _i3(wl.cell); c.cell_k = _i3(wl.cell); c.win_q = _i3(wl.win); c.win_k = _i3(wl.win)
+    c.iters = wl.iters; c.tile_q, c.tile_k = wl.tile
+    c.top_p = wl.top_p if top_p is None else top_p
+    c.min_kc = min_kc
+    c.merge_rounds = wl.merge_rounds if merge_rounds is None else merge_rounds
+    c.max_q_tiles = max_q_tiles; c.seed = wl.seed; c.subset_frac = subset_frac
+    c.hybrid_refresh_all = refresh_all; c.softmax_scale = 0.0
+    return c
+
+
+def _ws(nbytes, device="cuda"):
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def hva_num_clusters(shape, cell):
+    return lib().hva_num_clusters(C.byref(shape), _i3(cell))
+
+
+def hva_workspace_bytes(shape, cfg):
+    return lib().hva_workspace_bytes(C.byref(shape), C.byref(cfg))
+
+
+def hva_state_bytes(shape, cfg):
+    return lib().hva_state_bytes(C.byref(shape), C.byref(cfg))
+
+
+def hva_plan_describe(BH, n, Nq, Nk, tile_q) -> hva_plan_layout:
+    L = hva_plan_layout()
+    _check(lib().hva_plan_describe(BH, n, Nq, Nk, tile_q, C.byref(L)))
+    return L
+
+
+def hva_cluster(shape, cell, win, iters, X, mu_init=None, want_sums=True, want_lowe=True):
+    """-> dict(assign [BH,n] i32, mu [BH,Nc,D] f32, sizes [BH,Nc] i32, sums, lowe)."""
+    BH, n, D = shape.B * shape.heads, shape.T * shape.H * shape.W, shape.D
+    Nc = hva_num_clusters(shape, cell)
+    K = [-(-d // k) for d, k in zip((shape.T, shape.H, shape.W), cell)]
+    nwin = math.prod(min(w, k) for w, k in zip(win, K))
+    dev = X.device
+    out = dict(assign=torch.empty((BH, n), dtype=torch.int32, device=dev),
+               mu=torch.empty((BH, Nc, D), dtype=torch.float32, device=dev),
+               sizes=torch.empty((BH, Nc), dtype=torch.int32, device=dev),
+               sums=torch.empty((BH, Nc, D), dtype=torch.float32, device=dev) if want_sums else None,
+               lowe=torch.empty((BH, n), dtype=torch.float32, device=dev) if want_lowe else None)
+    ws = _ws(BH * Nc * nwin * (D * 4 + 4) + 1024, dev)
+    _check(lib().hva_cluster(C.byref(shape), _i3(cell), _i3(win), int(iters), _p(X), _p(mu_init), _p(out["assign"]),
+                             _p(out["mu"]), _p(out["sizes"]), _p(out["sums"]), _p(out["lowe"]), _p(ws),
+                             C.c_size_t(ws.numel()), _stream()))
+    return out
+
+
+def hva_select_subset(lowe, m):
+    BH, n = lowe.shape
+    subset = torch.empty((BH, m), dtype=torch.int32, device=lowe.device)
+    _check(lib().hva_select_subset(BH, n, _p(lowe), int(m), _p(subset), C.c_void_p(0), C.c_size_t(0), _stream()))
+    return subset
+
+
+def hva_cluster_update(shape, X, subset, assign, mu, sums, sizes, refresh_all=0):
+    """In place on assign / mu / sums / sizes."""
+    BH, m = subset.shape
+    ws = _ws(BH * max(m, 1) * 8 + 512, X.device)
+    _check(lib().hva_cluster_update(C.byref(shape), mu.shape[1], _p(X), _p(subset), int(m), int(refresh_all), _p(assign),
+                                    _p(mu), _p(sums), _p(sizes), _p(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def hva_build_mask(mu_q, mu_k, sizes_k, scale, top_p, min_kc=0.0):
+    BH, Nq, D = mu_q.shape
+    Nk = mu_k.shape[1]
+    mask = torch.empty((BH, Nq, Nk), dtype=torch.uint8, device=mu_q.device)
+    _check(lib().hva_build_mask(BH, Nq, Nk, D, _p(mu_q), _p(mu_k), _p(sizes_k), C.c_float(scale), C.c_float(top_p),
+                                C.c_float(min_kc), _p(mask), C.c_void_p(0), C.c_size_t(0), _stream()))
+    return mask
+
+
+def hva_merge(sizes_q, sizes_k, mask, tile_q, tile_k, rounds, seed=0, max_q_tiles=0):
+    BH, Nq, Nk = mask.shape
+    dev = mask.device
+    group_of = torch.empty((BH, Nq), dtype=torch.int32, device=dev)
+    n_groups = torch.empty((BH,), dtype=torch.int32, device=dev)
+    gmask = torch.empty((BH, Nq, Nk), dtype=torch.uint8, device=dev)
+    ws = _ws(BH * Nq * ((Nk + 31) // 32) * 4 + 6 * (BH * Nq * 8 + 256) + 4096, dev)
+    _check(lib().hva_merge(BH, Nq, Nk, _p(sizes_q), _p(sizes_k), _p(mask), int(tile_q), int(tile_k), int(rounds),
+                           int(max_q_tiles), C.c_uint32(seed), _p(group_of), _p(n_groups), _p(gmask), _p(ws),
+                           C.c_size_t(ws.numel()), _stream()))
+    return group_of, n_groups, gmask
+
+
+class Plan:
+    """Opaque device plan buffer + typed views of its arrays."""
+
+    def __init__(self, buf, L, BH, n, Nq, Nk):
+        self.buf, self.L, self.BH, self.n, self.Nq, self.Nk = buf, L, BH, n, Nq, Nk
+
+    def _view(self, off, shape, dtype=torch.int32):
+        nb = int(math.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+        return self.buf[off:off + nb].view(dtype).view(*shape)
+
+    def __getattr__(self, k):
+        L, BH, n, Nq, Nk = self.L, self.BH, self.n, self.Nq, self.Nk
+        shapes = dict(perm_q=(BH, n), inv_perm_q=(BH, n), perm_k=(BH, n), koff=(BH, Nk + 1), n_groups=(BH,),
+                      gid=(BH, Nq), goff=(BH, Nq + 1), kappa=(BH, Nq), run_cnt=(BH, Nq),
+                      runs=(BH, Nq, L.run_stride), work_cnt=(BH,), work=(BH, L.work_cap))
+        if k in shapes:
+            return self._view(getattr(L, k), shapes[k])
+        if k == "stats":
+            return self._view(L.stats, (BH, 7), torch.int64)   # hva_stats = 2 x int32 + 6 x int64 = 7 words
+        raise AttributeError(k)
+
+    def stats_dicts(self):
+        raw = self.stats.cpu().numpy()
+        out = []
+        for r in raw:
+            out.append(dict(n_groups=int(r[0] & 0xffffffff), q_tiles=int(r[0] >> 32), q_rows_valid=int(r[1]),
+                            q_rows_padded=int(r[2]), k_cols_valid=int(r[3]), k_cols_padded=int(r[4]),
+                            tiles_executed=int(r[5]), pairs_valid=int(r[6])))
+        return out
+
+
+def hva_build_plan(n, assign_q, assign_k, sizes_q, sizes_k, group_of, n_groups, gmask, tile_q, tile_k) -> Plan:
+    BH, Nq, Nk = gmask.shape
+    dev = gmask.device
+    L = hva_plan_describe(BH, n, Nq, Nk, tile_q)
+    buf = torch.zeros(L.total, dtype=torch.uint8, device=dev)
+    ws = _ws(BH * ((n + 1023) // 1024) * max(Nq, Nk) * 4 + BH * Nq * 4 + 1024, dev)
+    _check(lib().hva_build_plan(BH, n, Nq, Nk, _p(assign_q), _p(assign_k), _p(sizes_q), _p(sizes_k), _p(group_of),
+                                _p(n_groups), _p(gmask), int(tile_q), int(tile_k), _p(buf), C.c_size_t(L.total), _p(ws),
+                                C.c_size_t(ws.numel()), _stream()))
+    return Plan(buf, L, BH, n, Nq, Nk)
+
+
+def hva_permute(shape, X, perm):
+    Y = torch.empty_like(X)
+    _check(lib().hva_permute(C.byref(shape), _p(X), _p(perm), _p(Y), _stream()))
+    return Y
+
+
+def hva_unpermute(shape, Xp, perm):
+    Y = torch.empty_like(Xp)
+    _check(lib().hva_unpermute(C.byref(shape), _p(Xp), _p(perm), _p(Y), _stream()))
+    return Y
+
+
+def hva_sparse_attention(shape, cfg, Qp, Kp, Vp, plan: Plan, unpermute=True):
+    O = torch.empty_like(Qp)
+    _check(lib().hva_sparse_attention(C.byref(shape), C.byref(cfg), _p(Qp), _p(Kp), _p(Vp), _p(plan.buf),
+                                      C.c_size_t(plan.L.total), plan.Nq, plan.Nk, _p(O), int(bool(unpermute)),
+                                      C.c_void_p(0), C.c_size_t(0), _stream()))
+    return O
+
+
+class Forward:
+    """Owns the workspace / state / stats buffers of hva_forward for one (shape, config)."""
+
+    def __init__(self, shape, cfg, device="cuda", with_state=False):
+        self.shape, self.cfg = shape, cfg
+        self.BH = shape.B * shape.heads
+        sb = hva_state_bytes(shape, cfg)
+        wb = hva_workspace_bytes(shape, cfg)
+        if wb == 0:
+            raise HvaError("invalid shape/config")
+        self.state = _ws(sb, device) if with_state else None
+        self.ws = _ws(wb - (sb if with_state else 0) + 1024, device)
+        self.stats = torch.zeros((self.BH, 7), dtype=torch.int64, device=device)
+
+    def __call__(self, Q, K, V, O=None, step_kind=HVA_ANCHOR):
+        O = torch.empty_like(Q) if O is None else O
+        _check(lib().hva_forward(C.byref(self.shape), C.byref(self.cfg), _p(Q), _p(K), _p(V), _p(O), int(step_kind),
+                                 _p(self.state), _p(self.stats), _p(self.ws), C.c_size_t(self.ws.numel()), _stream()))
+        return O
+
+    def host(self, hQ, hK, hV, hO, dev_qkvo, step_kind=HVA_ANCHOR):
+        _check(lib().hva_forward_host(C.byref(self.shape), C.byref(self.cfg), _p(hQ), _p(hK), _p(hV), _p(hO),
+                                      int(step_kind), _p(self.state), _p(dev_qkvo), _p(self.ws),
+                                      C.c_size_t(self.ws.numel()), _stream()))
+        return hO
+
+    def state_views(self):
+        """Typed views of the hybrid cache (layout of api.cu make_layout: per tensor Q then K, 256-byte aligned
+        assign[BH,n] i32, mu[BH,Nc,D] f32, sums[BH,Nc,D] f32, sizes[BH,Nc] i32, subset[BH,m] i32)."""
+        assert self.state is not None
+        s, c = self.shape, self.cfg
+        BH, n, D = self.BH, s.T * s.H * s.W, s.D
+        m = int(math.floor(float(c.subset_frac) * n + 0.5))
+        al = lambda x: (x + 255) // 256 * 256
+        out, o = {}, 0
+        for t, cell in (("q", c.cell_q), ("k", c.cell_k)):
+            Nc = hva_num_clusters(s, list(cell))
+            for name, shp, dt in (("assign", (BH, n), torch.int32), ("mu", (BH, Nc, D), torch.float32),
+                                  ("sums", (BH, Nc, D), torch.float32), ("sizes", (BH, Nc), torch.int32),
+                                  ("subset", (BH, max(m, 1)), torch.int32)):
+                nb = int(math.prod(shp)) * 4
+                out[f"{name}_{t}"] = self.state[o:o + nb].view(dt).view(*shp)
+                o += al(nb)
+        return out
+
+    def stats_dicts(self):
+        out = []
+        for r in self.stats.cpu().numpy():
+            out.append(dict(n_groups=int(r[0] & 0xffffffff), q_tiles=int(r[0] >> 32), q_rows_valid=int(r[1]),
+                            q_rows_padded=int(r[2]), k_cols_valid=int(r[3]), k_cols_padded=int(r[4]),
+                            tiles_executed=int(r[5]), pairs_valid=int(r[6])))
+        return out
+
+
+hva_forward = Forward

@@ -1,0 +1,194 @@
+// C-ABI glue: size queries, hva_sparse_attention dispatch, hva_forward orchestration (include/hva.h).
+// Stage order follows the data flow the paper implies:
+// cluster (Alg. 2) -> mask (Eq. 2-3) -> merge (Alg. 1, takes M as input l.134) -> plan/permute (Eq. 1)
+// -> attention + inverse permutation (Eq. 4).  Everything is enqueued on one stream, no host sync.
+#include "common.cuh"
+#include <cmath>
+#include <cstdlib>
+
+namespace {
+
+struct FwdLayout {
+  // persistent per-tensor state (index 0 = Q, 1 = K)
+  size_t assign[2], mu[2], sums[2], sizes[2], subset[2], state_total;
+  // per-call workspace
+  size_t lowe, mask, group_of, n_groups, group_mask, plan, qp, kp, vp, scratch, scratch_bytes, ws_total;
+  int Nq, Nk, n, BH, m;
+  hva_plan_layout PL;
+};
+
+bool valid_shape(const hva_shape* s) {
+  return s && s->B >= 1 && s->heads >= 1 && s->T >= 1 && s->H >= 1 && s->W >= 1 && (s->D == 64 || s->D == 128) &&
+         (s->dtype == HVA_F32 || s->dtype == HVA_BF16);
+}
+bool valid_config(const hva_config* c) {
+  if (!c) return false;
+  for (int a = 0; a < 3; ++a)
+    if (c->cell_q[a] < 1 || c->cell_k[a] < 1 || c->win_q[a] < 1 || c->win_k[a] < 1) return false;
+  return c->iters >= 1 && c->tile_q >= 1 && c->tile_k >= 1 && c->top_p > 0.f && c->min_kc >= 0.f && c->min_kc <= 1.f &&
+         c->merge_rounds >= 0 && c->max_q_tiles >= 0 && c->subset_frac >= 0.f && c->subset_frac <= 1.f;
+}
+
+int make_layout(const hva_shape* s, const hva_config* c, FwdLayout* F) {
+  const size_t es = s->dtype == HVA_F32 ? 4 : 2;
+  F->n = s->T * s->H * s->W; F->BH = s->B * s->heads;
+  F->Nq = hva_num_clusters(s, c->cell_q); F->Nk = hva_num_clusters(s, c->cell_k);
+  F->m = (int)std::floor((double)c->subset_frac * (double)F->n + 0.5);   // m = floor(f n + 1/2)  (R-H2)
+  const size_t BH = F->BH, n = F->n, D = s->D;
+  size_t o = 0;
+  auto take = [&](size_t b) { size_t r = o; o += hva_align(b); return r; };
+  for (int t = 0; t < 2; ++t) {
+    const size_t Nc = t ? F->Nk : F->Nq;
+    F->assign[t] = take(BH * n * 4); F->mu[t] = take(BH * Nc * D * 4); F->sums[t] = take(BH * Nc * D * 4);
+    F->sizes[t] = take(BH * Nc * 4); F->subset[t] = take(BH * (size_t)(F->m > 0 ? F->m : 1) * 4);
+  }
+  F->state_total = o;
+  const int Nqp = F->Nq > 1 ? F->Nq : 1, Nkp = F->Nk > 1 ? F->Nk : 1;
+  HVA_TRY(hva_plan_describe(F->BH, F->n, Nqp, Nkp, c->tile_q, &F->PL));
+  o = 0;
+  F->lowe = take(BH * n * 4); F->mask = take(BH * (size_t)F->Nq * F->Nk); F->group_of = take(BH * F->Nq * 4);
+  F->n_groups = take(BH * 4); F->group_mask = take(BH * (size_t)F->Nq * F->Nk); F->plan = take(F->PL.total);
+  F->qp = take(BH * n * D * es); F->kp = take(BH * n * D * es); F->vp = take(BH * n * D * es);
+  HvaGrid gq = hva_make_grid(s, c->cell_q, c->win_q), gk = hva_make_grid(s, c->cell_k, c->win_k);
+  size_t sc = hva_cluster_ws_bytes(gq, F->BH, s->D);
+  sc = std::max(sc, hva_cluster_ws_bytes(gk, F->BH, s->D));
+  sc = std::max(sc, hva_merge_ws_bytes(F->BH, F->Nq, F->Nk));
+  sc = std::max(sc, hva_plan_ws_bytes(F->BH, F->n, F->Nq, F->Nk));
+  sc = std::max(sc, hva_hybrid_ws_bytes(F->BH, F->n, std::max(F->Nq, F->Nk), F->m, s->D));
+  F->scratch_bytes = sc; F->scratch = take(sc);
+  F->ws_total = o;
+  return HVA_OK;
+}
+
+}  // namespace
+
+extern "C" const char* hva_strerror(int code) {
+  switch (code) {
+    case HVA_OK: return "ok";
+    case HVA_EINVAL: return "invalid argument";
+    case HVA_EWORKSPACE: return "workspace / plan / state buffer too small";
+    case HVA_EUNSUPPORTED: return "unsupported dtype / tile / size combination";
+    case HVA_ECUDA: return "CUDA runtime error";
+    default: return "unknown error";
+  }
+}
+extern "C" int hva_version(void) { return 100; }
+
+extern "C" int32_t hva_num_clusters(const hva_shape* s, const int32_t cell[3]) {
+  if (!s || !cell || cell[0] < 1 || cell[1] < 1 || cell[2] < 1) return HVA_EINVAL;
+  return ((s->T + cell[0] - 1) / cell[0]) * ((s->H + cell[1] - 1) / cell[1]) * ((s->W + cell[2] - 1) / cell[2]);
+}
+
+extern "C" size_t hva_workspace_bytes(const hva_shape* s, const hva_config* c) {
+  if (!valid_shape(s) || !valid_config(c)) return 0;
+  FwdLayout F;
+  if (make_layout(s, c, &F) != HVA_OK) return 0;
+  // without a caller-provided state buffer the per-tensor arrays also live in the workspace
+  return F.ws_total + F.state_total;
+}
+extern "C" size_t hva_state_bytes(const hva_shape* s, const hva_config* c) {
+  if (!valid_shape(s) || !valid_config(c)) return 0;
+  FwdLayout F;
+  if (make_layout(s, c, &F) != HVA_OK) return 0;
+  return F.state_total;
+}
+
+extern "C" int hva_sparse_attention(const hva_shape* s, const hva_config* c, const void* Qp, const void* Kp, const void* Vp,
+                                    const void* plan, size_t plan_bytes, int32_t Nq, int32_t Nk, void* O,
+                                    int32_t unpermute, void* ws, size_t ws_bytes, void* stream) {
+  (void)ws; (void)ws_bytes;
+  if (!valid_shape(s) || !valid_config(c) || !Qp || !Kp || !Vp || !plan || !O || Nq < 1 || Nk < 1) return HVA_EINVAL;
+  const int n = s->T * s->H * s->W, BH = s->B * s->heads;
+  hva_plan_layout L;
+  HVA_TRY(hva_plan_describe(BH, n, Nq, Nk, c->tile_q, &L));
+  if (plan_bytes < L.total) return HVA_EWORKSPACE;
+  const float scale = c->softmax_scale > 0.f ? c->softmax_scale : 1.0f / sqrtf((float)s->D);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const char* force = getenv("HVA_ATTN_SIMT");
+  const bool tc_ok = s->dtype == HVA_BF16 && s->D == 128 && c->tile_q == 128 && c->tile_k == 128;
+  if (tc_ok && !(force && force[0] == '1')) return hva_attention_tc_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st);
+  return hva_attention_simt_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st, c->tile_q);
+}
+
+extern "C" int hva_forward(const hva_shape* s, const hva_config* c, const void* Q, const void* K, const void* V, void* O,
+                           int32_t step_kind, void* state, hva_stats* stats_out, void* ws, size_t ws_bytes, void* stream) {
+  if (!valid_shape(s) || !valid_config(c) || !Q || !K || !V || !O || !ws) return HVA_EINVAL;
+  if (step_kind != HVA_ANCHOR && step_kind != HVA_INTERMEDIATE && step_kind != HVA_DENSE) return HVA_EINVAL;
+  if (step_kind == HVA_INTERMEDIATE && (!state || c->subset_frac <= 0.f)) return HVA_EINVAL;
+  FwdLayout F;
+  HVA_TRY(make_layout(s, c, &F));
+  if (ws_bytes < F.ws_total + (state ? 0 : F.state_total)) return HVA_EWORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  char* w = reinterpret_cast<char*>(ws);
+  char* sb = state ? reinterpret_cast<char*>(state) : w + F.ws_total;
+  void* plan = w + F.plan;
+  const int BH = F.BH, n = F.n;
+
+  if (step_kind == HVA_DENSE) {   // full attention (warm-up steps / layers, l.324): one group, one key run
+    hva_plan_layout L;
+    HVA_TRY(hva_plan_describe(BH, n, 1, 1, c->tile_q, &L));
+    HVA_TRY(hva_attention_dense_plan(BH, n, c->tile_q, plan, L, st));
+    HVA_TRY(hva_sparse_attention(s, c, Q, K, V, plan, L.total, 1, 1, O, 0, nullptr, 0, stream));
+    if (stats_out && cudaMemcpyAsync(stats_out, (char*)plan + L.stats, sizeof(hva_stats) * BH, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+      return HVA_ECUDA;
+    return HVA_OK;
+  }
+
+  const void* X[2] = {Q, K};
+  const int32_t* cell[2] = {c->cell_q, c->cell_k};
+  const int32_t* win[2] = {c->win_q, c->win_k};
+  const int Nc[2] = {F.Nq, F.Nk};
+  const bool hybrid = c->subset_frac > 0.f && state != nullptr && F.m > 0;
+  for (int t = 0; t < 2; ++t) {
+    int32_t* assign = (int32_t*)(sb + F.assign[t]);
+    float* mu = (float*)(sb + F.mu[t]);
+    float* sums = (float*)(sb + F.sums[t]);
+    int32_t* sizes = (int32_t*)(sb + F.sizes[t]);
+    int32_t* subset = (int32_t*)(sb + F.subset[t]);
+    if (step_kind == HVA_ANCHOR) {
+      float* lowe = hybrid ? (float*)(w + F.lowe) : nullptr;
+      HVA_TRY(hva_cluster(s, cell[t], win[t], c->iters, X[t], nullptr, assign, mu, sizes, sums, lowe, w + F.scratch,
+                          F.scratch_bytes, stream));
+      if (hybrid) HVA_TRY(hva_select_subset(BH, n, lowe, F.m, subset, w + F.scratch, F.scratch_bytes, stream));
+    } else {
+      HVA_TRY(hva_cluster_update(s, Nc[t], X[t], subset, F.m, c->hybrid_refresh_all, assign, mu, sums, sizes,
+                                 w + F.scratch, F.scratch_bytes, stream));
+    }
+  }
+  const float scale = c->softmax_scale > 0.f ? c->softmax_scale : 1.0f / sqrtf((float)s->D);
+  uint8_t* mask = (uint8_t*)(w + F.mask);
+  uint8_t* gmask = (uint8_t*)(w + F.group_mask);
+  int32_t* group_of = (int32_t*)(w + F.group_of);
+  int32_t* n_groups = (int32_t*)(w + F.n_groups);
+  HVA_TRY(hva_build_mask(BH, F.Nq, F.Nk, s->D, (float*)(sb + F.mu[0]), (float*)(sb + F.mu[1]), (int32_t*)(sb + F.sizes[1]),
+                         scale, c->top_p, c->min_kc, mask, w + F.scratch, F.scratch_bytes, stream));
+  HVA_TRY(hva_merge(BH, F.Nq, F.Nk, (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), mask, c->tile_q, c->tile_k,
+                    c->merge_rounds, c->max_q_tiles, c->seed, group_of, n_groups, gmask, w + F.scratch, F.scratch_bytes, stream));
+  HVA_TRY(hva_build_plan(BH, n, F.Nq, F.Nk, (int32_t*)(sb + F.assign[0]), (int32_t*)(sb + F.assign[1]),
+                         (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), group_of, n_groups, gmask, c->tile_q,
+                         c->tile_k, plan, F.PL.total, w + F.scratch, F.scratch_bytes, stream));
+  const char* pb = reinterpret_cast<const char*>(plan);
+  HVA_TRY(hva_permute(s, Q, (const int32_t*)(pb + F.PL.perm_q), w + F.qp, stream));
+  HVA_TRY(hva_permute(s, K, (const int32_t*)(pb + F.PL.perm_k), w + F.kp, stream));
+  HVA_TRY(hva_permute(s, V, (const int32_t*)(pb + F.PL.perm_k), w + F.vp, stream));
+  HVA_TRY(hva_sparse_attention(s, c, w + F.qp, w + F.kp, w + F.vp, plan, F.PL.total, F.Nq, F.Nk, O, 1, nullptr, 0, stream));
+  if (stats_out && cudaMemcpyAsync(stats_out, pb + F.PL.stats, sizeof(hva_stats) * BH, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+    return HVA_ECUDA;
+  return HVA_OK;
+}
+
+extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const void* hQ, const void* hK, const void* hV,
+                                void* hO, int32_t step_kind, void* state, void* dev_qkvo, void* ws, size_t ws_bytes,
+                                void* stream) {
+  if (!valid_shape(s) || !hQ || !hK || !hV || !hO || !dev_qkvo) return HVA_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const size_t bytes = (size_t)s->B * s->heads * s->T * s->H * s->W * s->D * (s->dtype == HVA_F32 ? 4 : 2);
+  char* d = reinterpret_cast<char*>(dev_qkvo);
+  if (cudaMemcpyAsync(d, hQ, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
+  if (cudaMemcpyAsync(d + bytes, hK, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
+  if (cudaMemcpyAsync(d + 2 * bytes, hV, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
+  HVA_TRY(hva_forward(s, c, d, d + bytes, d + 2 * bytes, d + 3 * bytes, step_kind, state, nullptr, ws, ws_bytes, stream));
+  if (cudaMemcpyAsync(hO, d + 3 * bytes, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return HVA_ECUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return HVA_ECUDA;
+  return HVA_OK;
+}

@@ -1,0 +1,455 @@
+// S9 (+S10), tensor-core variant for bf16, D = 128, 128x128 tiles (sm_100a only):
+// block-sparse FlashAttention over the plan's packed key runs (Eq. 4 l.56; packed key
+// blocks l.109; union masks Eq. 8 l.115).
+//
+// One CTA per (group, q-tile) work item.  Warp roles:
+//   warps 0-3  softmax / correction / epilogue: thread i owns query row i == TMEM lane i
+//   warp  4    TMA producer: Q tile once, then per packed key tile the K and V rows of the group's
+//              key runs, as power-of-two-height boxes of a 128B-swizzled 2-D tensor map, packed
+//              back to back in the stage buffer (exact packing across cluster boundaries)
+//   warp  5    TMEM allocator + single-thread tcgen05.mma issuer
+// Per key tile j:  S_j = Q K_j^T (SS MMA, K-major operands, fp32 accumulators in TMEM, two S buffers)
+//                  P_j = exp2(S_j*scale*log2e - m) written back over S_j as bf16 (tcgen05.st)
+//                  O  += P_j V_j (TS MMA: A = P from TMEM, B = V from smem, MN-major)
+// with lazy (thresholded) rescaling of O in TMEM, 1/l normalisation and the inverse permutation
+// fused into the epilogue's row stores.
+#include "common.cuh"
+#include <cuda.h>
+#include <cstdlib>
+
+namespace {
+
+constexpr int kBM = 128, kBN = 128, kD = 128;
+constexpr int kHalfBytes = 128 * 128;          // one 64-dim half of a 128-row tile: 128 rows x 128 B
+constexpr int kTileBytes = 2 * kHalfBytes;     // 32 KB
+constexpr int kStages = 2;
+constexpr int kThreadsTC = 192;
+constexpr int kNumBoxes = 8;                   // box heights 1,2,4,...,128
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO = 256;
+constexpr float kRescaleThreshold = 8.0f;      // log2 units
+
+struct TcMaps {
+  CUtensorMap q;
+  CUtensorMap k[kNumBoxes];
+  CUtensorMap v[kNumBoxes];
+};
+
+struct TcParams {
+  int n, Nq, Nk, run_stride, work_cap, unpermute;
+  float scale_log2;
+  const int *goff, *koff, *kappa, *run_cnt, *work_cnt, *work, *perm_q;
+  const uint32_t* runs;
+  __nv_bfloat16* O;
+};
+
+// ------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(const CUtensorMap* map, uint64_t* bar, void* dst, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]
+__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]
+__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+      "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+      "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
+      "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
+      "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+      "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+
+// UMMA shared-memory descriptor (sm_100): start address, LBO, SBO in 16-byte units, version = 1
+// (bit 46), layout SWIZZLE_128B = 2 (bits 61-63).
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  return (uint64_t)((saddr & 0x3FFFF) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
+         (1ull << 46) | (2ull << 61);
+}
+// instruction descriptor: D = F32, A = B = BF16, M = 128, N = 128; b_major selects MN-major B
+__device__ __forceinline__ uint32_t umma_idesc(uint32_t b_mn_major) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | (b_mn_major << 16) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+}
+
+struct __align__(8) TcBarriers {
+  uint64_t q_full, k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages], s_full[2], p_ready[2], o_done;
+  uint32_t tmem_base;
+};
+
+constexpr size_t kSmemTC = 1024 + kTileBytes * (1 + 2 * kStages) + sizeof(TcBarriers);
+
+// Walks the group's key runs (maximal runs of consecutive selected key clusters, contiguous in K')
+// and packs them back to back into 128-row tiles (l.109).
+struct RunWalker {
+  const uint32_t* runs; const int* koff; int nrun, r, row0, len, used;
+  __device__ void load() {
+    if (r < nrun) { uint32_t rr = runs[r]; row0 = koff[rr & 0xffff]; len = koff[(rr >> 16) + 1] - row0; }
+    else { len = 1 << 30; }   // past the last run: only reached for the finite over-read padding rows
+    used = 0;
+  }
+};
+
+__device__ __forceinline__ void emit_boxes(const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int grow, int dst, int len) {
+#pragma unroll 1
+  for (int b = kNumBoxes - 1; b >= 0; --b) {
+    const int h = 1 << b;
+    if (len & h) {
+      tma_load_2d(maps + b, bar, stage + dst * 128, 0, grow);
+      tma_load_2d(maps + b, bar, stage + kHalfBytes + dst * 128, 64, grow);
+      grow += h; dst += h;
+    }
+  }
+}
+
+__device__ __forceinline__ void load_tile(RunWalker& w, const CUtensorMap* maps, uint64_t* bar, unsigned char* stage,
+                                          int base_row, int rows_valid, int rows_load) {
+  int dst = 0;
+  while (dst < rows_valid) {
+    while (w.used == w.len) { ++w.r; w.load(); }
+    int seg = min(w.len - w.used, rows_valid - dst);
+    emit_boxes(maps, bar, stage, base_row + w.row0 + w.used, dst, seg);
+    w.used += seg; dst += seg;
+  }
+  if (rows_load > rows_valid)   // ragged last tile: round up to the MMA K granule with finite over-read rows
+    emit_boxes(maps, bar, stage, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
+}
+
+__global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid_constant__ TcMaps maps, TcParams p) {
+  const int bh = blockIdx.y;
+  if ((int)blockIdx.x >= p.work_cnt[bh]) return;
+  const uint32_t wi = (uint32_t)p.work[(size_t)bh * p.work_cap + blockIdx.x];
+  const int g = wi & 0xffff, t = wi >> 16;
+  const int* goff = p.goff + (size_t)bh * (p.Nq + 1);
+  const int row0 = goff[g] + t * kBM, row1 = min(goff[g + 1], row0 + kBM);
+  const int kappa = p.kappa[(size_t)bh * p.Nq + g];
+  const int jn = (kappa + kBN - 1) / kBN;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int base_row = bh * p.n;
+
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  unsigned char* sQ = smem;
+  unsigned char* sK = smem + kTileBytes;
+  unsigned char* sV = smem + kTileBytes * (1 + kStages);
+  TcBarriers* B = reinterpret_cast<TcBarriers*>(smem + kTileBytes * (1 + 2 * kStages));
+
+  if (jn == 0) {   // no key selected: defined as a zero row
+    if (tid < kBM && row0 + tid < row1) {
+      size_t orow = (size_t)base_row + (p.unpermute ? p.perm_q[(size_t)base_row + row0 + tid] : row0 + tid);
+      uint4 z = make_uint4(0, 0, 0, 0);
+      for (int c = 0; c < 16; ++c) reinterpret_cast<uint4*>(p.O + orow * kD)[c] = z;
+    }
+    return;
+  }
+
+  if (tid == 0) {
+    mbar_init(&B->q_full, 1);
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(&B->k_full[s], 1); mbar_init(&B->k_empty[s], 1);
+      mbar_init(&B->v_full[s], 1); mbar_init(&B->v_empty[s], 1);
+    }
+    for (int b = 0; b < 2; ++b) { mbar_init(&B->s_full[b], 1); mbar_init(&B->p_ready[b], 128); }
+    mbar_init(&B->o_done, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  if (warp == 5) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&B->tmem_base)), "r"(kTmemCols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = B->tmem_base;
+
+  if (warp == 4) {
+    // ===================================================== TMA producer
+    if (lane == 0) {
+      mbar_expect_tx(&B->q_full, kTileBytes);
+      tma_load_2d(&maps.q, &B->q_full, sQ, 0, base_row + row0);
+      tma_load_2d(&maps.q, &B->q_full, sQ + kHalfBytes, 64, base_row + row0);
+      RunWalker wk{p.runs + ((size_t)bh * p.Nq + g) * p.run_stride, p.koff + (size_t)bh * (p.Nk + 1),
+                   p.run_cnt[(size_t)bh * p.Nq + g], 0, 0, 0, 0};
+      wk.load();
+      RunWalker wv = wk;
+      for (int j = 0; j < jn; ++j) {
+        const int s = j % kStages, use = j / kStages;
+        const int rows_valid = min(kBN, kappa - j * kBN);
+        const int rows_load = rows_valid == kBN ? kBN : (rows_valid + 15) & ~15;
+        if (use > 0) mbar_wait(&B->k_empty[s], (use - 1) & 1);
+        mbar_expect_tx(&B->k_full[s], rows_load * 256);
+        load_tile(wk, maps.k, &B->k_full[s], sK + s * kTileBytes, base_row, rows_valid, rows_load);
+        if (use > 0) mbar_wait(&B->v_empty[s], (use - 1) & 1);
+        mbar_expect_tx(&B->v_full[s], rows_load * 256);
+        load_tile(wv, maps.v, &B->v_full[s], sV + s * kTileBytes, base_row, rows_valid, rows_load);
+      }
+    }
+  } else if (warp == 5) {
+    // ===================================================== MMA issuer (one thread)
+    if (lane == 0) {
+      const uint32_t idesc_qk = umma_idesc(0), idesc_pv = umma_idesc(1);
+      const uint32_t q_addr = smem_u32(sQ), k_addr = smem_u32(sK), v_addr = smem_u32(sV);
+      auto issue_qk = [&](int j) {
+        const int s = j % kStages;
+        mbar_wait(&B->k_full[s], (j / kStages) & 1);
+        tc_fence_after();
+        const uint32_t d = tmem + ((j & 1) ? kColS1 : kColS0);
+#pragma unroll
+        for (int ks = 0; ks < kD / 16; ++ks) {
+          const uint32_t off = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
+          mma_ss(d, umma_desc(q_addr + off, 16, 1024), umma_desc(k_addr + s * kTileBytes + off, 16, 1024), idesc_qk, ks > 0);
+        }
+        tc_commit(&B->s_full[j & 1]);
+        tc_commit(&B->k_empty[s]);
+      };
+      mbar_wait(&B->q_full, 0);
+      issue_qk(0);
+      for (int j = 0; j < jn; ++j) {
+        if (j + 1 < jn) issue_qk(j + 1);
+        const int s = j % kStages;
+        mbar_wait(&B->p_ready[j & 1], (j >> 1) & 1);
+        mbar_wait(&B->v_full[s], (j / kStages) & 1);
+        tc_fence_after();
+        const int rows_valid = min(kBN, kappa - j * kBN);
+        const int ksteps = (rows_valid + 15) >> 4;
+        const uint32_t a = tmem + ((j & 1) ? kColS1 : kColS0);
+        for (int ks = 0; ks < ksteps; ++ks)
+          mma_ts(tmem + kColO, a + ks * 8, umma_desc(v_addr + s * kTileBytes + ks * 2048, kHalfBytes, 1024), idesc_pv,
+                 (j > 0 || ks > 0));
+        tc_commit(&B->v_empty[s]);
+        tc_commit(&B->o_done);
+      }
+    }
+  } else {
+    // ===================================================== softmax / correction / epilogue (thread = row)
+    const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+    const float sl2 = p.scale_log2;
+    float m_ref = -INFINITY, l = 0.f;
+    uint32_t v[32];
+    for (int j = 0; j < jn; ++j) {
+      const int b = j & 1;
+      const uint32_t s_addr = tmem + lane_base + (b ? kColS1 : kColS0);
+      const int rows_valid = min(kBN, kappa - j * kBN);
+      mbar_wait(&B->s_full[b], (j >> 1) & 1);
+      tc_fence_after();
+      float mx = -INFINITY;
+#pragma unroll 1
+      for (int c = 0; c < 4; ++c) {
+        tmem_ld32(s_addr + c * 32, v);
+        if (rows_valid == kBN) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(v[i]));
+        } else {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) mx = fmaxf(mx, (c * 32 + i < rows_valid) ? __uint_as_float(v[i]) : -INFINITY);
+        }
+      }
+      const float m_new = fmaxf(m_ref, mx * sl2);
+      if (__any_sync(0xffffffffu, m_new - m_ref > kRescaleThreshold)) {   // lazy rescale, warp-uniform
+        if (j > 0) {
+          mbar_wait(&B->o_done, (j - 1) & 1);
+          tc_fence_after();
+          const float f = ex2(m_ref - m_new);
+          l *= f;
+#pragma unroll 1
+          for (int c = 0; c < 4; ++c) {
+            tmem_ld32(tmem + lane_base + kColO + c * 32, v);
+#pragma unroll
+            for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) * f);
+            tmem_st32(tmem + lane_base + kColO + c * 32, v);
+          }
+        }
+        m_ref = m_new;
+      }
+#pragma unroll 1
+      for (int c = 0; c < 4; ++c) {
+        tmem_ld32(s_addr + c * 32, v);
+        uint32_t pk[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          float p0 = ex2(fmaf(__uint_as_float(v[2 * i]), sl2, -m_ref));
+          float p1 = ex2(fmaf(__uint_as_float(v[2 * i + 1]), sl2, -m_ref));
+          if (rows_valid != kBN) {
+            p0 = (c * 32 + 2 * i < rows_valid) ? p0 : 0.f;
+            p1 = (c * 32 + 2 * i + 1 < rows_valid) ? p1 : 0.f;
+          }
+          l += p0 + p1;
+          pk[i] = pack_bf16(p0, p1);
+        }
+        tmem_st16(s_addr + c * 16, pk);
+      }
+      tmem_st_wait();
+      tc_fence_before();
+      mbar_arrive(&B->p_ready[b]);
+    }
+    // epilogue: O / l, bf16, row store with the inverse permutation fused (Eq. 4: O = Pi^{q-1} O')
+    mbar_wait(&B->o_done, (jn - 1) & 1);
+    tc_fence_after();
+    const float inv = 1.f / l;
+    const int row = row0 + tid;
+    const bool ok = row < row1;
+    size_t orow = 0;
+    if (ok) orow = (size_t)base_row + (p.unpermute ? p.perm_q[(size_t)base_row + row] : row);
+#pragma unroll 1
+    for (int c = 0; c < 4; ++c) {
+      tmem_ld32(tmem + lane_base + kColO + c * 32, v);
+      if (ok) {
+        uint4* dst = reinterpret_cast<uint4*>(p.O + orow * kD + c * 32);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          uint4 o;
+          o.x = pack_bf16(__uint_as_float(v[8 * q + 0]) * inv, __uint_as_float(v[8 * q + 1]) * inv);
+          o.y = pack_bf16(__uint_as_float(v[8 * q + 2]) * inv, __uint_as_float(v[8 * q + 3]) * inv);
+          o.z = pack_bf16(__uint_as_float(v[8 * q + 4]) * inv, __uint_as_float(v[8 * q + 5]) * inv);
+          o.w = pack_bf16(__uint_as_float(v[8 * q + 6]) * inv, __uint_as_float(v[8 * q + 7]) * inv);
+          dst[q] = o;
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 5) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
+  }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      return nullptr;
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// 2-D map over X[rows, 128] bf16, box = 64 dims x box_rows rows, 128-byte swizzle, OOB rows read as zero.
+bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint32_t box_rows) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return false;
+  cuuint64_t dims[2] = {(cuuint64_t)kD, rows};
+  cuuint64_t strides[1] = {(cuuint64_t)kD * 2};
+  cuuint32_t box[2] = {64, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+int hva_attention_tc_launch(const hva_shape* s, float scale, const void* Qp, const void* Kp, const void* Vp,
+                            const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute,
+                            cudaStream_t st) {
+  if (s->D != kD || s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
+  const int n = s->T * s->H * s->W, BH = s->B * s->heads;
+  const uint64_t rows = (uint64_t)BH * n;
+  if (rows >= (1ull << 31)) return HVA_EUNSUPPORTED;
+  TcMaps maps;
+  if (!make_map(&maps.q, Qp, rows, kBM)) return HVA_ECUDA;
+  for (int b = 0; b < kNumBoxes; ++b) {
+    if (!make_map(&maps.k[b], Kp, rows, 1u << b)) return HVA_ECUDA;
+    if (!make_map(&maps.v[b], Vp, rows, 1u << b)) return HVA_ECUDA;
+  }
+  const char* b = reinterpret_cast<const char*>(plan);
+  TcParams p;
+  p.n = n; p.Nq = Nq; p.Nk = Nk; p.run_stride = (int)L.run_stride; p.work_cap = (int)L.work_cap; p.unpermute = unpermute;
+  p.scale_log2 = scale * 1.4426950408889634f;
+  p.goff = (const int*)(b + L.goff); p.koff = (const int*)(b + L.koff); p.kappa = (const int*)(b + L.kappa);
+  p.run_cnt = (const int*)(b + L.run_cnt); p.work_cnt = (const int*)(b + L.work_cnt); p.work = (const int*)(b + L.work);
+  p.perm_q = (const int*)(b + L.perm_q); p.runs = (const uint32_t*)(b + L.runs);
+  p.O = reinterpret_cast<__nv_bfloat16*>(O);
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(hva_attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemTC) != cudaSuccess)
+      return HVA_ECUDA;
+    attr_set = true;
+  }
+  dim3 grid((unsigned)L.work_cap, BH);
+  hva_attn_tc_kernel<<<grid, kThreadsTC, kSmemTC, st>>>(maps, p);
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
+}

@@ -1,0 +1,280 @@
+// S0-S2 (+A4): 3D local-window k-means (Alg. 2, l.346-388; Eq. 5 l.81; Eq. 6 l.97).
+//
+// v1 layout: one CTA per home cell.  The cell's window centroids (fp32) and the cell's tokens are
+// staged in shared memory; one thread per token evaluates the direct form sum_c (x_c - mu_c)^2 in
+// fp32 for every window candidate (ascending centroid id, strict '<' => first minimum, R-C1) and
+// keeps the best / second best (Eq. 6).  Tokens are then counting-sorted by target slot and each
+// thread (= one feature dim) adds its column in token order: a deterministic segmented per-cell
+// reduction with no atomics.  The per-(cell, slot) partial sums are combined per centroid, in a
+// fixed cell order, by hva_finalize_kernel (Alg. 2 line 23: mu <- z/n, empty keeps mu).
+#include "common.cuh"
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr int kCB = 9;  // candidates evaluated per register block
+
+__device__ __forceinline__ void load8(const float* p, float x[8]) {
+  float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
+  x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y; x[6] = b.z; x[7] = b.w;
+}
+__device__ __forceinline__ void load8(const __nv_bfloat16* p, float x[8]) {
+  uint4 r = *reinterpret_cast<const uint4*>(p);  // bf16 -> fp32 is a 16-bit shift (exact)
+  x[0] = __uint_as_float(r.x << 16); x[1] = __uint_as_float(r.x & 0xffff0000u);
+  x[2] = __uint_as_float(r.y << 16); x[3] = __uint_as_float(r.y & 0xffff0000u);
+  x[4] = __uint_as_float(r.z << 16); x[5] = __uint_as_float(r.z & 0xffff0000u);
+  x[6] = __uint_as_float(r.w << 16); x[7] = __uint_as_float(r.w & 0xffff0000u);
+}
+
+struct ClusterParams {
+  HvaGrid g;
+  int BH;
+  const void* X;       // [BH, n, D]
+  const float* mu;     // [BH, Nc, D]
+  float* part;         // [BH, Nc(cells), nwin, D]
+  int* part_cnt;       // [BH, Nc(cells), nwin]
+  int* assign;         // [BH, n] or null
+  float* lowe;         // [BH, n] or null
+};
+
+template <typename T, int D>
+__global__ void __launch_bounds__(kThreads) hva_init_centroids_kernel(HvaGrid g, const T* __restrict__ X,
+                                                                      float* __restrict__ mu) {
+  // mu_u <- X[c_t, c_h, c_w, :],  c = min(u*k + floor(k/2), dim-1)   (Alg. 2 lines 7-11)
+  int u = blockIdx.x, bh = blockIdx.y;
+  int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
+  int ct = min(ut * g.kt + g.kt / 2, g.T - 1), ch = min(uh * g.kh + g.kh / 2, g.H - 1),
+      cw = min(uw * g.kw + g.kw / 2, g.W - 1);
+  size_t tok = (size_t)(ct * g.H + ch) * g.W + cw;
+  for (int c = threadIdx.x; c < D; c += blockDim.x)
+    mu[((size_t)bh * g.Nc + u) * D + c] = HvaElem<T>::ld(X + ((size_t)bh * g.n + tok) * D + c);
+}
+
+template <typename T, int D>
+__global__ void __launch_bounds__(kThreads) hva_assign_kernel(ClusterParams p) {
+  constexpr int kVec = 16 / sizeof(T);          // elements per 16-byte chunk
+  constexpr int kRowStride = D + kVec;          // padded row (elements): conflict-free 16 B row reads
+  const HvaGrid& g = p.g;
+  const int cell = blockIdx.x, bh = blockIdx.y, tid = threadIdx.x;
+  const int ut = cell / (g.Kh * g.Kw), uh = (cell / g.Kw) % g.Kh, uw = cell % g.Kw;
+  const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
+  const int ctok = g.kt * g.kh * g.kw;          // token slots of a cell (border cells: some invalid)
+
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float* s_mu = reinterpret_cast<float*>(smem_raw);                 // [nwin][D]
+  T* s_x = reinterpret_cast<T*>(s_mu + (size_t)g.nwin * D);         // [ctok][kRowStride]
+  int* s_lab = reinterpret_cast<int*>(s_x + (size_t)ctok * kRowStride);  // [ctok] slot or -1
+  int* s_cnt = s_lab + ctok;                                        // [nwin]
+  int* s_start = s_cnt + g.nwin;                                    // [nwin+1]
+  int* s_order = s_start + g.nwin + 1;                              // [ctok]
+
+  // ---- stage window centroids (ascending centroid id == delta_t-major, Alg. 2 line 18)
+  const float* mu_b = p.mu + (size_t)bh * g.Nc * D;
+  for (int i = tid; i < g.nwin * (D / 4); i += kThreads) {
+    int v = i / (D / 4), q = i % (D / 4);
+    int dt = v / (g.wh * g.ww), dh = (v / g.ww) % g.wh, dw = v % g.ww;
+    int u = ((st + dt) * g.Kh + (sh + dh)) * g.Kw + (sw + dw);
+    reinterpret_cast<float4*>(s_mu)[i] = reinterpret_cast<const float4*>(mu_b + (size_t)u * D)[q];
+  }
+  // ---- stage the cell's tokens (16-byte coalesced loads; runs of k_w consecutive tokens)
+  const T* X_b = reinterpret_cast<const T*>(p.X) + (size_t)bh * g.n * D;
+  constexpr int kChunks = D / kVec;
+  for (int i = tid; i < ctok * kChunks; i += kThreads) {
+    int li = i / kChunks, q = i % kChunks;
+    int dt = li / (g.kh * g.kw), dh = (li / g.kw) % g.kh, dw = li % g.kw;
+    int t = ut * g.kt + dt, h = uh * g.kh + dh, w = uw * g.kw + dw;
+    if (t < g.T && h < g.H && w < g.W) {
+      size_t tok = (size_t)(t * g.H + h) * g.W + w;
+      *reinterpret_cast<uint4*>(s_x + (size_t)li * kRowStride + q * kVec) =
+          __ldg(reinterpret_cast<const uint4*>(X_b + tok * D) + q);
+    }
+  }
+  __syncthreads();
+
+  // ---- one thread per token: distances to every window candidate (Eq. 5), best and second best
+  for (int li = tid; li < ctok; li += kThreads) {
+    int dt = li / (g.kh * g.kw), dh = (li / g.kw) % g.kh, dw = li % g.kw;
+    int t = ut * g.kt + dt, h = uh * g.kh + dh, w = uw * g.kw + dw;
+    bool valid = (t < g.T && h < g.H && w < g.W);
+    int lab = valid ? 0 : -1;
+    if (valid) {
+      float best = __int_as_float(0x7f800000), second = __int_as_float(0x7f800000);
+      const T* xr = s_x + (size_t)li * kRowStride;
+      for (int v0 = 0; v0 < g.nwin; v0 += kCB) {
+        float acc[kCB];
+#pragma unroll
+        for (int j = 0; j < kCB; ++j) acc[j] = 0.f;
+        for (int c0 = 0; c0 < D; c0 += 8) {
+          float x[8];
+          load8(xr + c0, x);
+#pragma unroll
+          for (int j = 0; j < kCB; ++j) {
+            int v = min(v0 + j, g.nwin - 1);
+            const float4 m0 = *reinterpret_cast<const float4*>(s_mu + (size_t)v * D + c0);
+            const float4 m1 = *reinterpret_cast<const float4*>(s_mu + (size_t)v * D + c0 + 4);
+            float d;
+            d = x[0] - m0.x; acc[j] = fmaf(d, d, acc[j]);
+            d = x[1] - m0.y; acc[j] = fmaf(d, d, acc[j]);
+            d = x[2] - m0.z; acc[j] = fmaf(d, d, acc[j]);
+            d = x[3] - m0.w; acc[j] = fmaf(d, d, acc[j]);
+            d = x[4] - m1.x; acc[j] = fmaf(d, d, acc[j]);
+            d = x[5] - m1.y; acc[j] = fmaf(d, d, acc[j]);
+            d = x[6] - m1.z; acc[j] = fmaf(d, d, acc[j]);
+            d = x[7] - m1.w; acc[j] = fmaf(d, d, acc[j]);
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < kCB; ++j) {
+          if (v0 + j < g.nwin) {
+            float dd = acc[j];
+            if (dd < best) { second = best; best = dd; lab = v0 + j; }
+            else if (dd < second) second = dd;
+          }
+        }
+      }
+      size_t tok = (size_t)(t * g.H + h) * g.W + w;
+      if (p.assign) {
+        int dtv = lab / (g.wh * g.ww), dhv = (lab / g.ww) % g.wh, dwv = lab % g.ww;
+        p.assign[(size_t)bh * g.n + tok] = ((st + dtv) * g.Kh + (sh + dhv)) * g.Kw + (sw + dwv);
+      }
+      if (p.lowe) {  // rho = d1/d2, unsquared (Eq. 6); single candidate -> 0; d2 == 0 -> 1 (R-H1)
+        float rho = (second == __int_as_float(0x7f800000)) ? 0.f : (second > 0.f ? sqrtf(best / second) : 1.f);
+        p.lowe[(size_t)bh * g.n + tok] = rho;
+      }
+    }
+    s_lab[li] = lab;
+  }
+  __syncthreads();
+
+  // ---- counting sort of the cell's tokens by slot (stable in token order)
+  for (int v = tid; v < g.nwin; v += kThreads) {
+    int c = 0;
+    for (int li = 0; li < ctok; ++li) c += (s_lab[li] == v);
+    s_cnt[v] = c;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int a = 0;
+    for (int v = 0; v < g.nwin; ++v) { s_start[v] = a; a += s_cnt[v]; }
+    s_start[g.nwin] = a;
+  }
+  __syncthreads();
+  for (int v = tid; v < g.nwin; v += kThreads) {
+    int pos = s_start[v];
+    for (int li = 0; li < ctok; ++li)
+      if (s_lab[li] == v) s_order[pos++] = li;
+  }
+  __syncthreads();
+
+  // ---- segmented per-cell reduction: thread = feature dim, tokens added in token order (z_a += x)
+  const size_t pbase = ((size_t)bh * g.Nc + cell) * g.nwin;
+  constexpr int kGroups = kThreads / D;  // 1 for D=128, 2 for D=64
+  const int c = tid % D, grp = tid / D;
+  for (int v = grp; v < g.nwin; v += kGroups) {
+    int b = s_start[v], e = s_start[v + 1];
+    if (c == 0) p.part_cnt[pbase + v] = e - b;
+    if (e > b) {
+      float acc = 0.f;
+      for (int i = b; i < e; ++i) acc += HvaElem<T>::ld(s_x + (size_t)s_order[i] * kRowStride + c);
+      p.part[(pbase + v) * D + c] = acc;
+    }
+  }
+}
+
+// mu_u <- z_u / n_u if n_u > 0 else mu_u   (Alg. 2 lines 22-23).  z_u = sum over the home cells g whose
+// window contains u of part[g][slot(u in g)], in ascending cell order (fixed => deterministic).
+template <int D>
+__global__ void __launch_bounds__(D) hva_finalize_kernel(HvaGrid g, const float* __restrict__ part,
+                                                         const int* __restrict__ part_cnt, float* __restrict__ mu,
+                                                         int* __restrict__ sizes, float* __restrict__ sums) {
+  const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
+  const int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
+  float z = 0.f;
+  int n = 0;
+  for (int gt = max(0, ut - g.wt); gt <= min(g.Kt - 1, ut + g.wt); ++gt) {
+    int st = hva_win_start(gt, g.wt, g.Kt);
+    if (ut < st || ut >= st + g.wt) continue;
+    for (int gh = max(0, uh - g.wh); gh <= min(g.Kh - 1, uh + g.wh); ++gh) {
+      int sh = hva_win_start(gh, g.wh, g.Kh);
+      if (uh < sh || uh >= sh + g.wh) continue;
+      for (int gw = max(0, uw - g.ww); gw <= min(g.Kw - 1, uw + g.ww); ++gw) {
+        int sw = hva_win_start(gw, g.ww, g.Kw);
+        if (uw < sw || uw >= sw + g.ww) continue;
+        int cell = (gt * g.Kh + gh) * g.Kw + gw;
+        int slot = ((ut - st) * g.wh + (uh - sh)) * g.ww + (uw - sw);
+        size_t idx = ((size_t)bh * g.Nc + cell) * g.nwin + slot;
+        int k = part_cnt[idx];
+        if (k > 0) { z += part[idx * D + c]; n += k; }
+      }
+    }
+  }
+  size_t o = ((size_t)bh * g.Nc + u) * D + c;
+  if (n > 0) mu[o] = __fdiv_rn(z, (float)n);
+  if (sums) sums[o] = z;
+  if (c == 0) sizes[(size_t)bh * g.Nc + u] = n;
+}
+
+size_t assign_smem_bytes(const HvaGrid& g, int D, int esize) {
+  int ctok = g.kt * g.kh * g.kw;
+  int rowstride = D + 16 / esize;
+  return (size_t)g.nwin * D * 4 + (size_t)ctok * rowstride * esize + sizeof(int) * (ctok + g.nwin + g.nwin + 1 + ctok) + 16;
+}
+
+template <typename T, int D>
+int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float* mu_init, int* assign, float* mu,
+                int* sizes, float* sums, float* lowe, float* part, int* part_cnt, cudaStream_t st) {
+  dim3 grid(g.Nc, BH);
+  size_t smem = assign_smem_bytes(g, D, sizeof(T));
+  if (smem > 227 * 1024) return HVA_EUNSUPPORTED;
+  if (cudaFuncSetAttribute(hva_assign_kernel<T, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return HVA_ECUDA;
+  if (mu_init) {
+    if (mu_init != mu &&
+        cudaMemcpyAsync(mu, mu_init, (size_t)BH * g.Nc * D * sizeof(float), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+      return HVA_ECUDA;
+  } else {
+    hva_init_centroids_kernel<T, D><<<grid, kThreads, 0, st>>>(g, reinterpret_cast<const T*>(X), mu);
+    HVA_CHECK_LAUNCH();
+  }
+  for (int it = 0; it < iters; ++it) {
+    bool last = (it == iters - 1);
+    ClusterParams p{g, BH, X, mu, part, part_cnt, last ? assign : nullptr, last ? lowe : nullptr};
+    hva_assign_kernel<T, D><<<grid, kThreads, smem, st>>>(p);
+    HVA_CHECK_LAUNCH();
+    hva_finalize_kernel<D><<<grid, D, 0, st>>>(g, part, part_cnt, mu, sizes, last ? sums : nullptr);
+    HVA_CHECK_LAUNCH();
+  }
+  return HVA_OK;
+}
+
+}  // namespace
+
+size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D) {
+  return hva_align((size_t)BH * g.Nc * g.nwin * D * sizeof(float)) + hva_align((size_t)BH * g.Nc * g.nwin * sizeof(int));
+}
+
+extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int32_t win[3], int32_t iters, const void* X,
+                           const float* mu_init, int32_t* assign, float* mu, int32_t* sizes, float* sums, float* lowe,
+                           void* ws, size_t ws_bytes, void* stream) {
+  if (!s || !cell || !win || !X || !assign || !mu || !sizes || !ws) return HVA_EINVAL;
+  if (s->B < 1 || s->heads < 1 || s->T < 1 || s->H < 1 || s->W < 1 || iters < 1) return HVA_EINVAL;
+  if (s->D != 64 && s->D != 128) return HVA_EINVAL;
+  for (int a = 0; a < 3; ++a)
+    if (cell[a] < 1 || win[a] < 1) return HVA_EINVAL;
+  if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
+  HvaGrid g = hva_make_grid(s, cell, win);
+  int BH = s->B * s->heads;
+  if (ws_bytes < hva_cluster_ws_bytes(g, BH, s->D)) return HVA_EWORKSPACE;
+  float* part = reinterpret_cast<float*>(ws);
+  int* part_cnt = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + hva_align((size_t)BH * g.Nc * g.nwin * s->D * sizeof(float)));
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+#define HVA_DISPATCH(T, DD) return run_cluster<T, DD>(g, BH, iters, X, mu_init, assign, mu, sizes, sums, lowe, part, part_cnt, st)
+  if (s->dtype == HVA_F32) {
+    if (s->D == 64) HVA_DISPATCH(float, 64);
+    HVA_DISPATCH(float, 128);
+  } else {
+    if (s->D == 64) HVA_DISPATCH(__nv_bfloat16, 64);
+    HVA_DISPATCH(__nv_bfloat16, 128);
+  }
+#undef HVA_DISPATCH
+}

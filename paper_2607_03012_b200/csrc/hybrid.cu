@@ -1,0 +1,280 @@
+// S3 / S4: hybrid clustering across denoising steps (section 4.2 l.93-103; A.1 l.322).
+//   hva_select_subset : top-m tokens by Lowe ratio (radix select + ordered compaction), ties -> lower index
+//   hva_cluster_update: subset tokens re-assigned against ALL centroids (direct form, fp32, first
+//                       minimum), then per-centroid deterministic adjustment of sums / sizes / mu
+//                       (DESIGN.md R-H3), or a full refresh of every centroid (R-H3').
+#include "common.cuh"
+
+namespace {
+
+constexpr int kSelThreads = 1024;
+
+// block-wide exclusive scan of a 0/1 flag; returns rank, *total receives the block count
+__device__ __forceinline__ int block_rank(bool flag, int* s_warp, int* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  unsigned b = __ballot_sync(0xffffffffu, flag);
+  int r = __popc(b & ((1u << lane) - 1));
+  if (lane == 0) s_warp[warp] = __popc(b);
+  __syncthreads();
+  if (warp == 0) {
+    int v = s_warp[lane], x = v;
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    s_warp[lane] = x - v;
+    if (lane == 31) *total = x;
+  }
+  __syncthreads();
+  r += s_warp[warp];
+  return r;   // caller reads *total, then must __syncthreads() before the next call
+}
+
+__global__ void __launch_bounds__(kSelThreads) hva_select_subset_kernel(int n, int m, const float* __restrict__ lowe,
+                                                                        int* __restrict__ subset) {
+  const int bh = blockIdx.x, tid = threadIdx.x;
+  const uint32_t* bits = reinterpret_cast<const uint32_t*>(lowe) + (size_t)bh * n;   // rho >= 0: bit order == value order
+  __shared__ int s_hist[256];
+  __shared__ int s_warp[32];
+  __shared__ int s_tot;
+  __shared__ uint32_t s_prefix;
+  __shared__ int s_remain;
+  if (tid == 0) { s_prefix = 0; s_remain = m; }
+  __syncthreads();
+  // MSB-first radix select of the m-th largest value
+  for (int shift = 24; shift >= 0; shift -= 8) {
+    for (int i = tid; i < 256; i += kSelThreads) s_hist[i] = 0;
+    __syncthreads();
+    const uint32_t prefix = s_prefix, pmask = shift == 24 ? 0u : (0xffffffffu << (shift + 8));
+    for (int i0 = 0; i0 < n; i0 += kSelThreads) {   // warp-aggregated: rho values share their top bytes
+      int i = i0 + tid;
+      uint32_t v = i < n ? bits[i] : 0u;
+      int key = (i < n && (v & pmask) == prefix) ? (int)((v >> shift) & 255) : -1;
+      unsigned peers = __match_any_sync(0xffffffffu, key);
+      if (key >= 0 && (peers & ((1u << (tid & 31)) - 1)) == 0) atomicAdd(&s_hist[key], __popc(peers));
+    }
+    __syncthreads();
+    if (tid == 0) {
+      int rem = s_remain, d = 255;
+      for (; d > 0; --d) { if (s_hist[d] >= rem) break; rem -= s_hist[d]; }
+      s_prefix = prefix | ((uint32_t)d << shift);
+      s_remain = rem;
+    }
+    __syncthreads();
+  }
+  const uint32_t thr = s_prefix;   // m-th largest value; s_remain = how many == thr to take (lowest indices first)
+  const int need_eq = s_remain;
+  int out = 0, eq_seen = 0;
+  for (int i0 = 0; i0 < n; i0 += kSelThreads) {
+    int i = i0 + tid;
+    uint32_t v = i < n ? bits[i] : 0u;
+    bool gt = i < n && v > thr, eq = i < n && v == thr;
+    int eq_tot;
+    int eq_rank = block_rank(eq, s_warp, &s_tot);
+    eq_tot = s_tot;
+    __syncthreads();
+    bool take = gt || (eq && eq_seen + eq_rank < need_eq);
+    int r = block_rank(take, s_warp, &s_tot);
+    int tot = s_tot;
+    __syncthreads();
+    if (take) subset[(size_t)bh * m + out + r] = i;
+    out += tot; eq_seen += eq_tot;
+  }
+}
+
+// ---- subset re-assignment against all centroids (thread = subset token, centroid tiles in smem)
+constexpr int kUpdThreads = 128, kCTile = 32, kCB2 = 8;
+
+__device__ __forceinline__ void ld8(const float* p, float x[8]) {
+  float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
+  x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y; x[6] = b.z; x[7] = b.w;
+}
+__device__ __forceinline__ void ld8(const __nv_bfloat16* p, float x[8]) {
+  uint4 r = *reinterpret_cast<const uint4*>(p);
+  x[0] = __uint_as_float(r.x << 16); x[1] = __uint_as_float(r.x & 0xffff0000u);
+  x[2] = __uint_as_float(r.y << 16); x[3] = __uint_as_float(r.y & 0xffff0000u);
+  x[4] = __uint_as_float(r.z << 16); x[5] = __uint_as_float(r.z & 0xffff0000u);
+  x[6] = __uint_as_float(r.w << 16); x[7] = __uint_as_float(r.w & 0xffff0000u);
+}
+
+template <typename T, int D>
+__global__ void __launch_bounds__(kUpdThreads) hva_subset_assign_kernel(int n, int Nc, int m, const T* __restrict__ X,
+                                                                        const int* __restrict__ subset,
+                                                                        const float* __restrict__ mu,
+                                                                        const int* __restrict__ assign,
+                                                                        int* __restrict__ oldlab, int* __restrict__ newlab) {
+  constexpr int kVec = 16 / sizeof(T), kRow = D + kVec;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float* s_mu = reinterpret_cast<float*>(smem_raw);            // [kCTile][D]
+  T* s_x = reinterpret_cast<T*>(s_mu + kCTile * D);            // [kUpdThreads][kRow]
+  const int bh = blockIdx.y, tid = threadIdx.x, i0 = blockIdx.x * kUpdThreads;
+  constexpr int kChunks = D / kVec;
+  for (int e = tid; e < kUpdThreads * kChunks; e += kUpdThreads) {
+    int li = e / kChunks, q = e % kChunks;
+    if (i0 + li < m) {
+      size_t tok = (size_t)bh * n + subset[(size_t)bh * m + i0 + li];
+      *reinterpret_cast<uint4*>(s_x + (size_t)li * kRow + q * kVec) = __ldg(reinterpret_cast<const uint4*>(X + tok * D) + q);
+    }
+  }
+  float best = __int_as_float(0x7f800000);
+  int lab = 0;
+  const T* xr = s_x + (size_t)tid * kRow;
+  for (int u0 = 0; u0 < Nc; u0 += kCTile) {
+    __syncthreads();
+    for (int e = tid; e < kCTile * (D / 4); e += kUpdThreads) {
+      int v = e / (D / 4), q = e % (D / 4);
+      int u = min(u0 + v, Nc - 1);
+      reinterpret_cast<float4*>(s_mu)[e] = reinterpret_cast<const float4*>(mu + ((size_t)bh * Nc + u) * D)[q];
+    }
+    __syncthreads();
+    if (i0 + tid < m) {
+      for (int v0 = 0; v0 < kCTile; v0 += kCB2) {
+        float acc[kCB2];
+#pragma unroll
+        for (int j = 0; j < kCB2; ++j) acc[j] = 0.f;
+        for (int c0 = 0; c0 < D; c0 += 8) {
+          float x[8];
+          ld8(xr + c0, x);
+#pragma unroll
+          for (int j = 0; j < kCB2; ++j) {
+            float mm[8];
+            ld8(s_mu + (size_t)(v0 + j) * D + c0, mm);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { float d = x[e] - mm[e]; acc[j] = fmaf(d, d, acc[j]); }
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < kCB2; ++j)
+          if (u0 + v0 + j < Nc && acc[j] < best) { best = acc[j]; lab = u0 + v0 + j; }   // first minimum
+      }
+    }
+  }
+  if (i0 + tid < m) {
+    newlab[(size_t)bh * m + i0 + tid] = lab;
+    oldlab[(size_t)bh * m + i0 + tid] = assign[(size_t)bh * n + subset[(size_t)bh * m + i0 + tid]];
+  }
+}
+
+// ---- per-centroid deterministic adjustment (R-H3): moves are applied in subset order.
+// The CTA of centroid u scans the subset cooperatively (one entry per thread, ballot) and applies the
+// few matching moves sequentially, thread = feature dim.
+template <typename T, int D>
+__global__ void __launch_bounds__(D) hva_subset_apply_kernel(int n, int Nc, int m, const T* __restrict__ X,
+                                                             const int* __restrict__ subset, const int* __restrict__ oldlab,
+                                                             const int* __restrict__ newlab, float* __restrict__ mu,
+                                                             float* __restrict__ sums, int* __restrict__ sizes) {
+  const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x, lane = c & 31, warp = c >> 5;
+  __shared__ unsigned s_bal[D / 32];
+  __shared__ int s_tok[D];
+  __shared__ int s_dir[D];
+  const size_t o = ((size_t)bh * Nc + u) * D + c;
+  float z = sums[o];
+  int cnt = sizes[(size_t)bh * Nc + u];
+  bool touched = false;
+  for (int i0 = 0; i0 < m; i0 += D) {
+    const int i = i0 + c;
+    int ol = -1, nl = -1;
+    if (i < m) { ol = oldlab[(size_t)bh * m + i]; nl = newlab[(size_t)bh * m + i]; }
+    const bool hit = (ol != nl) && (ol == u || nl == u);
+    const unsigned b = __ballot_sync(0xffffffffu, hit);
+    if (lane == 0) s_bal[warp] = b;
+    if (hit) { s_tok[c] = subset[(size_t)bh * m + i]; s_dir[c] = (ol == u) ? -1 : 1; }
+    __syncthreads();
+    for (int w = 0; w < D / 32; ++w) {
+      unsigned bits = s_bal[w];
+      while (bits) {
+        int e = w * 32 + __ffs(bits) - 1;
+        bits &= bits - 1;
+        float x = HvaElem<T>::ld(X + ((size_t)bh * n + s_tok[e]) * D + c);
+        if (s_dir[e] < 0) { z -= x; --cnt; } else { z += x; ++cnt; }
+        touched = true;
+      }
+    }
+    __syncthreads();
+  }
+  if (touched) {
+    sums[o] = z;
+    if (c == 0) sizes[(size_t)bh * Nc + u] = cnt;
+    if (cnt > 0) mu[o] = __fdiv_rn(z, (float)cnt);
+  }
+}
+
+__global__ void hva_subset_commit_kernel(int n, int m, const int* __restrict__ subset, const int* __restrict__ newlab,
+                                         int* __restrict__ assign) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x, bh = blockIdx.y;
+  if (i < m) assign[(size_t)bh * n + subset[(size_t)bh * m + i]] = newlab[(size_t)bh * m + i];
+}
+
+// ---- R-H3': every centroid = mean of the current features of its members (token order => deterministic)
+template <typename T, int D>
+__global__ void __launch_bounds__(D) hva_refresh_kernel(int n, int Nc, const T* __restrict__ X, const int* __restrict__ assign,
+                                                        float* __restrict__ mu, float* __restrict__ sums, int* __restrict__ sizes) {
+  const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
+  float z = 0.f;
+  int cnt = 0;
+  for (int tok = 0; tok < n; ++tok) {
+    if (assign[(size_t)bh * n + tok] != u) continue;
+    z += HvaElem<T>::ld(X + ((size_t)bh * n + tok) * D + c);
+    ++cnt;
+  }
+  const size_t o = ((size_t)bh * Nc + u) * D + c;
+  sums[o] = z;
+  if (c == 0) sizes[(size_t)bh * Nc + u] = cnt;
+  if (cnt > 0) mu[o] = __fdiv_rn(z, (float)cnt);
+}
+
+template <typename T, int D>
+int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, int refresh_all, int* assign, float* mu,
+               float* sums, int* sizes, int* newlab, cudaStream_t st) {
+  int* oldlab = newlab + (size_t)BH * (m > 0 ? m : 1);
+  const T* x = reinterpret_cast<const T*>(X);
+  size_t smem = (size_t)kCTile * D * 4 + (size_t)kUpdThreads * (D + 16 / sizeof(T)) * sizeof(T);
+  if (cudaFuncSetAttribute(hva_subset_assign_kernel<T, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return HVA_ECUDA;
+  hva_subset_assign_kernel<T, D><<<dim3((m + kUpdThreads - 1) / kUpdThreads, BH), kUpdThreads, smem, st>>>(n, Nc, m, x, subset, mu, assign, oldlab, newlab);
+  HVA_CHECK_LAUNCH();
+  if (!refresh_all) {
+    hva_subset_apply_kernel<T, D><<<dim3(Nc, BH), D, 0, st>>>(n, Nc, m, x, subset, oldlab, newlab, mu, sums, sizes);
+    HVA_CHECK_LAUNCH();
+  }
+  hva_subset_commit_kernel<<<dim3((m + 255) / 256, BH), 256, 0, st>>>(n, m, subset, newlab, assign);
+  HVA_CHECK_LAUNCH();
+  if (refresh_all) {
+    hva_refresh_kernel<T, D><<<dim3(Nc, BH), D, 0, st>>>(n, Nc, x, assign, mu, sums, sizes);
+    HVA_CHECK_LAUNCH();
+  }
+  return HVA_OK;
+}
+
+}  // namespace
+
+size_t hva_hybrid_ws_bytes(int BH, int n, int Nc, int m, int D) {
+  (void)n; (void)Nc; (void)D;
+  return hva_align((size_t)BH * (m > 0 ? m : 1) * 8);
+}
+
+extern "C" int hva_select_subset(int32_t BH, int32_t n, const float* lowe, int32_t m, int32_t* subset, void* ws,
+                                 size_t ws_bytes, void* stream) {
+  (void)ws; (void)ws_bytes;
+  if (!lowe || !subset || BH < 1 || n < 1 || m < 0 || m > n) return HVA_EINVAL;
+  if (m == 0) return HVA_OK;
+  hva_select_subset_kernel<<<BH, kSelThreads, 0, reinterpret_cast<cudaStream_t>(stream)>>>(n, m, lowe, subset);
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
+}
+
+extern "C" int hva_cluster_update(const hva_shape* s, int32_t Nc, const void* X, const int32_t* subset, int32_t m,
+                                  int32_t refresh_all, int32_t* assign, float* mu, float* sums, int32_t* sizes, void* ws,
+                                  size_t ws_bytes, void* stream) {
+  if (!s || !X || !subset || !assign || !mu || !sums || !sizes || !ws) return HVA_EINVAL;
+  if (Nc < 1 || m < 0 || (s->D != 64 && s->D != 128)) return HVA_EINVAL;
+  if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
+  const int BH = s->B * s->heads, n = s->T * s->H * s->W;
+  if (m > n) return HVA_EINVAL;
+  if (ws_bytes < hva_hybrid_ws_bytes(BH, n, Nc, m, s->D)) return HVA_EWORKSPACE;
+  if (m == 0 && !refresh_all) return HVA_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  int* newlab = reinterpret_cast<int*>(ws);
+#define HVA_DISPATCH(T, DD) return run_update<T, DD>(BH, n, Nc, m, X, subset, refresh_all, assign, mu, sums, sizes, newlab, st)
+  if (s->dtype == HVA_F32) { if (s->D == 64) HVA_DISPATCH(float, 64); HVA_DISPATCH(float, 128); }
+  if (s->D == 64) HVA_DISPATCH(__nv_bfloat16, 64);
+  HVA_DISPATCH(__nv_bfloat16, 128);
+#undef HVA_DISPATCH
+}
