@@ -1,0 +1,277 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one hva_forward call (anchor step: clustering of Q and K, mask, merge, plan,
+permutation, block-sparse attention, inverse permutation) over one batch of synthetic input.
+
+Default workload = BASELINE.json configs[3] (C4, HunyuanVideo shape: 24 heads x 118,800 tokens x 128, bf16),
+the configuration the metric is quoted on.  Prints ONE JSON line.
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
+N > 1 (torchrun): every rank runs the same-size call on its own heads' worth of data (head sharding, no
+collective; "weak" scaling); value = max-over-ranks ms per step / N.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+from paper_2607_03012_b200 import inputs  # noqa: E402
+
+METRIC = "sparse-attn ms/call + clustering ms/step at 118,800-token HunyuanVideo shape"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], tf_burst=d["bf16_tflops"], tf_sust=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    src="measured")
+    return dict(hbm=6650.0, tf_burst=1590.0, tf_sust=1400.0, src="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, idx):
+        self.idx, self.rows, self.proc = idx, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        pw = [float(r[2]) for r in self.rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def ev_time(fn, reps):
+    """ms per call of fn over `reps` back-to-back calls, CUDA events on the current stream."""
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(reps):
+        fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def oracle_sample(wl, head=0, attn_rows=32, merge_rounds=None):
+    """The CPU oracle, as it stands, on a bounded sample of the workload: one head's clustering (Q and K), mask,
+    merge, plan, and `attn_rows` attention rows.  Returns (seconds by stage, extrapolated ms per full call)."""
+    import oracle
+    x = inputs.make_head(wl, head)
+    Q, K, V = [inputs.to_f64(t) for t in x]
+    lat = (wl.T, wl.H, wl.W)
+    t = {}
+    t0 = time.perf_counter(); cq = oracle.local_window_kmeans(Q, lat, wl.cell, wl.win, wl.iters)
+    ck = oracle.local_window_kmeans(K, lat, wl.cell, wl.win, wl.iters); t["cluster"] = time.perf_counter() - t0
+    scale = float(np.float32(1 / math.sqrt(wl.D)))
+    t0 = time.perf_counter(); M = oracle.build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(np.float32(wl.top_p)))
+    t["mask"] = time.perf_counter() - t0
+    R = wl.merge_rounds if merge_rounds is None else merge_rounds
+    t0 = time.perf_counter(); gof, gids, chi = oracle.merge_clusters(cq["sizes"], ck["sizes"], M, wl.tile[0], wl.tile[1], R, seed=wl.seed, bh=head)
+    t["merge"] = time.perf_counter() - t0
+    t0 = time.perf_counter(); oracle.build_plan(cq["assign"], ck["assign"], gof, len(cq["sizes"]), len(ck["sizes"]))
+    t["plan"] = time.perf_counter() - t0
+    rows = np.sort(np.random.default_rng(0).choice(wl.n, attn_rows, replace=False))
+    t0 = time.perf_counter(); oracle.masked_attention_rows(Q, K, V, rows, cq["assign"], ck["assign"], gof, gids, chi, scale)
+    t["attn_rows"] = time.perf_counter() - t0
+    per_head = t["cluster"] + t["mask"] + t["merge"] + t["plan"] + t["attn_rows"] * (wl.n / attn_rows)
+    return t, per_head * wl.heads * 1e3
+
+
+def run_reference(args, wl):
+    """--impl reference: the oracle timed on the host cores, each step a bounded sample, extrapolated to ms/call."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vals = []
+    for i in range(args.warmup + args.steps):
+        t, ms = oracle_sample(wl, head=i % wl.heads, attn_rows=16, merge_rounds=1 if wl.n > 50000 else None)
+        if i >= args.warmup:
+            vals.append(ms)
+    v = float(np.mean(vals))
+    cores = os.cpu_count()
+    sample = ("per step: one head of %s through oracle clustering (Q,K), mask, 1 merge round, plan and 16 attention rows; "
+              "extrapolated x heads and x n/16 rows" % wl.name)
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "f64", "data": "synthetic", "config": {"workload": wl.name},
+                      "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C4")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--top-p", type=float, default=None)
+    ap.add_argument("--merge-rounds", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stages", action="store_true")
+    args = ap.parse_args()
+    wl = inputs.CONFIGS[args.config]
+    if args.impl == "reference":
+        return run_reference(args, wl)
+
+    from paper_2607_03012_b200 import binding as b
+    b.lib()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hva path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    pk = peaks()
+
+    # ---- inputs: generated on the host, resident in HBM before the timed region
+    import dataclasses
+    wl_r = dataclasses.replace(wl, seed=wl.seed + 1000 * rank) if rank else wl
+    hQ, hK, hV = [t.contiguous().pin_memory() for t in inputs.make_qkv(wl_r)]
+    Q, K, V = hQ.cuda(), hK.cuda(), hV.cuda()
+    shape = b.make_shape(wl)
+    cfg = b.make_config(wl, top_p=args.top_p, merge_rounds=args.merge_rounds)
+    fwd = b.Forward(shape, cfg)
+    O = torch.empty_like(Q)
+    step = lambda: fwd(Q, K, V, O)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clk = ClockSampler(local)
+    clk.start()
+    ms = ev_time(step, args.steps)
+    clocks = clk.stop()
+    if world > 1:
+        tt = torch.tensor([ms], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+        dist.barrier()
+    stats = fwd.stats_dicts()
+
+    # ---- end to end through the C ABI with HOST buffers (H2D of Q,K,V and D2H of O inside the timed region)
+    hO = torch.empty_like(hQ).pin_memory()
+    dev4 = torch.empty((4,) + tuple(Q.shape), dtype=Q.dtype, device="cuda")
+    fwd.host(hQ, hK, hV, hO, dev4)
+    t0 = time.perf_counter()
+    for _ in range(max(1, min(args.steps, 3))):
+        fwd.host(hQ, hK, hV, hO, dev4)
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / max(1, min(args.steps, 3))
+    nbytes = Q.numel() * Q.element_size()
+    del dev4
+
+    out = {"metric": METRIC, "value": ms / world, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+           "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+           "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
+           "config": {"workload": wl.name, "B": wl.B, "heads": wl.heads, "n": wl.n, "D": wl.D, "cell": wl.cell, "iters": wl.iters,
+                      "top_p": float(cfg.top_p), "merge_rounds": int(cfg.merge_rounds), "tile": wl.tile,
+                      "l2": "inputs (2.2 GB) larger than L2", "parallelism": "head-sharded replicas, no collective"},
+           "clocks": clocks,
+           "e2e": {"value": e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
+           "gpu_launches": args.steps * (2 * (1 + 2 * wl.iters) + 1 + 1 + 7 + 3 + 1)}
+
+    # ---- per-stage times and rooflines (rank 0)
+    if rank == 0 and not args.no_stages:
+        out.update(stage_report(b, wl, shape, cfg, Q, K, V, stats, pk))
+    if rank == 0 and not args.no_cpu_baseline:
+        t, cpu_ms = oracle_sample(wl, attn_rows=32, merge_rounds=1 if wl.n > 50000 else None)
+        out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": os.cpu_count(), "kind": "oracle",
+                               "sample": "one head of %s: oracle clustering Q,K %.1fs, mask %.2fs, merge(1 round) %.1fs, plan %.2fs, "
+                                         "32 attention rows %.2fs; extrapolated x%d heads, x n/32 rows" % (
+                                             wl.name, t["cluster"], t["mask"], t["merge"], t["plan"], t["attn_rows"], wl.heads)}
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
+    BH, n, D = wl.B * wl.heads, wl.n, wl.D
+    es = Q.element_size()
+    reps = 3
+    st = {}
+    cq = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, Q, want_lowe=False)
+    ck = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, K, want_lowe=False)
+    st["cluster_qk"] = ev_time(lambda: (b.hva_cluster(shape, wl.cell, wl.win, wl.iters, Q, want_lowe=False),
+                                        b.hva_cluster(shape, wl.cell, wl.win, wl.iters, K, want_lowe=False)), reps)
+    scale = 1.0 / math.sqrt(D)
+    M = b.hva_build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(cfg.top_p))
+    st["mask"] = ev_time(lambda: b.hva_build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(cfg.top_p)), reps)
+    mg = lambda: b.hva_merge(cq["sizes"], ck["sizes"], M, wl.tile[0], wl.tile[1], int(cfg.merge_rounds), seed=wl.seed)
+    gof, ng, gm = mg()
+    st["merge"] = ev_time(mg, reps)
+    pl = lambda: b.hva_build_plan(n, cq["assign"], ck["assign"], cq["sizes"], ck["sizes"], gof, ng, gm, wl.tile[0], wl.tile[1])
+    plan = pl()
+    st["plan"] = ev_time(pl, reps)
+    Qp, Kp, Vp = b.hva_permute(shape, Q, plan.perm_q), b.hva_permute(shape, K, plan.perm_k), b.hva_permute(shape, V, plan.perm_k)
+    st["permute_qkv"] = ev_time(lambda: (b.hva_permute(shape, Q, plan.perm_q), b.hva_permute(shape, K, plan.perm_k),
+                                         b.hva_permute(shape, V, plan.perm_k)), reps)
+    at = lambda: b.hva_sparse_attention(shape, cfg, Qp, Kp, Vp, plan, unpermute=True)
+    at()
+    st["attention"] = ev_time(at, reps)
+    tiles = sum(s["tiles_executed"] for s in stats)
+    tq, tk = wl.tile
+    exec_flop = 4.0 * D * tq * tk * tiles                    # QK^T + PV on every executed (padded) tile
+    dense_flop = 4.0 * BH * float(n) * n * D
+    t_att = st["attention"] * 1e-3
+    ach = exec_flop / t_att / 1e12
+    pairs = sum(s["pairs_valid"] for s in stats)
+    padded = tiles * tq * tk
+    cl_bytes = 2 * wl.iters * BH * n * D * es + 2 * BH * n * 4      # X read once per iteration (Q and K) + labels
+    pm_bytes = 3 * 2 * BH * n * D * es + 3 * BH * n * 4
+    rep = {
+        "stages_ms": {k: round(v, 4) for k, v in st.items()},
+        "roofline": {"bound": "tensor", "kernel": "hva_attn_tc_kernel", "achieved": ach, "peak": pk["tf_sust"], "unit": "TFLOP/s",
+                     "frac": ach / pk["tf_sust"], "frac_of_burst": ach / pk["tf_burst"], "peak_source": pk["src"] + " (sustained)",
+                     "traffic": None, "executed_tflop": exec_flop / 1e12, "dense_equiv_tflops": dense_flop / t_att / 1e12},
+        "roofline_cluster": {"bound": "hbm", "kernel": "hva_assign_kernel+hva_finalize_kernel", "achieved": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9,
+                             "peak": pk["hbm"], "unit": "GB/s", "frac": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9 / pk["hbm"],
+                             "algorithmic_bytes": cl_bytes},
+        "roofline_permute": {"bound": "hbm", "kernel": "hva_permute_kernel", "achieved": pm_bytes / (st["permute_qkv"] * 1e-3) / 1e9,
+                             "peak": pk["hbm"], "unit": "GB/s", "frac": pm_bytes / (st["permute_qkv"] * 1e-3) / 1e9 / pk["hbm"]},
+        "occupancy": {"groups": sum(s["n_groups"] for s in stats), "theoretical_density": pairs / (BH * float(n) * n),
+                      "cta_density": padded / (BH * float(n) * n), "cta_tile_occupancy": pairs / padded,
+                      "q_rows_valid_over_padded": sum(s["q_rows_valid"] for s in stats) / sum(s["q_rows_padded"] for s in stats),
+                      "k_cols_valid_over_padded": sum(s["k_cols_valid"] for s in stats) / sum(s["k_cols_padded"] for s in stats)},
+    }
+    return rep
+
+
+if __name__ == "__main__":
+    main()

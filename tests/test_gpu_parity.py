@@ -253,7 +253,9 @@ def test_attention_tc_matches_simt_kernel(monkeypatch):
     monkeypatch.setenv("HVA_ATTN_SIMT", "1")
     O2 = fwd(*dev).clone()
     torch.cuda.synchronize()
-    assert (O1.float() - O2.float()).abs().max().item() <= 2e-2
+    d = (O1.float() - O2.float()).abs()
+    assert (d <= 2e-2 + 2.0 ** -7 * O2.float().abs()).all()          # both are bf16-rounded: allow 2 output ulps
+    assert (d.norm() / O2.float().norm()).item() <= 5e-3
     assert torch.equal(fwd(*dev), O2)                        # deterministic
 
 
