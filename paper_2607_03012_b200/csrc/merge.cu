@@ -1,6 +1,6 @@
 // S6: hardware-aware cluster merging (Eq. 7-10 l.111-125, Alg. 1 l.131-168).
 //
-// One CTA (32 warps) per (batch, head); all state is integer.  Costs are kept in tile units
+// All state is integer and lives in the workspace; one launch per phase.  Costs are kept in tile units
 // c(S) = ceil(s^q(S)/tau_q) * ceil(kappa(S)/tau_k) (Eq. 8 / (tau_q tau_k)).  Per round:
 //   1. side(g) from the counter-based hash of include/hva.h (Alg. 1 line 6),
 //   2. warp-parallel pairwise-cost pass: one warp per A in side 1 walks every B in side 0 in
@@ -14,7 +14,6 @@
 
 namespace {
 
-constexpr int kMergeThreads = 1024;
 constexpr unsigned long long kNoProp = ~0ull;
 
 __host__ __device__ __forceinline__ uint32_t hva_side_hash(uint32_t seed, uint32_t bh, uint32_t rnd, uint32_t gid) {
@@ -33,110 +32,136 @@ struct MergeParams {
 
 __device__ __forceinline__ int cdiv(int a, int b) { return (a + b - 1) / b; }
 
-__global__ void __launch_bounds__(kMergeThreads) hva_merge_kernel(MergeParams p) {
-  const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int Nq = p.Nq, Nk = p.Nk, Wd = p.Wd;
-  extern __shared__ int s_sk[];  // [Wd*32] key cluster sizes (zero padded)
-  uint32_t* chi = p.chi + (size_t)bh * Nq * Wd;
-  int* sq = p.sq + (size_t)bh * Nq; int* kap = p.kap + (size_t)bh * Nq; int* alive = p.alive + (size_t)bh * Nq;
-  int* side = p.side + (size_t)bh * Nq; int* remap = p.remap + (size_t)bh * Nq;
-  unsigned long long* best = p.best + (size_t)bh * Nq;
-  int* group_of = p.group_of + (size_t)bh * Nq;
-  const uint8_t* mask = p.mask + (size_t)bh * Nq * Nk;
+// Alg. 1 lines 3-4: singleton groups, chi_j({i}) = m_ij (bit-packed by ballot), kappa({i}).  One warp per cluster.
+__global__ void __launch_bounds__(256) hva_merge_init_kernel(MergeParams p) {
+  const int bh = blockIdx.y, lane = threadIdx.x & 31, i = blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (i >= p.Nq) return;
+  const uint8_t* mrow = p.mask + ((size_t)bh * p.Nq + i) * p.Nk;
+  const int* sk = p.sizes_k + (size_t)bh * p.Nk;
+  int k = 0;
+  for (int w = 0; w < p.Wd; ++w) {
+    int j = w * 32 + lane;
+    bool bit = j < p.Nk && mrow[j];
+    unsigned bits = __ballot_sync(0xffffffffu, bit);
+    if (bit) k += sk[j];
+    if (lane == 0) p.chi[((size_t)bh * p.Nq + i) * p.Wd + w] = bits;
+  }
+  for (int o = 16; o > 0; o >>= 1) k += __shfl_xor_sync(0xffffffffu, k, o);
+  if (lane == 0) {
+    size_t e = (size_t)bh * p.Nq + i;
+    int s = p.sizes_q[e];
+    p.sq[e] = s; p.kap[e] = k; p.alive[e] = s > 0; p.group_of[e] = i; p.remap[e] = -1; p.best[e] = kNoProp;
+  }
+}
 
-  for (int j = tid; j < Wd * 32; j += kMergeThreads) s_sk[j] = j < Nk ? p.sizes_k[(size_t)bh * Nk + j] : 0;
+// Alg. 1 lines 6-13 for round r: one warp per A in side 1 (warp-parallel pairwise-cost pass).
+__global__ void __launch_bounds__(256) hva_merge_propose_kernel(MergeParams p, int r) {
+  const int bh = blockIdx.y, tid = threadIdx.x, lane = tid & 31, Nq = p.Nq, Wd = p.Wd;
+  extern __shared__ int s_mem[];
+  int* s_sk = s_mem;                 // [Wd*32] key cluster sizes, zero padded
+  int* s_sq = s_sk + Wd * 32;        // [Nq] s^q(B) for B in side 0, else 0 (0 => skip)
+  int* s_kap = s_sq + Nq;            // [Nq]
+  const uint32_t* chi = p.chi + (size_t)bh * Nq * Wd;
+  const size_t e0 = (size_t)bh * Nq;
+  for (int j = tid; j < Wd * 32; j += 256) s_sk[j] = j < p.Nk ? p.sizes_k[(size_t)bh * p.Nk + j] : 0;
+  for (int g = tid; g < Nq; g += 256) {
+    bool isB = p.alive[e0 + g] && hva_side_hash(p.seed, (uint32_t)bh, (uint32_t)r, (uint32_t)g) == 0;
+    s_sq[g] = isB ? p.sq[e0 + g] : 0;
+    s_kap[g] = p.kap[e0 + g];
+  }
   __syncthreads();
-  // Alg. 1 lines 3-4: singleton groups, chi_j({i}) = m_ij (bit-packed); kappa({i})
-  for (int i = warp; i < Nq; i += kMergeThreads / 32) {
+  const int A = blockIdx.x * 8 + (tid >> 5);
+  if (A >= Nq || !p.alive[e0 + A] || hva_side_hash(p.seed, (uint32_t)bh, (uint32_t)r, (uint32_t)A) != 1) return;
+  const int sA = p.sq[e0 + A], kA = p.kap[e0 + A], rA = cdiv(sA, p.tile_q), cA = rA * cdiv(kA, p.tile_k);
+  const uint32_t a0 = lane < Wd ? ~chi[(size_t)A * Wd + lane] : 0u;
+  const uint32_t a1 = lane + 32 < Wd ? ~chi[(size_t)A * Wd + lane + 32] : 0u;
+  int best_dc = 0, best_B = -1;
+  for (int B = 0; B < Nq; ++B) {
+    const int sB = s_sq[B];
+    if (sB == 0) continue;
+    const int kB = s_kap[B], rB = cdiv(sB, p.tile_q), cB = rB * cdiv(kB, p.tile_k);
+    const int rU = cdiv(sA + sB, p.tile_q);
+    if (p.max_q_tiles > 0 && rU > p.max_q_tiles) continue;
+    if (rU >= rA + rB) continue;                                      // no row tile saved => dC >= 0 (R-M6)
+    const int kLow = kA > kB ? kA : kB;
+    if (rU * cdiv(kLow, p.tile_k) - cA - cB >= best_dc) continue;     // lower bound cannot beat the current best
+    int add = 0;                                                      // sum of s^k over B \ A
+    uint32_t b0 = lane < Wd ? chi[(size_t)B * Wd + lane] & a0 : 0u;
+    uint32_t b1 = lane + 32 < Wd ? chi[(size_t)B * Wd + lane + 32] & a1 : 0u;
+    while (b0) { int b = __ffs(b0) - 1; b0 &= b0 - 1; add += s_sk[lane * 32 + b]; }
+    while (b1) { int b = __ffs(b1) - 1; b1 &= b1 - 1; add += s_sk[(lane + 32) * 32 + b]; }
+    for (int o = 16; o > 0; o >>= 1) add += __shfl_xor_sync(0xffffffffu, add, o);
+    const int dc = rU * cdiv(kA + add, p.tile_k) - cA - cB;           // Eq. 10 in tile units
+    if (dc < best_dc) { best_dc = dc; best_B = B; }                   // strict: ties -> lower gid(B)
+  }
+  if (lane == 0 && best_B >= 0) {
+    unsigned long long key = ((unsigned long long)(uint32_t)(best_dc + 0x40000000) << 32) | (uint32_t)A;
+    atomicMin(&p.best[e0 + best_B], key);                             // line 14: best A per B, ties -> lower gid(A)
+  }
+}
+
+// Alg. 1 lines 15-16: accepted pairs are disjoint, applied in parallel.  One CTA per (b, head); warp per pair.
+__global__ void __launch_bounds__(1024) hva_merge_apply_kernel(MergeParams p) {
+  const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, Nq = p.Nq, Wd = p.Wd;
+  uint32_t* chi = p.chi + (size_t)bh * Nq * Wd;
+  const size_t e0 = (size_t)bh * Nq;
+  const int* sk = p.sizes_k + (size_t)bh * p.Nk;
+  for (int B = warp; B < Nq; B += 32) {
+    unsigned long long key = p.best[e0 + B];
+    if (key == kNoProp) continue;
+    const int A = (int)(uint32_t)(key & 0xffffffffu);
+    const int g = A < B ? A : B, o = A < B ? B : A;
     int k = 0;
     for (int w = lane; w < Wd; w += 32) {
-      uint32_t bits = 0;
-      for (int b = 0; b < 32; ++b) {
-        int j = w * 32 + b;
-        if (j < Nk && mask[(size_t)i * Nk + j]) { bits |= 1u << b; k += s_sk[j]; }
-      }
-      chi[(size_t)i * Wd + w] = bits;
+      uint32_t bits = chi[(size_t)g * Wd + w] | chi[(size_t)o * Wd + w];
+      chi[(size_t)g * Wd + w] = bits;
+      while (bits) { int b = __ffs(bits) - 1; bits &= bits - 1; k += sk[w * 32 + b]; }
     }
-    for (int o = 16; o > 0; o >>= 1) k += __shfl_xor_sync(0xffffffffu, k, o);
+    for (int x = 16; x > 0; x >>= 1) k += __shfl_xor_sync(0xffffffffu, k, x);
     if (lane == 0) {
-      int s = p.sizes_q[(size_t)bh * Nq + i];
-      sq[i] = s; kap[i] = k; alive[i] = s > 0; group_of[i] = i; remap[i] = -1;
+      p.sq[e0 + g] = p.sq[e0 + A] + p.sq[e0 + B]; p.kap[e0 + g] = k; p.alive[e0 + o] = 0; p.remap[e0 + o] = g;
     }
   }
   __syncthreads();
+  for (int i = tid; i < Nq; i += 1024) {
+    int m = p.remap[e0 + p.group_of[e0 + i]];
+    if (m >= 0) p.group_of[e0 + i] = m;
+  }
+  __syncthreads();
+  for (int i = tid; i < Nq; i += 1024) { p.remap[e0 + i] = -1; p.best[e0 + i] = kNoProp; }
+}
 
-  for (int r = 1; r <= p.rounds; ++r) {
-    for (int g = tid; g < Nq; g += kMergeThreads) {
-      side[g] = alive[g] ? (int)hva_side_hash(p.seed, (uint32_t)bh, (uint32_t)r, (uint32_t)g) : -1;
-      best[g] = kNoProp;
-    }
-    __syncthreads();
-    for (int A = warp; A < Nq; A += kMergeThreads / 32) {
-      if (side[A] != 1) continue;
-      const int sA = sq[A], kA = kap[A], rA = cdiv(sA, p.tile_q), cA = rA * cdiv(kA, p.tile_k);
-      uint32_t a0 = lane < Wd ? chi[(size_t)A * Wd + lane] : 0u;
-      uint32_t a1 = lane + 32 < Wd ? chi[(size_t)A * Wd + lane + 32] : 0u;
-      int best_dc = 0, best_B = -1;
-      for (int B = 0; B < Nq; ++B) {
-        if (side[B] != 0) continue;
-        const int sB = sq[B], kB = kap[B], rB = cdiv(sB, p.tile_q), cB = rB * cdiv(kB, p.tile_k);
-        const int rU = cdiv(sA + sB, p.tile_q);
-        if (p.max_q_tiles > 0 && rU > p.max_q_tiles) continue;
-        if (rU >= rA + rB) continue;                                      // no row tile saved => dC >= 0 (R-M6)
-        const int kLow = kA > kB ? kA : kB;
-        if (rU * cdiv(kLow, p.tile_k) - cA - cB >= best_dc) continue;     // lower bound cannot beat current best
-        int add = 0;
-        uint32_t b0 = lane < Wd ? chi[(size_t)B * Wd + lane] & ~a0 : 0u;
-        uint32_t b1 = lane + 32 < Wd ? chi[(size_t)B * Wd + lane + 32] & ~a1 : 0u;
-        while (b0) { int b = __ffs(b0) - 1; b0 &= b0 - 1; add += s_sk[lane * 32 + b]; }
-        while (b1) { int b = __ffs(b1) - 1; b1 &= b1 - 1; add += s_sk[(lane + 32) * 32 + b]; }
-        for (int o = 16; o > 0; o >>= 1) add += __shfl_xor_sync(0xffffffffu, add, o);
-        const int dc = rU * cdiv(kA + add, p.tile_k) - cA - cB;           // Eq. 10 in tile units
-        if (dc < best_dc) { best_dc = dc; best_B = B; }                   // strict: ties -> lower gid(B)
-      }
-      if (lane == 0 && best_B >= 0) {
-        unsigned long long key = ((unsigned long long)(uint32_t)(best_dc + 0x40000000) << 32) | (uint32_t)A;
-        atomicMin(&best[best_B], key);                                    // ties -> lower gid(A)
-      }
-    }
-    __syncthreads();
-    for (int B = tid; B < Nq; B += kMergeThreads) {
-      unsigned long long key = best[B];
-      if (key == kNoProp) continue;
-      int A = (int)(uint32_t)(key & 0xffffffffu);
-      int g = A < B ? A : B, o = A < B ? B : A;
-      int k = 0;
-      for (int w = 0; w < Wd; ++w) {
-        uint32_t bits = chi[(size_t)g * Wd + w] | chi[(size_t)o * Wd + w];
-        chi[(size_t)g * Wd + w] = bits;
-        while (bits) { int b = __ffs(bits) - 1; bits &= bits - 1; k += s_sk[w * 32 + b]; }
-      }
-      sq[g] = sq[A] + sq[B]; kap[g] = k; alive[o] = 0; remap[o] = g;
-    }
-    __syncthreads();
-    for (int i = tid; i < Nq; i += kMergeThreads) {
-      int m = remap[group_of[i]];
-      if (m >= 0) group_of[i] = m;
-    }
-    __syncthreads();
-    for (int i = tid; i < Nq; i += kMergeThreads) remap[i] = -1;
-    __syncthreads();
-  }
-  // outputs: n_groups, chi rows of the active groups in ascending gid order
-  __shared__ int s_ng;
-  if (tid == 0) {
-    int c = 0;
-    for (int g = 0; g < Nq; ++g) if (alive[g]) side[c++] = g;   // reuse side[] as the ascending gid list
-    s_ng = c; p.n_groups[bh] = c;
-  }
+// n_groups and the chi rows of the active groups in ascending gid order.
+__global__ void __launch_bounds__(1024) hva_merge_rank_kernel(MergeParams p) {
+  const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, Nq = p.Nq;
+  const size_t e0 = (size_t)bh * Nq;
+  __shared__ int s_w[32];
+  __shared__ int s_base;
+  if (tid == 0) s_base = 0;
   __syncthreads();
-  uint8_t* gm = p.group_mask + (size_t)bh * Nq * Nk;
-  for (size_t e = tid; e < (size_t)Nq * Nk; e += kMergeThreads) {
-    int row = (int)(e / Nk), j = (int)(e % Nk);
-    uint8_t v = 0;
-    if (row < s_ng) v = (chi[(size_t)side[row] * Wd + (j >> 5)] >> (j & 31)) & 1u;
-    gm[e] = v;
+  for (int g0 = 0; g0 < Nq; g0 += 1024) {
+    int g = g0 + tid;
+    bool al = g < Nq && p.alive[e0 + g];
+    unsigned bal = __ballot_sync(0xffffffffu, al);
+    if (lane == 0) s_w[warp] = __popc(bal);
+    __syncthreads();
+    int off = s_base;
+    for (int w = 0; w < warp; ++w) off += s_w[w];
+    if (al) p.side[e0 + off + __popc(bal & ((1u << lane) - 1))] = g;     // side[] reused: ascending active gids
+    __syncthreads();
+    if (tid == 0) { int t = 0; for (int w = 0; w < 32; ++w) t += s_w[w]; s_base += t; }
+    __syncthreads();
   }
+  if (tid == 0) p.n_groups[bh] = s_base;
+}
+
+__global__ void __launch_bounds__(256) hva_merge_out_kernel(MergeParams p) {
+  const int bh = blockIdx.y, row = blockIdx.x, Nq = p.Nq, Nk = p.Nk, Wd = p.Wd;
+  const int ng = p.n_groups[bh];
+  uint8_t* out = p.group_mask + ((size_t)bh * Nq + row) * Nk;
+  if (row >= ng) { for (int j = threadIdx.x; j < Nk; j += 256) out[j] = 0; return; }
+  const uint32_t* c = p.chi + ((size_t)bh * Nq + p.side[(size_t)bh * Nq + row]) * Wd;
+  for (int j = threadIdx.x; j < Nk; j += 256) out[j] = (c[j >> 5] >> (j & 31)) & 1u;
 }
 
 }  // namespace
@@ -168,7 +193,20 @@ extern "C" int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* size
   p.side = reinterpret_cast<int*>(w); w += a4;
   p.remap = reinterpret_cast<int*>(w); w += a4;
   p.best = reinterpret_cast<unsigned long long*>(w);
-  hva_merge_kernel<<<BH, kMergeThreads, (size_t)p.Wd * 32 * sizeof(int), reinterpret_cast<cudaStream_t>(stream)>>>(p);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const dim3 gw((Nq + 7) / 8, BH);
+  hva_merge_init_kernel<<<gw, 256, 0, st>>>(p);
+  HVA_CHECK_LAUNCH();
+  const size_t smem = ((size_t)p.Wd * 32 + 2 * (size_t)Nq) * sizeof(int);
+  for (int r = 1; r <= rounds; ++r) {
+    hva_merge_propose_kernel<<<gw, 256, smem, st>>>(p, r);
+    HVA_CHECK_LAUNCH();
+    hva_merge_apply_kernel<<<BH, 1024, 0, st>>>(p);
+    HVA_CHECK_LAUNCH();
+  }
+  hva_merge_rank_kernel<<<BH, 1024, 0, st>>>(p);
+  HVA_CHECK_LAUNCH();
+  hva_merge_out_kernel<<<dim3(Nq, BH), 256, 0, st>>>(p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }
