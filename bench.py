@@ -240,9 +240,10 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
     plan = pl()
     st["plan"] = ev_time(pl, reps)
     Qp, Kp, Vp = b.hva_permute(shape, Q, plan.perm_q), b.hva_permute(shape, K, plan.perm_k), b.hva_permute(shape, V, plan.perm_k)
-    st["permute_qkv"] = ev_time(lambda: (b.hva_permute(shape, Q, plan.perm_q), b.hva_permute(shape, K, plan.perm_k),
-                                         b.hva_permute(shape, V, plan.perm_k)), reps)
-    at = lambda: b.hva_sparse_attention(shape, cfg, Qp, Kp, Vp, plan, unpermute=True)
+    st["permute_qkv"] = ev_time(lambda: (b.hva_permute(shape, Q, plan.perm_q, out=Qp), b.hva_permute(shape, K, plan.perm_k, out=Kp),
+                                         b.hva_permute(shape, V, plan.perm_k, out=Vp)), reps)
+    Oo = torch.empty_like(Q)
+    at = lambda: b.hva_sparse_attention(shape, cfg, Qp, Kp, Vp, plan, unpermute=True, out=Oo)
     at()
     st["attention"] = ev_time(at, reps)
     tiles = sum(s["tiles_executed"] for s in stats)

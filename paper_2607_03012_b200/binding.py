@@ -231,20 +231,20 @@ def hva_build_plan(n, assign_q, assign_k, sizes_q, sizes_k, group_of, n_groups, 
     return Plan(buf, L, BH, n, Nq, Nk)
 
 
-def hva_permute(shape, X, perm):
-    Y = torch.empty_like(X)
+def hva_permute(shape, X, perm, out=None):
+    Y = torch.empty_like(X) if out is None else out
     _check(lib().hva_permute(C.byref(shape), _p(X), _p(perm), _p(Y), _stream()))
     return Y
 
 
-def hva_unpermute(shape, Xp, perm):
-    Y = torch.empty_like(Xp)
+def hva_unpermute(shape, Xp, perm, out=None):
+    Y = torch.empty_like(Xp) if out is None else out
     _check(lib().hva_unpermute(C.byref(shape), _p(Xp), _p(perm), _p(Y), _stream()))
     return Y
 
 
-def hva_sparse_attention(shape, cfg, Qp, Kp, Vp, plan: Plan, unpermute=True):
-    O = torch.empty_like(Qp)
+def hva_sparse_attention(shape, cfg, Qp, Kp, Vp, plan: Plan, unpermute=True, out=None):
+    O = torch.empty_like(Qp) if out is None else out
     _check(lib().hva_sparse_attention(C.byref(shape), C.byref(cfg), _p(Qp), _p(Kp), _p(Vp), _p(plan.buf),
                                       C.c_size_t(plan.L.total), plan.Nq, plan.Nk, _p(O), int(bool(unpermute)),
                                       C.c_void_p(0), C.c_size_t(0), _stream()))

@@ -8,7 +8,8 @@
 //              key runs, as power-of-two-height boxes of a 128B-swizzled 2-D tensor map, packed
 //              back to back in the stage buffer (exact packing across cluster boundaries)
 //   warp  5    TMEM allocator + single-thread tcgen05.mma issuer
-// Per key tile j:  S_j = Q K_j^T (SS MMA, K-major operands, fp32 accumulators in TMEM, two S buffers)
+// Two CTAs are resident per SM (96 KB smem, 256 TMEM columns each): one CTA's softmax overlaps the other's MMAs.
+// Per key tile j:  S_j = Q K_j^T (SS MMA, K-major operands, fp32 accumulators in TMEM)
 //                  P_j = exp2(S_j*scale*log2e - m) written back over S_j as bf16 (tcgen05.st)
 //                  O  += P_j V_j (TS MMA: A = P from TMEM, B = V from smem, MN-major)
 // with lazy (thresholded) rescaling of O in TMEM, 1/l normalisation and the inverse permutation
@@ -22,11 +23,11 @@ namespace {
 constexpr int kBM = 128, kBN = 128, kD = 128;
 constexpr int kHalfBytes = 128 * 128;          // one 64-dim half of a 128-row tile: 128 rows x 128 B
 constexpr int kTileBytes = 2 * kHalfBytes;     // 32 KB
-constexpr int kStages = 2;
+constexpr int kStages = 1;                     // one K and one V buffer per CTA: two CTAs share an SM
 constexpr int kThreadsTC = 192;
 constexpr int kNumBoxes = 8;                   // box heights 1,2,4,...,128
-constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kColS0 = 0, kColS1 = 128, kColO = 256;
+constexpr uint32_t kTmemCols = 256;            // S (P aliased over it) + O; two CTAs fit the SM's 512 columns
+constexpr uint32_t kColS = 0, kColO = 128;
 constexpr float kRescaleThreshold = 8.0f;      // log2 units
 
 struct TcMaps {
@@ -147,7 +148,7 @@ __device__ __forceinline__ uint32_t umma_idesc(uint32_t b_mn_major) {
 }
 
 struct __align__(8) TcBarriers {
-  uint64_t q_full, k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages], s_full[2], p_ready[2], o_done;
+  uint64_t q_full, k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages], s_full, p_ready, o_done;
   uint32_t tmem_base;
 };
 
@@ -189,7 +190,7 @@ __device__ __forceinline__ void load_tile(RunWalker& w, const CUtensorMap* maps,
     emit_boxes(maps, bar, stage, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
 }
 
-__global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid_constant__ TcMaps maps, TcParams p) {
+__global__ void __launch_bounds__(kThreadsTC, 2) hva_attn_tc_kernel(const __grid_constant__ TcMaps maps, TcParams p) {
   const int bh = blockIdx.y;
   if ((int)blockIdx.x >= p.work_cnt[bh]) return;
   const uint32_t wi = (uint32_t)p.work[(size_t)bh * p.work_cap + blockIdx.x];
@@ -223,7 +224,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
       mbar_init(&B->k_full[s], 1); mbar_init(&B->k_empty[s], 1);
       mbar_init(&B->v_full[s], 1); mbar_init(&B->v_empty[s], 1);
     }
-    for (int b = 0; b < 2; ++b) { mbar_init(&B->s_full[b], 1); mbar_init(&B->p_ready[b], 128); }
+    mbar_init(&B->s_full, 1); mbar_init(&B->p_ready, 128);
     mbar_init(&B->o_done, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -268,31 +269,29 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
         const int s = j % kStages;
         mbar_wait(&B->k_full[s], (j / kStages) & 1);
         tc_fence_after();
-        const uint32_t d = tmem + ((j & 1) ? kColS1 : kColS0);
 #pragma unroll
         for (int ks = 0; ks < kD / 16; ++ks) {
           const uint32_t off = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
-          mma_ss(d, umma_desc(q_addr + off, 16, 1024), umma_desc(k_addr + s * kTileBytes + off, 16, 1024), idesc_qk, ks > 0);
+          mma_ss(tmem + kColS, umma_desc(q_addr + off, 16, 1024), umma_desc(k_addr + s * kTileBytes + off, 16, 1024), idesc_qk, ks > 0);
         }
-        tc_commit(&B->s_full[j & 1]);
+        tc_commit(&B->s_full);
         tc_commit(&B->k_empty[s]);
       };
       mbar_wait(&B->q_full, 0);
       issue_qk(0);
       for (int j = 0; j < jn; ++j) {
-        if (j + 1 < jn) issue_qk(j + 1);
         const int s = j % kStages;
-        mbar_wait(&B->p_ready[j & 1], (j >> 1) & 1);
+        mbar_wait(&B->p_ready, j & 1);
         mbar_wait(&B->v_full[s], (j / kStages) & 1);
         tc_fence_after();
         const int rows_valid = min(kBN, kappa - j * kBN);
         const int ksteps = (rows_valid + 15) >> 4;
-        const uint32_t a = tmem + ((j & 1) ? kColS1 : kColS0);
         for (int ks = 0; ks < ksteps; ++ks)
-          mma_ts(tmem + kColO, a + ks * 8, umma_desc(v_addr + s * kTileBytes + ks * 2048, kHalfBytes, 1024), idesc_pv,
+          mma_ts(tmem + kColO, tmem + kColS + ks * 8, umma_desc(v_addr + s * kTileBytes + ks * 2048, kHalfBytes, 1024), idesc_pv,
                  (j > 0 || ks > 0));
         tc_commit(&B->v_empty[s]);
         tc_commit(&B->o_done);
+        if (j + 1 < jn) issue_qk(j + 1);   // S is aliased by P_j: issue order after PV(j) keeps the tensor pipe in order
       }
     }
   } else {
@@ -302,10 +301,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     float m_ref = -INFINITY, l = 0.f;
     uint32_t v[32];
     for (int j = 0; j < jn; ++j) {
-      const int b = j & 1;
-      const uint32_t s_addr = tmem + lane_base + (b ? kColS1 : kColS0);
+      const uint32_t s_addr = tmem + lane_base + kColS;
       const int rows_valid = min(kBN, kappa - j * kBN);
-      mbar_wait(&B->s_full[b], (j >> 1) & 1);
+      mbar_wait(&B->s_full, j & 1);
       tc_fence_after();
       float mx = -INFINITY;
 #pragma unroll 1
@@ -355,7 +353,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
       }
       tmem_st_wait();
       tc_fence_before();
-      mbar_arrive(&B->p_ready[b]);
+      mbar_arrive(&B->p_ready);
     }
     // epilogue: O / l, bf16, row store with the inverse permutation fused (Eq. 4: O = Pi^{q-1} O')
     mbar_wait(&B->o_done, (jn - 1) & 1);
