@@ -101,6 +101,8 @@ int hva_version(void);
 int32_t hva_num_clusters(const hva_shape* s, const int32_t cell[3]);
 size_t hva_workspace_bytes(const hva_shape* s, const hva_config* c);
 size_t hva_state_bytes(const hva_shape* s, const hva_config* c);   /* hybrid cache, l.101 */
+/* Scratch needed by one hva_cluster call (per-cell partial sums, split centroids); 0 on invalid arguments. */
+size_t hva_cluster_workspace_bytes(const hva_shape* s, const int32_t cell[3], const int32_t win[3]);
 int hva_plan_describe(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, int32_t tile_q, hva_plan_layout* out);
 
 /* S0-S2 (+A4): 3D local-window k-means on one tensor X[B,heads,n,D] (Alg. 2, l.346-388; Eq. 5

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libhva.so")
 HVA_F32, HVA_BF16 = 0, 1
 HVA_ANCHOR, HVA_INTERMEDIATE, HVA_DENSE = 0, 1, 2
 
-EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes",
+EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_cluster_workspace_bytes",
            "hva_plan_describe", "hva_cluster", "hva_select_subset", "hva_cluster_update", "hva_build_mask", "hva_merge",
            "hva_build_plan", "hva_permute", "hva_unpermute", "hva_sparse_attention", "hva_forward", "hva_forward_host"]
 
@@ -58,6 +58,7 @@ def lib():
         L.hva_strerror.restype = C.c_char_p
         L.hva_workspace_bytes.restype = C.c_size_t
         L.hva_state_bytes.restype = C.c_size_t
+        L.hva_cluster_workspace_bytes.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -144,7 +145,7 @@ def hva_cluster(shape, cell, win, iters, X, mu_init=None, want_sums=True, want_l
                sizes=torch.empty((BH, Nc), dtype=torch.int32, device=dev),
                sums=torch.empty((BH, Nc, D), dtype=torch.float32, device=dev) if want_sums else None,
                lowe=torch.empty((BH, n), dtype=torch.float32, device=dev) if want_lowe else None)
-    ws = _ws(BH * Nc * nwin * (D * 4 + 4) + 1024, dev)
+    ws = _ws(lib().hva_cluster_workspace_bytes(C.byref(shape), _i3(cell), _i3(win)), dev)
     _check(lib().hva_cluster(C.byref(shape), _i3(cell), _i3(win), int(iters), _p(X), _p(mu_init), _p(out["assign"]),
                              _p(out["mu"]), _p(out["sizes"]), _p(out["sums"]), _p(out["lowe"]), _p(ws),
                              C.c_size_t(ws.numel()), _stream()))

@@ -8,6 +8,8 @@
 // reduction with no atomics.  The per-(cell, slot) partial sums are combined per centroid, in a
 // fixed cell order, by hva_finalize_kernel (Alg. 2 line 23: mu <- z/n, empty keeps mu).
 #include "common.cuh"
+#include "cluster_tc.cuh"
+#include <cstdlib>
 
 namespace {
 
@@ -36,6 +38,38 @@ struct ClusterParams {
   int* assign;         // [BH, n] or null
   float* lowe;         // [BH, n] or null
 };
+
+// Operands of the tensor-pipe assignment (cluster_tc.cu): two-term bf16 split hi + lo of the fp32 centroid and
+// |mu|^2 in fp32 (fixed shuffle-tree order => deterministic).  Block = D threads, thread c owns mu_c.
+struct MuSplit {
+  __nv_bfloat16 *hi, *lo;   // [BH, Nc, D] or null
+  float* musq;              // [BH, Nc]
+};
+template <int D>
+__device__ __forceinline__ void mu_split_store(const MuSplit& sp, size_t row, int c, float m) {
+  if (!sp.hi) return;
+  const __nv_bfloat16 h = __float2bfloat16_rn(m);
+  sp.hi[row * D + c] = h;
+  sp.lo[row * D + c] = __float2bfloat16_rn(m - __bfloat162float(h));
+  __shared__ float s_red[D / 32];
+  float q = m * m;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+  if ((c & 31) == 0) s_red[c >> 5] = q;
+  __syncthreads();
+  if (c == 0) {
+    float t = s_red[0];
+#pragma unroll
+    for (int w = 1; w < D / 32; ++w) t += s_red[w];
+    sp.musq[row] = t;
+  }
+}
+
+template <int D>
+__global__ void __launch_bounds__(D) hva_mu_split_kernel(int Nc, const float* __restrict__ mu, MuSplit sp) {
+  const size_t row = (size_t)blockIdx.y * Nc + blockIdx.x;
+  mu_split_store<D>(sp, row, threadIdx.x, mu[row * D + threadIdx.x]);
+}
 
 template <typename T, int D>
 __global__ void __launch_bounds__(kThreads) hva_init_centroids_kernel(HvaGrid g, const T* __restrict__ X,
@@ -186,7 +220,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_kernel(ClusterParams p) {
 template <int D>
 __global__ void __launch_bounds__(D) hva_finalize_kernel(HvaGrid g, const float* __restrict__ part,
                                                          const int* __restrict__ part_cnt, float* __restrict__ mu,
-                                                         int* __restrict__ sizes, float* __restrict__ sums) {
+                                                         int* __restrict__ sizes, float* __restrict__ sums, MuSplit sp) {
   const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
   const int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
   float z = 0.f;
@@ -209,9 +243,11 @@ __global__ void __launch_bounds__(D) hva_finalize_kernel(HvaGrid g, const float*
     }
   }
   size_t o = ((size_t)bh * g.Nc + u) * D + c;
-  if (n > 0) mu[o] = __fdiv_rn(z, (float)n);
+  float m = mu[o];
+  if (n > 0) { m = __fdiv_rn(z, (float)n); mu[o] = m; }
   if (sums) sums[o] = z;
   if (c == 0) sizes[(size_t)bh * g.Nc + u] = n;
+  mu_split_store<D>(sp, (size_t)bh * g.Nc + u, c, m);
 }
 
 size_t assign_smem_bytes(const HvaGrid& g, int D, int esize) {
@@ -220,14 +256,27 @@ size_t assign_smem_bytes(const HvaGrid& g, int D, int esize) {
   return (size_t)g.nwin * D * 4 + (size_t)ctok * rowstride * esize + sizeof(int) * (ctok + g.nwin + g.nwin + 1 + ctok) + 16;
 }
 
+struct ClusterWs {
+  float* part; int* part_cnt; __nv_bfloat16 *hi, *lo; float* musq;
+};
+
 template <typename T, int D>
 int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float* mu_init, int* assign, float* mu,
-                int* sizes, float* sums, float* lowe, float* part, int* part_cnt, cudaStream_t st) {
+                int* sizes, float* sums, float* lowe, const ClusterWs& ws, int dtype, cudaStream_t st) {
   dim3 grid(g.Nc, BH);
-  size_t smem = assign_smem_bytes(g, D, sizeof(T));
-  if (smem > 227 * 1024) return HVA_EUNSUPPORTED;
-  if (cudaFuncSetAttribute(hva_assign_kernel<T, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return HVA_ECUDA;
+  const char* force = getenv("HVA_CLUSTER_SIMT");
+  const bool tc = hva_assign_tc_supported(g, D, dtype) && !(force && force[0] == '1');
+  HvaAssignTc atc;
+  size_t smem = 0;
+  if (tc) {
+    HVA_TRY(hva_assign_tc_prepare(g, BH, X, ws.hi, ws.lo, &atc));
+  } else {
+    smem = assign_smem_bytes(g, D, sizeof(T));
+    if (smem > 227 * 1024) return HVA_EUNSUPPORTED;
+    if (cudaFuncSetAttribute(hva_assign_kernel<T, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+      return HVA_ECUDA;
+  }
+  const MuSplit sp{tc ? ws.hi : nullptr, tc ? ws.lo : nullptr, ws.musq}, none{nullptr, nullptr, nullptr};
   if (mu_init) {
     if (mu_init != mu &&
         cudaMemcpyAsync(mu, mu_init, (size_t)BH * g.Nc * D * sizeof(float), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
@@ -236,12 +285,23 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
     hva_init_centroids_kernel<T, D><<<grid, kThreads, 0, st>>>(g, reinterpret_cast<const T*>(X), mu);
     HVA_CHECK_LAUNCH();
   }
+  if (tc) {
+    hva_mu_split_kernel<D><<<grid, D, 0, st>>>(g.Nc, mu, sp);
+    HVA_CHECK_LAUNCH();
+  }
+  const char* probe_env = getenv("HVA_CLUSTER_PROBE");   // debug: device float receiving the observed filter error
+  float* probe = (tc && probe_env) ? reinterpret_cast<float*>(strtoull(probe_env, nullptr, 0)) : nullptr;
   for (int it = 0; it < iters; ++it) {
     bool last = (it == iters - 1);
-    ClusterParams p{g, BH, X, mu, part, part_cnt, last ? assign : nullptr, last ? lowe : nullptr};
-    hva_assign_kernel<T, D><<<grid, kThreads, smem, st>>>(p);
-    HVA_CHECK_LAUNCH();
-    hva_finalize_kernel<D><<<grid, D, 0, st>>>(g, part, part_cnt, mu, sizes, last ? sums : nullptr);
+    if (tc) {
+      HVA_TRY(hva_assign_tc_launch(atc, g, BH, mu, ws.musq, ws.part, ws.part_cnt, last ? assign : nullptr, last ? lowe : nullptr,
+                                   probe, st));
+    } else {
+      ClusterParams p{g, BH, X, mu, ws.part, ws.part_cnt, last ? assign : nullptr, last ? lowe : nullptr};
+      hva_assign_kernel<T, D><<<grid, kThreads, smem, st>>>(p);
+      HVA_CHECK_LAUNCH();
+    }
+    hva_finalize_kernel<D><<<grid, D, 0, st>>>(g, ws.part, ws.part_cnt, mu, sizes, last ? sums : nullptr, last ? none : sp);
     HVA_CHECK_LAUNCH();
   }
   return HVA_OK;
@@ -250,7 +310,15 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
 }  // namespace
 
 size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D) {
-  return hva_align((size_t)BH * g.Nc * g.nwin * D * sizeof(float)) + hva_align((size_t)BH * g.Nc * g.nwin * sizeof(int));
+  return hva_align((size_t)BH * g.Nc * g.nwin * D * sizeof(float)) + hva_align((size_t)BH * g.Nc * g.nwin * sizeof(int)) +
+         2 * hva_align((size_t)BH * g.Nc * D * sizeof(__nv_bfloat16)) + hva_align((size_t)BH * g.Nc * sizeof(float));
+}
+
+extern "C" size_t hva_cluster_workspace_bytes(const hva_shape* s, const int32_t cell[3], const int32_t win[3]) {
+  if (!s || !cell || !win || s->B < 1 || s->heads < 1 || s->T < 1 || s->H < 1 || s->W < 1) return 0;
+  for (int a = 0; a < 3; ++a)
+    if (cell[a] < 1 || win[a] < 1) return 0;
+  return hva_cluster_ws_bytes(hva_make_grid(s, cell, win), s->B * s->heads, s->D);
 }
 
 extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int32_t win[3], int32_t iters, const void* X,
@@ -265,10 +333,17 @@ extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int3
   HvaGrid g = hva_make_grid(s, cell, win);
   int BH = s->B * s->heads;
   if (ws_bytes < hva_cluster_ws_bytes(g, BH, s->D)) return HVA_EWORKSPACE;
-  float* part = reinterpret_cast<float*>(ws);
-  int* part_cnt = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + hva_align((size_t)BH * g.Nc * g.nwin * s->D * sizeof(float)));
+  ClusterWs cw;
+  {
+    char* w = reinterpret_cast<char*>(ws);
+    cw.part = reinterpret_cast<float*>(w); w += hva_align((size_t)BH * g.Nc * g.nwin * s->D * sizeof(float));
+    cw.part_cnt = reinterpret_cast<int*>(w); w += hva_align((size_t)BH * g.Nc * g.nwin * sizeof(int));
+    cw.hi = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
+    cw.lo = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
+    cw.musq = reinterpret_cast<float*>(w);
+  }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-#define HVA_DISPATCH(T, DD) return run_cluster<T, DD>(g, BH, iters, X, mu_init, assign, mu, sizes, sums, lowe, part, part_cnt, st)
+#define HVA_DISPATCH(T, DD) return run_cluster<T, DD>(g, BH, iters, X, mu_init, assign, mu, sizes, sums, lowe, cw, s->dtype, st)
   if (s->dtype == HVA_F32) {
     if (s->D == 64) HVA_DISPATCH(float, 64);
     HVA_DISPATCH(float, 128);

@@ -124,6 +124,40 @@ def test_cluster_non_dividing_lattice_and_wide_window():
         assert run_cluster_parity(wl, [0, 1], 0) == 0
 
 
+def test_cluster_tensor_pipe_edge_shapes():
+    # tcgen05 assignment path (bf16, D=128): non-dividing lattice with zero-filled TMA rows (R-C4), even window (R-C3),
+    # windows of 12 / 48 / 75 candidates (one and several 32-column TMEM chunks), cell of exactly 128 tokens
+    for T, H, W, cell, win in ((5, 7, 9, (2, 3, 4), (3, 4, 3)), (6, 13, 21, (2, 3, 5), (3, 4, 4)), (8, 16, 16, (2, 8, 8), (3, 2, 2)),
+                               (10, 11, 12, (2, 2, 2), (3, 5, 5))):
+        wl = dataclasses.replace(inputs.C2, name="edge-tc", heads=2, T=T, H=H, W=W, cell=cell, win=win, seed=12)
+        assert run_cluster_parity(wl, [0, 1], 1) <= 1
+
+
+@pytest.mark.parametrize("wl", [inputs.C2, dataclasses.replace(inputs.C2, name="edge-tc2", T=7, H=22, W=30, cell=(3, 4, 4), seed=13)])
+def test_cluster_tensor_pipe_equals_direct_form(wl, monkeypatch):
+    """The tensor-pipe score only filters: labels, sizes, sums, mu and rho are those of the fp32 direct-form kernel,
+    bit for bit, with and without the Lowe ratio (the filter-decided fast path), and the observed filter error stays
+    far inside the margin the kernel assumes (kEpsDot = 2^-15)."""
+    b = _b()
+    heads = [0, 5]
+    (Qd, Kd, _), _ = _heads(wl, heads, f64_idx=[])
+    shape = b.make_shape(wl, heads=len(heads))
+    for X in (Qd, Kd):
+        for lowe in (False, True):
+            monkeypatch.setenv("HVA_CLUSTER_SIMT", "1")
+            ref = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X, want_lowe=lowe)
+            monkeypatch.delenv("HVA_CLUSTER_SIMT")
+            probe = torch.zeros(1, dtype=torch.float32, device="cuda")
+            monkeypatch.setenv("HVA_CLUSTER_PROBE", str(probe.data_ptr()))
+            got = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X, want_lowe=lowe)
+            monkeypatch.delenv("HVA_CLUSTER_PROBE")
+            torch.cuda.synchronize()
+            for k in ("assign", "sizes", "mu", "sums") + (("lowe",) if lowe else ()):
+                assert torch.equal(ref[k], got[k]), k
+            # observed |score_tc - score_direct| / (|x| max|mu|) against the assumed bound 2 * kEpsDot = 2^-14
+            assert 0 < float(probe.item()) < 2.0 ** -14 / 8, float(probe.item())
+
+
 def _oracle_stage_inputs(wl, heads, f64):
     """Oracle clustering of Q and K per head (the 'teacher' for the downstream stages)."""
     out = []
