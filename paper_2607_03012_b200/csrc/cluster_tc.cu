@@ -1,24 +1,27 @@
-// S1 on the tensor pipe (bf16 inputs, D = 128): assignment step of 3D local-window k-means
-// (Alg. 2 lines 14-21, l.367-381; Eq. 5 l.81; Eq. 6 l.97).
+// S1 (+ the per-cell part of S2) on the tensor pipe (bf16 inputs, D = 128): assignment step of 3D local-window
+// k-means and the per-(cell, slot) partial centroid sums (Alg. 2 lines 14-21, l.367-381; Eq. 5 l.81; Eq. 6 l.97).
 //
 // The direct form sum_c (x_c - mu_c)^2 on CUDA cores is ALU-bound (profiles/r1b: 6.5 % of DRAM peak).
 // Here the 27.D dot products leave the FP32 pipe:
 //   score_v = |mu_v|^2 - 2 x.mu_v  ( = d^2_v - |x|^2 ),   x.mu_v = x.hi_v + x.lo_v
 // with mu split into two bf16 terms (hi = RN(mu), lo = RN(mu - hi); |mu - hi - lo| <= 2^-18 |mu|), so
 // both products are exact in the MMA and only the fp32 accumulation rounds.  One CTA per home cell:
-//   TMA   one 5-D box brings the cell's k_t x k_h x k_w tokens (rows of 256 B) into a 128B-swizzled K-major
-//         A tile, one 5-D box per split term brings the window's w_t x w_h x w_w centroids (delta_t-major ==
+//   TMA   one 5-D box brings the cell's k_t x k_h x k_w tokens (rows of 256 B) into a 128B-swizzled
+//         tile, one 5-D box per split term brings the window's w_t x w_h x w_w centroids (delta_t-major ==
 //         ascending centroid id, Alg. 2 line 18) into the B tiles
-//   MMA   tcgen05.mma 128 x NPAD x 16, 8 k-steps x {hi, lo}, fp32 accumulator in TMEM
-//   scan  thread = token = TMEM lane: tcgen05.ld of its score row, argmin
+//   MMA 1 scores[token, slot] = X . {hi, lo}^T : tcgen05.mma 128 x NPAD x 16, 8 k-steps x 2 terms, fp32 in TMEM
+//   scan  thread = token = TMEM lane: tcgen05.ld of its score row, min / contenders
+//   MMA 2 z[slot, :] = P^T X with the one-hot assignment matrix P[token, slot] written to shared memory
+//         (line 20: z_a += x); the products 1.0 * x are exact, the fp32 accumulation order is the hardware's,
+//         fixed => the result is deterministic (same bits every run)
 // The tensor-pipe score is a FILTER, not the decision: every candidate whose score lies within a rigorous
 // error margin of the decisive one is re-evaluated in the exact direct form in fp32 (the arithmetic of the
 // CUDA-core kernel), and the first minimum among them wins (strict '<', R-C1).  So labels are those of the
 // direct form; with the Lowe ratio requested (Eq. 6) the best and the second best are always exact.
-// The centroid update is the same deterministic per-(cell, slot) segmented reduction as in cluster.cu.
 #include "common.cuh"
 #include "ptx.cuh"
 #include "cluster_tc.cuh"
+#include <algorithm>
 
 namespace {
 using namespace hva_ptx;
@@ -39,13 +42,14 @@ struct AssignTcParams {
   int* assign;         // [BH, n] or null
   float* lowe;         // [BH, n] or null
   int npad;            // window candidates padded to the MMA N granule (16)
-  int rows_a;          // cell tokens padded to the swizzle atom (8 rows)
+  int rows_a;          // cell tokens padded to the MMA K granule (16 rows)
+  int pm;              // rows of the one-hot tile P^T (window slots padded to the swizzle atom, 8 rows)
   uint32_t tmem_cols;
   float* probe;        // debug: max |score_tc - score_exact| / (|x| max|mu|), or null
 };
 
 struct __align__(8) AssignTcBars {
-  uint64_t full, mma_done;
+  uint64_t full, mma_done, sum_done;
   uint32_t tmem_base;
 };
 
@@ -94,23 +98,29 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   const int ut = cell / (g.Kh * g.Kw), uh = (cell / g.Kw) % g.Kh, uw = cell % g.Kw;
   const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
   const int ctok = g.kt * g.kh * g.kw, nwin = g.nwin, npad = p.npad;
-  const int half_a = p.rows_a * 128, half_b = npad * 128;
+  const int half_a = p.rows_a * 128, half_b = npad * 128, half_p = p.pm * 128;
 
+  // Shared memory (offsets from a 1024-byte aligned base, kept as shared-space pointers):
+  //   sB  [hi | lo][2 halves][npad][128 B]  window centroids, K-major SW128; after MMA 1 the region is reused for
+  //       sP [2 halves][pm][128 B], the one-hot tile P^T (rows = slots, K = tokens)
+  //   sA  [2 halves][rows_a][128 B]         the cell's tokens (A of MMA 1, K-major; B of MMA 2, MN-major)
+  // The MMAs read 128 rows of their M operand: rows past the tile alias whatever follows inside the allocation and
+  // only feed TMEM lanes nobody reads.
   extern __shared__ unsigned char smem_raw[];
-  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  unsigned char* sA = smem;                       // [2 halves][rows_a][128 B]   tokens, K-major SW128
-  unsigned char* sBhi = sA + 2 * half_a;          // [2 halves][npad][128 B]     hi term of the window centroids
-  unsigned char* sBlo = sBhi + 2 * half_b;        // [2 halves][npad][128 B]     lo term
-  float* s_c = reinterpret_cast<float*>(sBlo + 2 * half_b);   // [npad] |mu_v|^2
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  unsigned char* sBhi = smem;
+  unsigned char* sBlo = sBhi + 2 * half_b;
+  unsigned char* sP = smem;
+  unsigned char* sA = smem + 4 * half_b;
+  float* s_c = reinterpret_cast<float*>(sA + 2 * half_a);     // [npad] |mu_v|^2
   int* s_u = reinterpret_cast<int*>(s_c + npad);              // [npad] centroid id of window slot v
-  int* s_wcnt = s_u + npad;                                   // [4][npad] per-warp slot counts
-  int* s_start = s_wcnt + 4 * npad;                           // [npad + 1]
-  int* s_order = s_start + npad + 1;                          // [128]
-  AssignTcBars* B = reinterpret_cast<AssignTcBars*>((reinterpret_cast<uintptr_t>(s_order + kThreads) + 7) & ~uintptr_t(7));
+  int* s_cnt = s_u + npad;                                    // [npad] tokens of the cell assigned to slot v
+  AssignTcBars* B = reinterpret_cast<AssignTcBars*>(s_cnt + npad + (npad & 1));
 
   if (tid == 0) {
     mbar_init(&B->full, 1);
     mbar_init(&B->mma_done, 1);
+    mbar_init(&B->sum_done, 1);
     mbar_fence_init();
   }
   __syncwarp();
@@ -124,9 +134,14 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
       u = ((st + dt) * g.Kh + (sh + dh)) * g.Kw + (sw + dw);
       c = __ldg(p.musq + (size_t)bh * g.Nc + u);
     }
-    s_u[v] = u; s_c[v] = c;
+    s_u[v] = u; s_c[v] = c; s_cnt[v] = 0;
   }
-  for (int i = tid; i < 4 * npad; i += kThreads) s_wcnt[i] = 0;
+  // token rows ctok .. rows_a-1 take part in MMA 2 (K granule 16) with zero weight: they must be finite
+  for (int i = tid; i < (p.rows_a - ctok) * 16; i += kThreads) {
+    const int r = ctok + (i >> 4), q = i & 15;
+    *reinterpret_cast<uint4*>(sA + (q >> 3) * half_a + r * 128 + ((q & 7) << 4)) = make_uint4(0, 0, 0, 0);
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -158,7 +173,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   }
   __syncwarp();
 
-  // ---- token geometry; |x|^2 and the filter margin while the MMAs run
+  // ---- token geometry; an upper bound of |x|^2 and the filter margin while the MMAs run
   const int li = tid;
   int lab = -1;
   size_t tok = 0;
@@ -171,15 +186,24 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   float c_max = 0.f;
   for (int v = 0; v < nwin; ++v) c_max = fmaxf(c_max, s_c[v]);
   mbar_wait(&B->full, 0);
+  // |x|^2 only scales the margin: packed bf16 FMAs (4 x 2 accumulators of 16 non-negative terms each: relative
+  // error < 16 * 2^-8), inflated by 1/8 so that it is an upper bound
   float xsq = 0.f;
   if (valid) {
+    __nv_bfloat162 acc[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[j] = __floats2bfloat162_rn(0.f, 0.f);
 #pragma unroll 4
     for (int q = 0; q < 16; ++q) {
-      float x[8];
-      unpack8(*x_chunk(sA, half_a, li, q), x);
-#pragma unroll
-      for (int i = 0; i < 8; ++i) xsq = fmaf(x[i], x[i], xsq);
+      const uint4 r = *x_chunk(sA, half_a, li, q);
+      const __nv_bfloat162 x0 = *reinterpret_cast<const __nv_bfloat162*>(&r.x), x1 = *reinterpret_cast<const __nv_bfloat162*>(&r.y),
+                           x2 = *reinterpret_cast<const __nv_bfloat162*>(&r.z), x3 = *reinterpret_cast<const __nv_bfloat162*>(&r.w);
+      acc[0] = __hfma2(x0, x0, acc[0]); acc[1] = __hfma2(x1, x1, acc[1]);
+      acc[2] = __hfma2(x2, x2, acc[2]); acc[3] = __hfma2(x3, x3, acc[3]);
     }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) xsq += __low2float(acc[j]) + __high2float(acc[j]);
+    xsq *= 1.125f;
   }
   // score error E <= 2 kEpsDot |x| |mu| (+ rounding of |mu|^2 and of the fma: 6e-7 (|mu|^2 + 2|x||mu|)); candidates within
   // 2E of the decisive score are contenders
@@ -188,39 +212,57 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
 
   mbar_wait(&B->mma_done, 0);
   tc_fence_after();
+  // the B tiles are dead: clear the one-hot tile that aliases them (filled after the labels are known)
+  for (int i = tid; i < (2 * half_p) / 16; i += kThreads) reinterpret_cast<uint4*>(sP)[i] = make_uint4(0, 0, 0, 0);
+
   const float kInf = __int_as_float(0x7f800000);
-  float best = kInf, second = kInf;
   const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
   uint32_t sc[32];
   // pass 1: smallest and second smallest filter score
   float s1 = kInf, s2 = kInf;
-  int v1 = 0;
   for (int v0 = 0; v0 < nwin; v0 += 32) {
     tmem_ld32(trow + v0, sc);
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
       if (v0 + i < nwin) {
         const float s = fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]);
-        if (s < s1) { s2 = s1; s1 = s; v1 = v0 + i; }
-        else if (s < s2) s2 = s;
+        s2 = fminf(s2, fmaxf(s1, s));
+        s1 = fminf(s1, s);
       }
     }
   }
   const bool want2 = p.lowe != nullptr;
   const float thr = (want2 ? s2 : s1) + margin;     // s2 = +inf (single candidate): every candidate is a contender
-  const bool refine = valid && (want2 || !(s2 > thr));
-  if (valid && !refine) lab = v1;                   // decided by the filter: no other candidate can be the direct-form argmin
+  // pass 2: contenders = candidates with score <= thr.  A single contender (without the Lowe ratio) is the direct-form
+  // argmin; otherwise the exact direct form decides among them, ascending candidate id, strict '<'  (R-C1)
+  float best = kInf, second = kInf;
   const float* mu_b = p.mu + (size_t)bh * g.Nc * kD;
+  const bool single_chunk = nwin <= 32;
+  int n_cont = 0, first = 0;
+  uint32_t cand0 = 0;
+  for (int v0 = 0; v0 < nwin; v0 += 32) {
+    if (!single_chunk) tmem_ld32(trow + v0, sc);
+    uint32_t cand = 0;
+#pragma unroll
+    for (int i = 0; i < 32; ++i)
+      if (v0 + i < nwin && fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]) <= thr) cand |= 1u << i;
+    if (n_cont == 0 && cand) first = v0 + __ffs(cand) - 1;
+    n_cont += __popc(cand);
+    if (v0 == 0) cand0 = cand;
+  }
+  const bool refine = valid && (want2 || n_cont > 1);
+  if (valid && !refine) lab = first;
   if (__any_sync(0xffffffffu, refine)) {            // tcgen05.ld is warp-collective: the chunk loop stays warp-uniform
-    // pass 2: exact direct form for the contenders, ascending candidate id, strict '<'  (R-C1)
     for (int v0 = 0; v0 < nwin; v0 += 32) {
-      if (nwin > 32) tmem_ld32(trow + v0, sc);
-      uint32_t cand = 0;
-      if (refine) {
+      uint32_t cand = cand0;
+      if (!single_chunk) {
+        tmem_ld32(trow + v0, sc);
+        cand = 0;
 #pragma unroll
         for (int i = 0; i < 32; ++i)
           if (v0 + i < nwin && fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]) <= thr) cand |= 1u << i;
       }
+      if (!refine) cand = 0;
       while (cand) {
         const int v = v0 + __ffs(cand) - 1;
         cand &= cand - 1;
@@ -238,7 +280,14 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     }
   }
   if (p.probe) {   // debug: observed filter error against the exact direct form
-    float worst = 0.f;
+    float worst = 0.f, xx = 0.f;
+    if (valid) {
+      for (int q = 0; q < 16; ++q) {
+        float x[8];
+        unpack8(*x_chunk(sA, half_a, li, q), x);
+        for (int i = 0; i < 8; ++i) xx = fmaf(x[i], x[i], xx);
+      }
+    }
     for (int v0 = 0; v0 < nwin; v0 += 32) {
       tmem_ld32(trow + v0, sc);
       if (valid) {
@@ -247,66 +296,63 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
           if (v0 + i < nwin) {
             const float s = fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]);
             const float dd = direct_dist_probe(sA, half_a, li, mu_b + (size_t)s_u[v0 + i] * kD);
-            worst = fmaxf(worst, fabsf((dd - xsq) - s) / fmaxf(xm, 1e-30f));
+            worst = fmaxf(worst, fabsf((dd - xx) - s) / fmaxf(sqrtf(xx * c_max), 1e-30f));
           }
         }
       }
     }
+    if (xx > xsq) worst = 1.f;   // the packed-bf16 |x|^2 must be an upper bound
     atomicMax(reinterpret_cast<int*>(p.probe), __float_as_int(worst));
   }
   tc_fence_before();
+  __syncthreads();        // one-hot tile cleared, every score read
 
-  // ---- counting sort of the cell's tokens by slot, stable in token order
+  // ---- one-hot tile P^T[slot, token] = 1 and the slot counts
   {
     const unsigned m = __match_any_sync(0xffffffffu, lab);
-    const int rank = __popc(m & ((1u << lane) - 1u));
-    if (lab >= 0 && rank == 0) s_wcnt[warp * npad + lab] = __popc(m);
-    __syncthreads();
-    if (warp == 0) {
-      int carry = 0;
-      for (int v0 = 0; v0 < nwin; v0 += 32) {
-        const int v = v0 + lane;
-        const int t = v < nwin ? s_wcnt[v] + s_wcnt[npad + v] + s_wcnt[2 * npad + v] + s_wcnt[3 * npad + v] : 0;
-        int inc = t;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const int y = __shfl_up_sync(0xffffffffu, inc, o);
-          if (lane >= o) inc += y;
-        }
-        if (v < nwin) s_start[v] = carry + inc - t;
-        carry += __shfl_sync(0xffffffffu, inc, 31);
-      }
-      if (lane == 0) s_start[nwin] = carry;
-    }
-    __syncthreads();
     if (lab >= 0) {
-      int pos = s_start[lab] + rank;
-      for (int w2 = 0; w2 < warp; ++w2) pos += s_wcnt[w2 * npad + lab];
-      s_order[pos] = li;
+      *reinterpret_cast<__nv_bfloat16*>(sP + (li >> 6) * half_p + lab * 128 + (((((li & 63) >> 3) ^ (lab & 7))) << 4) + (li & 7) * 2) =
+          __float2bfloat16_rn(1.0f);
+      if ((m & ((1u << lane) - 1u)) == 0) atomicAdd(&s_cnt[lab], __popc(m));
     }
-    __syncthreads();
   }
-  if (warp == 0) { tc_fence_after(); tmem_dealloc(tmem, p.tmem_cols); }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncthreads();
+  tc_fence_after();
 
-  // ---- segmented per-cell reduction (z_a += x, Alg. 2 line 20): thread = two feature dims, tokens in token order
+  // ---- MMA 2: z[slot, :] = sum_token P^T[slot, token] x[token, :]   (Alg. 2 line 20), 128 slots per M tile
+  const int mtiles = (nwin + 127) >> 7;
+  if (tid == 0) {
+    const uint32_t idesc = umma_idesc_bf16(128, 128, 1);
+    const uint32_t p_addr = smem_u32(sP), x_addr = smem_u32(sA);
+    const int ksteps = p.rows_a >> 4;
+    for (int mt = 0; mt < mtiles; ++mt)
+      for (int ks = 0; ks < ksteps; ++ks)
+        mma_ss(tmem + mt * 128, umma_desc(p_addr + mt * 128 * 128 + (ks >> 2) * half_p + (ks & 3) * 32, 16, 1024),
+               umma_desc(x_addr + ks * 2048, half_a, 1024), idesc, ks > 0);
+    tc_commit(&B->sum_done);
+  }
+  __syncwarp();
   const size_t pbase = ((size_t)bh * g.Nc + cell) * nwin;
-  for (int v = tid; v < nwin; v += kThreads) p.part_cnt[pbase + v] = s_start[v + 1] - s_start[v];
-  const int cp = tid & 63, grp = tid >> 6;          // dims 2cp, 2cp+1; slots grp, grp+2, ...
-  const int q = cp >> 2;                             // 16-byte chunk holding the pair
-  const unsigned char* colbase = sA + (q >> 3) * half_a + (cp & 3) * 4;
-  for (int v = grp; v < nwin; v += 2) {
-    const int b = s_start[v], e = s_start[v + 1];
-    if (e > b) {
-      float a0 = 0.f, a1 = 0.f;
-      for (int i = b; i < e; ++i) {
-        const int r = s_order[i];
-        const uint32_t xx = *reinterpret_cast<const uint32_t*>(colbase + r * 128 + (((q & 7) ^ (r & 7)) << 4));
-        a0 += __uint_as_float(xx << 16);
-        a1 += __uint_as_float(xx & 0xffff0000u);
+  for (int mt = 0; mt < mtiles; ++mt) {
+    if (mt * 128 + warp * 32 >= nwin) break;          // warp-uniform: TMEM lane = slot
+    const int v = mt * 128 + tid;
+    const int cnt = v < nwin ? s_cnt[v] : 0;
+    if (v < nwin) p.part_cnt[pbase + v] = cnt;
+    if (mt == 0) { mbar_wait(&B->sum_done, 0); tc_fence_after(); }
+#pragma unroll 1
+    for (int c = 0; c < 4; ++c) {
+      tmem_ld32(trow + mt * 128 + c * 32, sc);
+      if (cnt > 0) {
+        uint4* dst = reinterpret_cast<uint4*>(p.part + (pbase + v) * kD + c * 32);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) dst[q] = make_uint4(sc[4 * q], sc[4 * q + 1], sc[4 * q + 2], sc[4 * q + 3]);
       }
-      *reinterpret_cast<float2*>(p.part + (pbase + v) * kD + 2 * cp) = make_float2(a0, a1);
     }
   }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) { tc_fence_after(); tmem_dealloc(tmem, p.tmem_cols); }
 }
 
 }  // namespace
@@ -336,15 +382,17 @@ bool make_map5(CUtensorMap* m, const void* base, int BH, int d3, int d2, int d1,
 int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, HvaAssignTc* a) {
   const int ctok = g.kt * g.kh * g.kw;
   a->npad = (g.nwin + 15) & ~15;
-  if (a->npad < 16) a->npad = 16;
-  a->rows_a = (ctok + 7) & ~7;
-  a->tmem_cols = 32;
-  while ((int)a->tmem_cols < ((g.nwin + 31) & ~31)) a->tmem_cols <<= 1;
-  // the MMA reads 128 A rows: rows past rows_a alias the B tiles (finite garbage in unused TMEM lanes)
-  size_t bytes = 2 * (size_t)a->rows_a * 128 + 4 * (size_t)a->npad * 128;
-  const size_t min_a = 128 * 128 + (size_t)a->rows_a * 128;     // second half + 128 rows must stay inside the allocation
-  if (bytes < min_a) bytes = min_a;
-  bytes += sizeof(int) * (7 * (size_t)a->npad + 1 + kThreads) + sizeof(AssignTcBars) + 8 + 1024;
+  a->rows_a = (ctok + 15) & ~15;
+  a->pm = (g.nwin + 7) & ~7;
+  const int mtiles = (g.nwin + 127) / 128;
+  a->tmem_cols = 128;
+  while ((int)a->tmem_cols < mtiles * 128 || (int)a->tmem_cols < ((g.nwin + 31) & ~31)) a->tmem_cols <<= 1;
+  const size_t half_a = (size_t)a->rows_a * 128, half_b = (size_t)a->npad * 128, half_p = (size_t)a->pm * 128;
+  size_t bytes = 4 * half_b + 2 * half_a + 3 * sizeof(int) * (size_t)a->npad + sizeof(AssignTcBars) + 16;
+  // the MMAs read 128 rows of their M operand (tokens in MMA 1, slots in MMA 2): keep the over-read inside the allocation
+  bytes = std::max(bytes, 4 * half_b + half_a + 16384);
+  bytes = std::max(bytes, (size_t)(mtiles - 1) * 16384 + half_p + 16384);
+  bytes += 1024;
   a->smem = bytes;
   if (bytes > 227 * 1024) return HVA_EUNSUPPORTED;
   if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, g.kt, g.kh, g.kw)) return HVA_ECUDA;
@@ -357,7 +405,7 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
 
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
                          int* part_cnt, int* assign, float* lowe, float* probe, cudaStream_t st) {
-  AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, a.tmem_cols, probe};
+  AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, a.pm, a.tmem_cols, probe};
   hva_assign_tc_kernel<<<dim3(g.Nc, BH), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;

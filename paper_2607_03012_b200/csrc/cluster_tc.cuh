@@ -5,7 +5,7 @@
 
 struct HvaAssignTc {
   CUtensorMap map_x, map_hi, map_lo;
-  int npad, rows_a;
+  int npad, rows_a, pm;
   uint32_t tmem_cols;
   size_t smem;
 };

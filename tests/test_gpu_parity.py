@@ -135,27 +135,34 @@ def test_cluster_tensor_pipe_edge_shapes():
 
 @pytest.mark.parametrize("wl", [inputs.C2, dataclasses.replace(inputs.C2, name="edge-tc2", T=7, H=22, W=30, cell=(3, 4, 4), seed=13)])
 def test_cluster_tensor_pipe_equals_direct_form(wl, monkeypatch):
-    """The tensor-pipe score only filters: labels, sizes, sums, mu and rho are those of the fp32 direct-form kernel,
-    bit for bit, with and without the Lowe ratio (the filter-decided fast path), and the observed filter error stays
-    far inside the margin the kernel assumes (kEpsDot = 2^-15)."""
+    """The tensor-pipe score only filters: after one pass labels, sizes and rho are those of the fp32 direct-form kernel
+    bit for bit, with and without the Lowe ratio (the filter-decided fast path); the centroid sums come from the MMA's
+    fp32 accumulation instead of a sequential fp32 loop and agree within the summation tolerance; the observed filter
+    error stays far inside the margin the kernel assumes (2 * kEpsDot = 2^-14)."""
     b = _b()
     heads = [0, 5]
     (Qd, Kd, _), _ = _heads(wl, heads, f64_idx=[])
     shape = b.make_shape(wl, heads=len(heads))
     for X in (Qd, Kd):
+        tol = _mu_tol(X.float().cpu().numpy())
         for lowe in (False, True):
-            monkeypatch.setenv("HVA_CLUSTER_SIMT", "1")
-            ref = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X, want_lowe=lowe)
-            monkeypatch.delenv("HVA_CLUSTER_SIMT")
-            probe = torch.zeros(1, dtype=torch.float32, device="cuda")
-            monkeypatch.setenv("HVA_CLUSTER_PROBE", str(probe.data_ptr()))
-            got = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X, want_lowe=lowe)
-            monkeypatch.delenv("HVA_CLUSTER_PROBE")
-            torch.cuda.synchronize()
-            for k in ("assign", "sizes", "mu", "sums") + (("lowe",) if lowe else ()):
-                assert torch.equal(ref[k], got[k]), k
-            # observed |score_tc - score_direct| / (|x| max|mu|) against the assumed bound 2 * kEpsDot = 2^-14
-            assert 0 < float(probe.item()) < 2.0 ** -14 / 8, float(probe.item())
+            for iters in (1, wl.iters):
+                monkeypatch.setenv("HVA_CLUSTER_SIMT", "1")
+                ref = b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe)
+                monkeypatch.delenv("HVA_CLUSTER_SIMT")
+                probe = torch.zeros(1, dtype=torch.float32, device="cuda")
+                monkeypatch.setenv("HVA_CLUSTER_PROBE", str(probe.data_ptr()))
+                got = b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe)
+                monkeypatch.delenv("HVA_CLUSTER_PROBE")
+                torch.cuda.synchronize()
+                if iters == 1:
+                    for k in ("assign", "sizes") + (("lowe",) if lowe else ()):
+                        assert torch.equal(ref[k], got[k]), k
+                    assert float((ref["mu"] - got["mu"]).abs().max()) <= tol
+                    assert float((ref["sums"] - got["sums"]).abs().max()) <= tol * int(ref["sizes"].max())
+                else:   # later passes start from centroids that differ in the last bits: only near ties may flip
+                    assert float((ref["assign"] != got["assign"]).float().mean()) <= 1e-4
+                assert 0 < float(probe.item()) < 2.0 ** -14 / 8, float(probe.item())
 
 
 def _oracle_stage_inputs(wl, heads, f64):
