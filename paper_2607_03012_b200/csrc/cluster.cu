@@ -215,39 +215,71 @@ __global__ void __launch_bounds__(kThreads) hva_assign_kernel(ClusterParams p) {
   }
 }
 
+// Home cells g (one axis) whose clipped window [start(g), start(g)+w) contains centroid coordinate u: a contiguous range.
+__device__ __forceinline__ void axis_cells(int u, int w, int K, int& lo, int& cnt) {
+  lo = 0; cnt = 0;
+  for (int gc = max(0, u - w); gc <= min(K - 1, u + w); ++gc) {
+    const int s0 = hva_win_start(gc, w, K);
+    if (u >= s0 && u < s0 + w) { if (cnt == 0) lo = gc; ++cnt; }
+  }
+}
+
 // mu_u <- z_u / n_u if n_u > 0 else mu_u   (Alg. 2 lines 22-23).  z_u = sum over the home cells g whose
-// window contains u of part[g][slot(u in g)], in ascending cell order (fixed => deterministic).
+// window contains u of part[g][slot(u in g)], in ascending cell order (fixed => deterministic).  Warp 0 lists the
+// non-empty (cell, slot) partials of u in shared memory (ordered ballot compaction); every thread (= feature dim)
+// then adds its column over that list.
 template <int D>
 __global__ void __launch_bounds__(D) hva_finalize_kernel(HvaGrid g, const float* __restrict__ part,
                                                          const int* __restrict__ part_cnt, float* __restrict__ mu,
                                                          int* __restrict__ sizes, float* __restrict__ sums, MuSplit sp) {
   const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
   const int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
-  float z = 0.f;
-  int n = 0;
-  for (int gt = max(0, ut - g.wt); gt <= min(g.Kt - 1, ut + g.wt); ++gt) {
-    int st = hva_win_start(gt, g.wt, g.Kt);
-    if (ut < st || ut >= st + g.wt) continue;
-    for (int gh = max(0, uh - g.wh); gh <= min(g.Kh - 1, uh + g.wh); ++gh) {
-      int sh = hva_win_start(gh, g.wh, g.Kh);
-      if (uh < sh || uh >= sh + g.wh) continue;
-      for (int gw = max(0, uw - g.ww); gw <= min(g.Kw - 1, uw + g.ww); ++gw) {
-        int sw = hva_win_start(gw, g.ww, g.Kw);
-        if (uw < sw || uw >= sw + g.ww) continue;
-        int cell = (gt * g.Kh + gh) * g.Kw + gw;
-        int slot = ((ut - st) * g.wh + (uh - sh)) * g.ww + (uw - sw);
-        size_t idx = ((size_t)bh * g.Nc + cell) * g.nwin + slot;
-        int k = part_cnt[idx];
-        if (k > 0) { z += part[idx * D + c]; n += k; }
+  __shared__ unsigned s_idx[1024];     // at most nwin <= 1024 home cells have u in their window (checked by hva_cluster)
+  __shared__ int s_m, s_n;
+  if (c < 32) {
+    int lt, nt, lh, nh, lw, nw;
+    axis_cells(ut, g.wt, g.Kt, lt, nt);
+    axis_cells(uh, g.wh, g.Kh, lh, nh);
+    axis_cells(uw, g.ww, g.Kw, lw, nw);
+    const int total = nt * nh * nw;
+    int m = 0, n = 0;
+    for (int e0 = 0; e0 < total; e0 += 32) {
+      const int e = e0 + c;
+      int k = 0;
+      unsigned idx = 0;
+      if (e < total) {
+        const int gt = lt + e / (nh * nw), gh = lh + (e / nw) % nh, gw = lw + e % nw;
+        const int cell = (gt * g.Kh + gh) * g.Kw + gw;
+        const int slot = ((ut - hva_win_start(gt, g.wt, g.Kt)) * g.wh + (uh - hva_win_start(gh, g.wh, g.Kh))) * g.ww +
+                         (uw - hva_win_start(gw, g.ww, g.Kw));
+        idx = (unsigned)(((size_t)bh * g.Nc + cell) * g.nwin + slot);
+        k = part_cnt[idx];
       }
+      const unsigned bal = __ballot_sync(0xffffffffu, k > 0);
+      if (k > 0) s_idx[m + __popc(bal & ((1u << c) - 1u))] = idx;
+      m += __popc(bal);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) k += __shfl_xor_sync(0xffffffffu, k, o);
+      n += k;
     }
+    if (c == 0) { s_m = m; s_n = n; }
   }
+  __syncthreads();
+  const int m = s_m, n = s_n;
+  float z = 0.f;
+  int e = 0;
+  for (; e + 4 <= m; e += 4) {
+    const float p0 = part[(size_t)s_idx[e] * D + c], p1 = part[(size_t)s_idx[e + 1] * D + c];
+    const float p2 = part[(size_t)s_idx[e + 2] * D + c], p3 = part[(size_t)s_idx[e + 3] * D + c];
+    z += p0; z += p1; z += p2; z += p3;
+  }
+  for (; e < m; ++e) z += part[(size_t)s_idx[e] * D + c];
   size_t o = ((size_t)bh * g.Nc + u) * D + c;
-  float m = mu[o];
-  if (n > 0) { m = __fdiv_rn(z, (float)n); mu[o] = m; }
+  float mval = mu[o];
+  if (n > 0) { mval = __fdiv_rn(z, (float)n); mu[o] = mval; }
   if (sums) sums[o] = z;
   if (c == 0) sizes[(size_t)bh * g.Nc + u] = n;
-  mu_split_store<D>(sp, (size_t)bh * g.Nc + u, c, m);
+  mu_split_store<D>(sp, (size_t)bh * g.Nc + u, c, mval);
 }
 
 size_t assign_smem_bytes(const HvaGrid& g, int D, int esize) {
@@ -332,6 +364,7 @@ extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int3
   if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
   HvaGrid g = hva_make_grid(s, cell, win);
   int BH = s->B * s->heads;
+  if (g.nwin > 1024 || (size_t)BH * g.Nc * g.nwin >= (1ull << 32)) return HVA_EUNSUPPORTED;
   if (ws_bytes < hva_cluster_ws_bytes(g, BH, s->D)) return HVA_EWORKSPACE;
   ClusterWs cw;
   {
