@@ -43,7 +43,7 @@ struct AssignTcParams {
   float* lowe;         // [BH, n] or null
   int npad;            // window candidates padded to the MMA N granule (16)
   int rows_a;          // cell tokens padded to the MMA K granule (16 rows)
-  int pm;              // rows of the one-hot tile P^T (window slots padded to the swizzle atom, 8 rows)
+  uint32_t m_khw, m_kw, m_whw, m_ww;   // fast_div multipliers for k_h k_w, k_w, w_h w_w, w_w
   uint32_t tmem_cols;
   float* probe;        // debug: max |score_tc - score_exact| / (|x| max|mu|), or null
 };
@@ -90,22 +90,27 @@ __device__ __noinline__ float direct_dist_probe(const unsigned char* sA, int hal
   return direct_dist(sA, half_bytes, r, mu);
 }
 
+// x / d for 0 <= x, x * d < 2^32 by one multiply-high (m = ceil(2^32 / d); d == 1 is passed as m = 0)
+__device__ __forceinline__ int fast_div(int x, uint32_t m) { return m ? (int)__umulhi((uint32_t)x, m) : x; }
+
+// One CTA per home cell: grid = (K_w, K_h, K_t * BH), 128 threads, thread = token row of the cell = TMEM lane.
 __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_hi,
                                                                  const __grid_constant__ CUtensorMap map_lo, AssignTcParams p) {
   const HvaGrid& g = p.g;
-  const int cell = blockIdx.x, bh = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int ut = cell / (g.Kh * g.Kw), uh = (cell / g.Kw) % g.Kh, uw = cell % g.Kw;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int uw = blockIdx.x, uh = blockIdx.y, bh = blockIdx.z / g.Kt, ut = blockIdx.z - bh * g.Kt;
+  const int cell = (ut * g.Kh + uh) * g.Kw + uw;
   const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
   const int ctok = g.kt * g.kh * g.kw, nwin = g.nwin, npad = p.npad;
-  const int half_a = p.rows_a * 128, half_b = npad * 128, half_p = p.pm * 128;
+  const int half_a = p.rows_a * 128, half_b = npad * 128;
 
   // Shared memory (offsets from a 1024-byte aligned base, kept as shared-space pointers):
-  //   sB  [hi | lo][2 halves][npad][128 B]  window centroids, K-major SW128; after MMA 1 the region is reused for
-  //       sP [2 halves][pm][128 B], the one-hot tile P^T (rows = slots, K = tokens)
-  //   sA  [2 halves][rows_a][128 B]         the cell's tokens (A of MMA 1, K-major; B of MMA 2, MN-major)
-  // The MMAs read 128 rows of their M operand: rows past the tile alias whatever follows inside the allocation and
-  // only feed TMEM lanes nobody reads.
+  //   sB  [hi | lo][2 halves][npad][128 B]  window centroids, K-major SW128; after MMA 1 the hi part is reused for
+  //       sP [2 halves][npad][128 B], the one-hot tile P^T (rows = slots, K = tokens; B of MMA 2, K-major)
+  //   sA  [2 halves][rows_a][128 B]         the cell's tokens (A of MMA 1, K-major; A of MMA 2, MN-major)
+  // MMA 1 reads 128 token rows: rows past the tile alias whatever follows inside the allocation and only feed TMEM
+  // lanes nobody reads.
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   unsigned char* sBhi = smem;
@@ -115,28 +120,37 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   float* s_c = reinterpret_cast<float*>(sA + 2 * half_a);     // [npad] |mu_v|^2
   int* s_u = reinterpret_cast<int*>(s_c + npad);              // [npad] centroid id of window slot v
   int* s_cnt = s_u + npad;                                    // [npad] tokens of the cell assigned to slot v
-  AssignTcBars* B = reinterpret_cast<AssignTcBars*>(s_cnt + npad + (npad & 1));
+  AssignTcBars* B = reinterpret_cast<AssignTcBars*>(s_cnt + npad);
 
   if (tid == 0) {
     mbar_init(&B->full, 1);
     mbar_init(&B->mma_done, 1);
     mbar_init(&B->sum_done, 1);
     mbar_fence_init();
+    // the loads need nothing but the barrier: issue them before any other set-up work
+    mbar_expect_tx(&B->full, (uint32_t)(2 * ctok * 128 + 4 * nwin * 128));
+    tma_load_5d(&map_x, &B->full, sA, 0, uw * g.kw, uh * g.kh, ut * g.kt, bh);
+    tma_load_5d(&map_x, &B->full, sA + half_a, 64, uw * g.kw, uh * g.kh, ut * g.kt, bh);
+    tma_load_5d(&map_hi, &B->full, sBhi, 0, sw, sh, st, bh);
+    tma_load_5d(&map_hi, &B->full, sBhi + half_b, 64, sw, sh, st, bh);
+    tma_load_5d(&map_lo, &B->full, sBlo, 0, sw, sh, st, bh);
+    tma_load_5d(&map_lo, &B->full, sBlo + half_b, 64, sw, sh, st, bh);
   }
   __syncwarp();
   if (warp == 0) tmem_alloc(&B->tmem_base, p.tmem_cols);
-  // window slot -> centroid id (ascending == delta_t-major, Alg. 2 line 18), |mu|^2
-  for (int v = tid; v < npad; v += kThreads) {
+  // window slot -> centroid id (ascending == delta_t-major, Alg. 2 line 18), |mu|^2   (warps 1..3)
+  for (int v = tid - 32; v < npad; v += kThreads - 32) {
+    if (v < 0) continue;
     int u = 0;
     float c = 0.f;
     if (v < nwin) {
-      const int dt = v / (g.wh * g.ww), dh = (v / g.ww) % g.wh, dw = v % g.ww;
+      const int dt = fast_div(v, p.m_whw), r = v - dt * g.wh * g.ww, dh = fast_div(r, p.m_ww), dw = r - dh * g.ww;
       u = ((st + dt) * g.Kh + (sh + dh)) * g.Kw + (sw + dw);
       c = __ldg(p.musq + (size_t)bh * g.Nc + u);
     }
     s_u[v] = u; s_c[v] = c; s_cnt[v] = 0;
   }
-  // token rows ctok .. rows_a-1 take part in MMA 2 (K granule 16) with zero weight: they must be finite
+  // token rows ctok .. rows_a-1 take part in MMA 2 (K granule 16) with zero weight: they must be finite; TMA never writes them
   for (int i = tid; i < (p.rows_a - ctok) * 16; i += kThreads) {
     const int r = ctok + (i >> 4), q = i & 15;
     *reinterpret_cast<uint4*>(sA + (q >> 3) * half_a + r * 128 + ((q & 7) << 4)) = make_uint4(0, 0, 0, 0);
@@ -148,16 +162,9 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   const uint32_t tmem = B->tmem_base;
 
   if (tid == 0) {
-    mbar_expect_tx(&B->full, (uint32_t)(2 * ctok * 128 + 4 * nwin * 128));
-    tma_load_5d(&map_x, &B->full, sA, 0, uw * g.kw, uh * g.kh, ut * g.kt, bh);
-    tma_load_5d(&map_x, &B->full, sA + half_a, 64, uw * g.kw, uh * g.kh, ut * g.kt, bh);
-    tma_load_5d(&map_hi, &B->full, sBhi, 0, sw, sh, st, bh);
-    tma_load_5d(&map_hi, &B->full, sBhi + half_b, 64, sw, sh, st, bh);
-    tma_load_5d(&map_lo, &B->full, sBlo, 0, sw, sh, st, bh);
-    tma_load_5d(&map_lo, &B->full, sBlo + half_b, 64, sw, sh, st, bh);
     mbar_wait(&B->full, 0);
     tc_fence_after();
-    const uint32_t idesc = umma_idesc_bf16(128, (uint32_t)npad, 0);
+    const uint32_t idesc = umma_idesc_bf16(128, (uint32_t)npad, 0, 0);
     const uint32_t a_addr = smem_u32(sA), hi_addr = smem_u32(sBhi), lo_addr = smem_u32(sBlo);
 #pragma unroll
     for (int ks = 0; ks < kD / 16; ++ks) {
@@ -178,13 +185,16 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   int lab = -1;
   size_t tok = 0;
   {
-    const int dt = li / (g.kh * g.kw), dh = (li / g.kw) % g.kh, dw = li % g.kw;
+    const int dt = fast_div(li, p.m_khw), r = li - dt * g.kh * g.kw, dh = fast_div(r, p.m_kw), dw = r - dh * g.kw;
     const int t = ut * g.kt + dt, h = uh * g.kh + dh, w = uw * g.kw + dw;
     if (li < ctok && t < g.T && h < g.H && w < g.W) { lab = 0; tok = (size_t)(t * g.H + h) * g.W + w; }
   }
   const bool valid = lab == 0;
   float c_max = 0.f;
-  for (int v = 0; v < nwin; ++v) c_max = fmaxf(c_max, s_c[v]);
+  for (int v = 0; v < npad; v += 4) {
+    const float4 c4 = *reinterpret_cast<const float4*>(s_c + v);
+    c_max = fmaxf(fmaxf(c_max, fmaxf(c4.x, c4.y)), fmaxf(c4.z, c4.w));
+  }
   mbar_wait(&B->full, 0);
   // |x|^2 only scales the margin: packed bf16 FMAs (4 x 2 accumulators of 16 non-negative terms each: relative
   // error < 16 * 2^-8), inflated by 1/8 so that it is an upper bound
@@ -193,7 +203,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     __nv_bfloat162 acc[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[j] = __floats2bfloat162_rn(0.f, 0.f);
-#pragma unroll 4
+#pragma unroll 8
     for (int q = 0; q < 16; ++q) {
       const uint4 r = *x_chunk(sA, half_a, li, q);
       const __nv_bfloat162 x0 = *reinterpret_cast<const __nv_bfloat162*>(&r.x), x1 = *reinterpret_cast<const __nv_bfloat162*>(&r.y),
@@ -212,25 +222,39 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
 
   mbar_wait(&B->mma_done, 0);
   tc_fence_after();
-  // the B tiles are dead: clear the one-hot tile that aliases them (filled after the labels are known)
-  for (int i = tid; i < (2 * half_p) / 16; i += kThreads) reinterpret_cast<uint4*>(sP)[i] = make_uint4(0, 0, 0, 0);
+  // the B tiles are dead: clear the one-hot tile that aliases the hi part (filled after the labels are known)
+  for (int i = tid; i < (2 * half_b) / 16; i += kThreads) reinterpret_cast<uint4*>(sP)[i] = make_uint4(0, 0, 0, 0);
 
   const float kInf = __int_as_float(0x7f800000);
   const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
-  uint32_t sc[32];
-  // pass 1: smallest and second smallest filter score
-  float s1 = kInf, s2 = kInf;
-  for (int v0 = 0; v0 < nwin; v0 += 32) {
-    tmem_ld32(trow + v0, sc);
+  float sv[32];
+  // scores of one 32-candidate chunk: sv[j] = |mu_v|^2 - 2 x.mu_v, +inf past the window
+  auto load_scores = [&](int v0) {
+    uint32_t raw[32];
+    tmem_ld32(trow + v0, raw);
 #pragma unroll
-    for (int i = 0; i < 32; ++i) {
-      if (v0 + i < nwin) {
-        const float s = fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]);
-        s2 = fminf(s2, fmaxf(s1, s));
-        s1 = fminf(s1, s);
-      }
+    for (int j = 0; j < 32; j += 4) {
+      const float4 c4 = *reinterpret_cast<const float4*>(s_c + v0 + j);   // npad is a multiple of 16
+      sv[j] = v0 + j < nwin ? fmaf(-2.f, __uint_as_float(raw[j]), c4.x) : kInf;
+      sv[j + 1] = v0 + j + 1 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 1]), c4.y) : kInf;
+      sv[j + 2] = v0 + j + 2 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 2]), c4.z) : kInf;
+      sv[j + 3] = v0 + j + 3 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 3]), c4.w) : kInf;
+    }
+  };
+  // pass 1: smallest and second smallest filter score (two independent chains, merged)
+  float s1 = kInf, s2 = kInf, r1 = kInf, r2 = kInf;
+  for (int v0 = 0; v0 < nwin; v0 += 32) {
+    load_scores(v0);
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+      s2 = fminf(s2, fmaxf(s1, sv[j]));
+      s1 = fminf(s1, sv[j]);
+      r2 = fminf(r2, fmaxf(r1, sv[j + 1]));
+      r1 = fminf(r1, sv[j + 1]);
     }
   }
+  s2 = fminf(fminf(s2, r2), fmaxf(s1, r1));
+  s1 = fminf(s1, r1);
   const bool want2 = p.lowe != nullptr;
   const float thr = (want2 ? s2 : s1) + margin;     // s2 = +inf (single candidate): every candidate is a contender
   // pass 2: contenders = candidates with score <= thr.  A single contender (without the Lowe ratio) is the direct-form
@@ -241,11 +265,14 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   int n_cont = 0, first = 0;
   uint32_t cand0 = 0;
   for (int v0 = 0; v0 < nwin; v0 += 32) {
-    if (!single_chunk) tmem_ld32(trow + v0, sc);
-    uint32_t cand = 0;
+    if (!single_chunk) load_scores(v0);
+    uint32_t cand = 0, cand_b = 0;
 #pragma unroll
-    for (int i = 0; i < 32; ++i)
-      if (v0 + i < nwin && fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]) <= thr) cand |= 1u << i;
+    for (int j = 0; j < 32; j += 2) {
+      if (sv[j] <= thr) cand |= 1u << j;
+      if (sv[j + 1] <= thr) cand_b |= 2u << j;
+    }
+    cand |= cand_b;
     if (n_cont == 0 && cand) first = v0 + __ffs(cand) - 1;
     n_cont += __popc(cand);
     if (v0 == 0) cand0 = cand;
@@ -256,11 +283,11 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     for (int v0 = 0; v0 < nwin; v0 += 32) {
       uint32_t cand = cand0;
       if (!single_chunk) {
-        tmem_ld32(trow + v0, sc);
+        load_scores(v0);
         cand = 0;
 #pragma unroll
-        for (int i = 0; i < 32; ++i)
-          if (v0 + i < nwin && fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]) <= thr) cand |= 1u << i;
+        for (int j = 0; j < 32; ++j)
+          if (sv[j] <= thr) cand |= 1u << j;
       }
       if (!refine) cand = 0;
       while (cand) {
@@ -289,14 +316,13 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
       }
     }
     for (int v0 = 0; v0 < nwin; v0 += 32) {
-      tmem_ld32(trow + v0, sc);
+      load_scores(v0);
       if (valid) {
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          if (v0 + i < nwin) {
-            const float s = fmaf(-2.f, __uint_as_float(sc[i]), s_c[v0 + i]);
-            const float dd = direct_dist_probe(sA, half_a, li, mu_b + (size_t)s_u[v0 + i] * kD);
-            worst = fmaxf(worst, fabsf((dd - xx) - s) / fmaxf(sqrtf(xx * c_max), 1e-30f));
+        for (int j = 0; j < 32; ++j) {
+          if (v0 + j < nwin) {
+            const float dd = direct_dist_probe(sA, half_a, li, mu_b + (size_t)s_u[v0 + j] * kD);
+            worst = fmaxf(worst, fabsf((dd - xx) - sv[j]) / fmaxf(sqrtf(xx * c_max), 1e-30f));
           }
         }
       }
@@ -311,7 +337,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   {
     const unsigned m = __match_any_sync(0xffffffffu, lab);
     if (lab >= 0) {
-      *reinterpret_cast<__nv_bfloat16*>(sP + (li >> 6) * half_p + lab * 128 + (((((li & 63) >> 3) ^ (lab & 7))) << 4) + (li & 7) * 2) =
+      *reinterpret_cast<__nv_bfloat16*>(sP + (li >> 6) * half_b + lab * 128 + (((((li & 63) >> 3) ^ (lab & 7))) << 4) + (li & 7) * 2) =
           __float2bfloat16_rn(1.0f);
       if ((m & ((1u << lane) - 1u)) == 0) atomicAdd(&s_cnt[lab], __popc(m));
     }
@@ -320,35 +346,30 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   __syncthreads();
   tc_fence_after();
 
-  // ---- MMA 2: z[slot, :] = sum_token P^T[slot, token] x[token, :]   (Alg. 2 line 20), 128 slots per M tile
-  const int mtiles = (nwin + 127) >> 7;
+  // ---- MMA 2: z^T[dim, slot] = sum_token x[token, dim] P^T[slot, token]   (Alg. 2 line 20): A = the token tile read
+  // MN-major (M = 128 feature dims), B = the one-hot tile, D overwrites the score columns; TMEM lane = feature dim
   if (tid == 0) {
-    const uint32_t idesc = umma_idesc_bf16(128, 128, 1);
+    const uint32_t idesc = umma_idesc_bf16(128, (uint32_t)npad, 1, 0);
     const uint32_t p_addr = smem_u32(sP), x_addr = smem_u32(sA);
     const int ksteps = p.rows_a >> 4;
-    for (int mt = 0; mt < mtiles; ++mt)
-      for (int ks = 0; ks < ksteps; ++ks)
-        mma_ss(tmem + mt * 128, umma_desc(p_addr + mt * 128 * 128 + (ks >> 2) * half_p + (ks & 3) * 32, 16, 1024),
-               umma_desc(x_addr + ks * 2048, half_a, 1024), idesc, ks > 0);
+    for (int ks = 0; ks < ksteps; ++ks)
+      mma_ss(tmem, umma_desc(x_addr + ks * 2048, half_a, 1024), umma_desc(p_addr + (ks >> 2) * half_b + (ks & 3) * 32, 16, 1024),
+             idesc, ks > 0);
     tc_commit(&B->sum_done);
   }
   __syncwarp();
   const size_t pbase = ((size_t)bh * g.Nc + cell) * nwin;
-  for (int mt = 0; mt < mtiles; ++mt) {
-    if (mt * 128 + warp * 32 >= nwin) break;          // warp-uniform: TMEM lane = slot
-    const int v = mt * 128 + tid;
-    const int cnt = v < nwin ? s_cnt[v] : 0;
-    if (v < nwin) p.part_cnt[pbase + v] = cnt;
-    if (mt == 0) { mbar_wait(&B->sum_done, 0); tc_fence_after(); }
-#pragma unroll 1
-    for (int c = 0; c < 4; ++c) {
-      tmem_ld32(trow + mt * 128 + c * 32, sc);
-      if (cnt > 0) {
-        uint4* dst = reinterpret_cast<uint4*>(p.part + (pbase + v) * kD + c * 32);
+  for (int v = tid; v < nwin; v += kThreads) p.part_cnt[pbase + v] = s_cnt[v];
+  mbar_wait(&B->sum_done, 0);
+  tc_fence_after();
+  // thread = feature dim: a warp stores 32 consecutive floats of a partial row (coalesced)
+  float* prow = p.part + pbase * kD + tid;
+  for (int v0 = 0; v0 < nwin; v0 += 32) {
+    uint32_t raw[32];
+    tmem_ld32(trow + v0, raw);
 #pragma unroll
-        for (int q = 0; q < 8; ++q) dst[q] = make_uint4(sc[4 * q], sc[4 * q + 1], sc[4 * q + 2], sc[4 * q + 3]);
-      }
-    }
+    for (int j = 0; j < 32; ++j)
+      if (v0 + j < nwin && s_cnt[v0 + j] > 0) prow[(size_t)(v0 + j) * kD] = __uint_as_float(raw[j]);
   }
   tc_fence_before();
   __syncthreads();
@@ -383,18 +404,15 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
   const int ctok = g.kt * g.kh * g.kw;
   a->npad = (g.nwin + 15) & ~15;
   a->rows_a = (ctok + 15) & ~15;
-  a->pm = (g.nwin + 7) & ~7;
-  const int mtiles = (g.nwin + 127) / 128;
-  a->tmem_cols = 128;
-  while ((int)a->tmem_cols < mtiles * 128 || (int)a->tmem_cols < ((g.nwin + 31) & ~31)) a->tmem_cols <<= 1;
-  const size_t half_a = (size_t)a->rows_a * 128, half_b = (size_t)a->npad * 128, half_p = (size_t)a->pm * 128;
+  a->tmem_cols = 32;
+  while ((int)a->tmem_cols < a->npad) a->tmem_cols <<= 1;
+  const size_t half_a = (size_t)a->rows_a * 128, half_b = (size_t)a->npad * 128;
   size_t bytes = 4 * half_b + 2 * half_a + 3 * sizeof(int) * (size_t)a->npad + sizeof(AssignTcBars) + 16;
-  // the MMAs read 128 rows of their M operand (tokens in MMA 1, slots in MMA 2): keep the over-read inside the allocation
+  // MMA 1 reads 128 token rows of its A operand: keep the over-read inside the allocation
   bytes = std::max(bytes, 4 * half_b + half_a + 16384);
-  bytes = std::max(bytes, (size_t)(mtiles - 1) * 16384 + half_p + 16384);
   bytes += 1024;
   a->smem = bytes;
-  if (bytes > 227 * 1024) return HVA_EUNSUPPORTED;
+  if (bytes > 227 * 1024 || (long long)g.Kt * BH > 65535 || g.Kh > 65535) return HVA_EUNSUPPORTED;
   if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, g.kt, g.kh, g.kw)) return HVA_ECUDA;
   if (!make_map5(&a->map_hi, mu_hi, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
   if (!make_map5(&a->map_lo, mu_lo, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
@@ -405,8 +423,10 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
 
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
                          int* part_cnt, int* assign, float* lowe, float* probe, cudaStream_t st) {
-  AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, a.pm, a.tmem_cols, probe};
-  hva_assign_tc_kernel<<<dim3(g.Nc, BH), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  auto magic = [](int d) -> uint32_t { return d <= 1 ? 0u : (uint32_t)(((1ull << 32) + d - 1) / d); };
+  AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, magic(g.kh * g.kw), magic(g.kw), magic(g.wh * g.ww),
+                   magic(g.ww), a.tmem_cols, probe};
+  hva_assign_tc_kernel<<<dim3(g.Kw, g.Kh, g.Kt * BH), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }

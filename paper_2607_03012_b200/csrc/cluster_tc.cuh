@@ -5,7 +5,7 @@
 
 struct HvaAssignTc {
   CUtensorMap map_x, map_hi, map_lo;
-  int npad, rows_a, pm;
+  int npad, rows_a;
   uint32_t tmem_cols;
   size_t smem;
 };
