@@ -261,7 +261,7 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
         "roofline": {"bound": "tensor", "kernel": "hva_attn_tc_kernel", "achieved": ach, "peak": pk["tf_sust"], "unit": "TFLOP/s",
                      "frac": ach / pk["tf_sust"], "frac_of_burst": ach / pk["tf_burst"], "peak_source": pk["src"] + " (sustained)",
                      "traffic": None, "executed_tflop": exec_flop / 1e12, "dense_equiv_tflops": dense_flop / t_att / 1e12},
-        "roofline_cluster": {"bound": "hbm", "kernel": "hva_assign_kernel+hva_finalize_kernel", "achieved": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9,
+        "roofline_cluster": {"bound": "hbm", "kernel": "hva_assign_tc_kernel+hva_finalize_kernel", "achieved": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9,
                              "peak": pk["hbm"], "unit": "GB/s", "frac": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9 / pk["hbm"],
                              "algorithmic_bytes": cl_bytes},
         "roofline_permute": {"bound": "hbm", "kernel": "hva_permute_kernel", "achieved": pm_bytes / (st["permute_qkv"] * 1e-3) / 1e9,
