@@ -50,6 +50,21 @@ __device__ __forceinline__ uint32_t umma_idesc(uint32_t b_mn_major) {
   return (1u << 4) | (1u << 7) | (1u << 10) | (b_mn_major << 16) | ((uint32_t)(kBN >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
 }
 
+// 2^x on the FMA pipe for a pair (FlashAttention-4 style software exponential): x = n + f, n = round(x), |f| <= 1/2,
+// 2^f by a degree-3 minimax polynomial (max relative error 7.5e-5, far below the bf16 rounding of P), exponent field += n.
+__device__ __forceinline__ float2 exp2_poly2(float2 x) {
+  x.x = fmaxf(x.x, -125.f); x.y = fmaxf(x.y, -125.f);
+  const float2 magic = make_float2(12582912.f, 12582912.f);     // 1.5 * 2^23: the sum's low mantissa bits hold round(x)
+  const float2 t = __fadd2_rn(x, magic);
+  const float2 r = __fadd2_rn(t, make_float2(-12582912.f, -12582912.f));
+  const float2 f = __fadd2_rn(x, make_float2(-r.x, -r.y));
+  float2 q = __ffma2_rn(make_float2(0.0551716685f, 0.0551716685f), f, make_float2(0.2426111251f, 0.2426111251f));
+  q = __ffma2_rn(q, f, make_float2(0.6932609677f, 0.6932609677f));
+  q = __ffma2_rn(q, f, make_float2(0.9999280572f, 0.9999280572f));
+  return make_float2(__uint_as_float(__float_as_uint(q.x) + (__float_as_uint(t.x) << 23)),
+                     __uint_as_float(__float_as_uint(q.y) + (__float_as_uint(t.y) << 23)));
+}
+
 struct __align__(8) TcBarriers {
   uint64_t q_full, k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages], s_full, p_ready, o_done;
   uint32_t tmem_base;
@@ -201,56 +216,73 @@ __global__ void __launch_bounds__(kThreadsTC, 2) hva_attn_tc_kernel(const __grid
     // ===================================================== softmax / correction / epilogue (thread = row)
     const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
     const float sl2 = p.scale_log2;
-    float m_ref = -INFINITY, l = 0.f;
+    const float2 sl2x2 = make_float2(sl2, sl2);
+    float m_ref = -INFINITY;          // reference exponent (log2 units) of the row: P = 2^(s*scale*log2e - m_ref)
+    float2 l2 = make_float2(0.f, 0.f);
     uint32_t v[32];
     for (int j = 0; j < jn; ++j) {
       const uint32_t s_addr = tmem + lane_base + kColS;
       const int rows_valid = min(kBN, kappa - j * kBN);
       mbar_wait(&B->s_full, j & 1);
       tc_fence_after();
-      float mx = -INFINITY;
+      // One pass over S, 32 columns at a time: chunk max -> (rarely) move the reference -> exponentials -> P over S.
+      // The reference only moves when a score exceeds it by > 2^8 (lazy rescale); then l, the P chunks of this tile already
+      // written and O (complete: the commit of S_j covers PV_{j-1}) are rescaled.
 #pragma unroll 1
       for (int c = 0; c < 4; ++c) {
         tmem_ld32(s_addr + c * 32, v);
-        if (rows_valid == kBN) {
+        if (rows_valid != kBN) {
 #pragma unroll
-          for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(v[i]));
-        } else {
-#pragma unroll
-          for (int i = 0; i < 32; ++i) mx = fmaxf(mx, (c * 32 + i < rows_valid) ? __uint_as_float(v[i]) : -INFINITY);
+          for (int i = 0; i < 32; ++i)
+            if (c * 32 + i >= rows_valid) v[i] = 0xff800000u;   // -inf: key columns past the packed list
         }
-      }
-      const float m_new = fmaxf(m_ref, mx * sl2);
-      if (__any_sync(0xffffffffu, m_new - m_ref > kRescaleThreshold)) {   // lazy rescale, warp-uniform
-        if (j > 0) {
-          mbar_wait(&B->o_done, (j - 1) & 1);
-          tc_fence_after();
-          const float f = ex2(m_ref - m_new);
-          l *= f;
-#pragma unroll 1
-          for (int c = 0; c < 4; ++c) {
-            tmem_ld32(tmem + lane_base + kColO + c * 32, v);
+        float mx0 = fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1])), mx1 = fmaxf(__uint_as_float(v[2]), __uint_as_float(v[3]));
 #pragma unroll
-            for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) * f);
-            tmem_st32(tmem + lane_base + kColO + c * 32, v);
+        for (int i = 4; i < 32; i += 4) {
+          mx0 = fmaxf(mx0, fmaxf(__uint_as_float(v[i]), __uint_as_float(v[i + 1])));
+          mx1 = fmaxf(mx1, fmaxf(__uint_as_float(v[i + 2]), __uint_as_float(v[i + 3])));
+        }
+        const float m_c = fmaxf(mx0, mx1) * sl2;
+        if (__any_sync(0xffffffffu, m_c - m_ref > kRescaleThreshold)) {   // warp-uniform
+          const float m_new = fmaxf(m_ref, m_c);
+          const float f = (m_new == m_ref) ? 1.f : ex2(m_ref - m_new);
+          l2.x *= f; l2.y *= f;
+          tmem_st_wait();
+          for (int cc = 0; cc < c; ++cc) {          // P chunks of this tile written against the old reference
+            uint32_t pk[16];
+            tmem_ld16(s_addr + cc * 16, pk);
+#pragma unroll
+            for (int i = 0; i < 16; ++i)
+              pk[i] = pack_bf16(__uint_as_float(pk[i] << 16) * f, __uint_as_float(pk[i] & 0xffff0000u) * f);
+            tmem_st16(s_addr + cc * 16, pk);
           }
-        }
-        m_ref = m_new;
-      }
+          if (j > 0) {
+            mbar_wait(&B->o_done, (j - 1) & 1);
+            tc_fence_after();
+            uint32_t o[32];
 #pragma unroll 1
-      for (int c = 0; c < 4; ++c) {
-        tmem_ld32(s_addr + c * 32, v);
+            for (int cc = 0; cc < 4; ++cc) {
+              tmem_ld32(tmem + lane_base + kColO + cc * 32, o);
+#pragma unroll
+              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+              tmem_st32(tmem + lane_base + kColO + cc * 32, o);
+            }
+          }
+          m_ref = m_new;
+        }
+        const float2 nm = make_float2(-m_ref, -m_ref);
         uint32_t pk[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-          float p0 = ex2(fmaf(__uint_as_float(v[2 * i]), sl2, -m_ref));
-          float p1 = ex2(fmaf(__uint_as_float(v[2 * i + 1]), sl2, -m_ref));
-          if (rows_valid != kBN) {
-            p0 = (c * 32 + 2 * i < rows_valid) ? p0 : 0.f;
-            p1 = (c * 32 + 2 * i + 1 < rows_valid) ? p1 : 0.f;
+          const float2 x = __ffma2_rn(make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), sl2x2, nm);
+          float2 e;
+          if ((i & 3) == 3) {
+            e = exp2_poly2(x);            // 1 pair in 4 on the FMA pipe: the MUFU rate (16/clk/SM) equals the MMA time of a tile
+          } else {
+            e.x = ex2(x.x); e.y = ex2(x.y);
           }
-          l += p0 + p1;
-          pk[i] = pack_bf16(p0, p1);
+          l2 = __fadd2_rn(l2, e);
+          pk[i] = pack_bf16(e.x, e.y);
         }
         tmem_st16(s_addr + c * 16, pk);
       }
@@ -258,6 +290,7 @@ __global__ void __launch_bounds__(kThreadsTC, 2) hva_attn_tc_kernel(const __grid
       tc_fence_before();
       mbar_arrive(&B->p_ready);
     }
+    const float l = l2.x + l2.y;
     // epilogue: O / l, bf16, row store with the inverse permutation fused (Eq. 4: O = Pi^{q-1} O')
     mbar_wait(&B->o_done, (jn - 1) & 1);
     tc_fence_after();
