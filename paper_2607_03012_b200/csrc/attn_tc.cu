@@ -24,11 +24,11 @@ using namespace hva_ptx;
 constexpr int kBM = 128, kBN = 128, kD = 128;
 constexpr int kHalfBytes = 128 * 128;          // one 64-dim half of a 128-row tile: 128 rows x 128 B
 constexpr int kTileBytes = 2 * kHalfBytes;     // 32 KB
-constexpr int kStages = 1;                     // one K and one V buffer per CTA: two CTAs share an SM
-constexpr int kThreadsTC = 192;
+constexpr int kStages = 3;                     // K ring and V ring of three 128-row tiles each
+constexpr int kThreadsTC = 416;                // warps 0-7 softmax (two threads per query row), 9: MMA, 8/10/11/12: TMA
 constexpr int kNumBoxes = 8;                   // box heights 1,2,4,...,128
-constexpr uint32_t kTmemCols = 256;            // S (P aliased over it) + O; two CTAs fit the SM's 512 columns
-constexpr uint32_t kColS = 0, kColO = 128;
+constexpr uint32_t kTmemCols = 512;            // S_0, S_1 (fp32 scores), O (fp32), P_0, P_1 (bf16 probabilities)
+constexpr uint32_t kColS = 0, kColO = 256, kColP = 384;   // S_b at kColS + 128 b, P_b at kColP + 64 b
 constexpr float kRescaleThreshold = 8.0f;      // log2 units
 
 struct TcMaps {
@@ -43,6 +43,7 @@ struct TcParams {
   const int *goff, *koff, *kappa, *run_cnt, *work_cnt, *work, *perm_q;
   const uint32_t* runs;
   __nv_bfloat16* O;
+  unsigned long long* probe;   // HVA_ATTN_TIMING builds only: per-phase cycle totals
 };
 
 // instruction descriptor: D = F32, A = B = BF16, M = 128, N = 128; b_major selects MN-major B
@@ -65,9 +66,16 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
                      __uint_as_float(__float_as_uint(q.y) + (__float_as_uint(t.y) << 23)));
 }
 
+#ifdef HVA_ATTN_TIMING
+#define AMARK(k) do { long long _t = clock64(); tacc[k] += (unsigned long long)(_t - tprev); tprev = _t; } while (0)
+#else
+#define AMARK(k) do { } while (0)
+#endif
+
 struct __align__(8) TcBarriers {
-  uint64_t q_full, k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages], s_full, p_ready, o_done;
+  uint64_t q_full, k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages], s_full[2], s_free[2], p_ready[2], p_free[2];
   uint32_t tmem_base;
+  float xch[2][kBM];          // half-row maxima / sums exchanged between the two threads of a query row
 };
 
 constexpr size_t kSmemTC = 1024 + kTileBytes * (1 + 2 * kStages) + sizeof(TcBarriers);
@@ -83,32 +91,32 @@ struct RunWalker {
   }
 };
 
-__device__ __forceinline__ void emit_boxes(const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int grow, int dst, int len) {
+__device__ __forceinline__ void emit_boxes(const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col, int grow, int dst, int len) {
 #pragma unroll 1
   for (int b = kNumBoxes - 1; b >= 0; --b) {
     const int h = 1 << b;
     if (len & h) {
-      tma_load_2d(maps + b, bar, stage + dst * 128, 0, grow);
-      tma_load_2d(maps + b, bar, stage + kHalfBytes + dst * 128, 64, grow);
+      if (elect_one()) tma_load_2d(maps + b, bar, stage + dst * 128, col, grow);
       grow += h; dst += h;
     }
   }
 }
 
-__device__ __forceinline__ void load_tile(RunWalker& w, const CUtensorMap* maps, uint64_t* bar, unsigned char* stage,
+// one 64-dim half (column `col`) of a packed key tile
+__device__ __forceinline__ void load_tile(RunWalker& w, const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col,
                                           int base_row, int rows_valid, int rows_load) {
   int dst = 0;
   while (dst < rows_valid) {
     while (w.used == w.len) { ++w.r; w.load(); }
     int seg = min(w.len - w.used, rows_valid - dst);
-    emit_boxes(maps, bar, stage, base_row + w.row0 + w.used, dst, seg);
+    emit_boxes(maps, bar, stage, col, base_row + w.row0 + w.used, dst, seg);
     w.used += seg; dst += seg;
   }
   if (rows_load > rows_valid)   // ragged last tile: round up to the MMA K granule with finite over-read rows
-    emit_boxes(maps, bar, stage, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
+    emit_boxes(maps, bar, stage, col, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
 }
 
-__global__ void __launch_bounds__(kThreadsTC, 2) hva_attn_tc_kernel(const __grid_constant__ TcMaps maps, TcParams p) {
+__global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid_constant__ TcMaps maps, TcParams p) {
   const int bh = blockIdx.y;
   if ((int)blockIdx.x >= p.work_cnt[bh]) return;
   const uint32_t wi = (uint32_t)p.work[(size_t)bh * p.work_cap + blockIdx.x];
@@ -139,15 +147,17 @@ __global__ void __launch_bounds__(kThreadsTC, 2) hva_attn_tc_kernel(const __grid
   if (tid == 0) {
     mbar_init(&B->q_full, 1);
     for (int s = 0; s < kStages; ++s) {
-      mbar_init(&B->k_full[s], 1); mbar_init(&B->k_empty[s], 1);
-      mbar_init(&B->v_full[s], 1); mbar_init(&B->v_empty[s], 1);
+      mbar_init(&B->k_full[s], 2); mbar_init(&B->k_empty[s], 1);     // two producers (one per 64-dim half) per ring
+      mbar_init(&B->v_full[s], 2); mbar_init(&B->v_empty[s], 1);
     }
-    mbar_init(&B->s_full, 1); mbar_init(&B->p_ready, 128);
-    mbar_init(&B->o_done, 1);
+    mbar_init(&B->s_full[0], 1); mbar_init(&B->s_full[1], 1);
+    mbar_init(&B->p_ready[0], 256); mbar_init(&B->p_ready[1], 256);
+    mbar_init(&B->s_free[0], 256); mbar_init(&B->s_free[1], 256);
+    mbar_init(&B->p_free[0], 1); mbar_init(&B->p_free[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  if (warp == 5) {
+  if (warp == 9) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&B->tmem_base)), "r"(kTmemCols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -156,125 +166,178 @@ __global__ void __launch_bounds__(kThreadsTC, 2) hva_attn_tc_kernel(const __grid
   tc_fence_after();
   const uint32_t tmem = B->tmem_base;
 
-  if (warp == 4) {
-    // ===================================================== TMA producer
-    if (lane == 0) {
+  if (warp == 8 || warp >= 10) {
+    // ===================================================== TMA producers (warp-uniform, one elected lane issues):
+    // warp 8: K ring dims 0-63 (+ Q), warp 10: V ring dims 0-63, warp 11: K ring dims 64-127, warp 12: V ring dims 64-127
+    const bool is_k = (warp == 8 || warp == 11);
+    const int half = warp >= 11;
+    if (warp == 8 && elect_one()) {
       mbar_expect_tx(&B->q_full, kTileBytes);
       tma_load_2d(&maps.q, &B->q_full, sQ, 0, base_row + row0);
       tma_load_2d(&maps.q, &B->q_full, sQ + kHalfBytes, 64, base_row + row0);
-      RunWalker wk{p.runs + ((size_t)bh * p.Nq + g) * p.run_stride, p.koff + (size_t)bh * (p.Nk + 1),
-                   p.run_cnt[(size_t)bh * p.Nq + g], 0, 0, 0, 0};
-      wk.load();
-      RunWalker wv = wk;
-      for (int j = 0; j < jn; ++j) {
-        const int s = j % kStages, use = j / kStages;
-        const int rows_valid = min(kBN, kappa - j * kBN);
-        const int rows_load = rows_valid == kBN ? kBN : (rows_valid + 15) & ~15;
-        if (use > 0) mbar_wait(&B->k_empty[s], (use - 1) & 1);
-        mbar_expect_tx(&B->k_full[s], rows_load * 256);
-        load_tile(wk, maps.k, &B->k_full[s], sK + s * kTileBytes, base_row, rows_valid, rows_load);
-        if (use > 0) mbar_wait(&B->v_empty[s], (use - 1) & 1);
-        mbar_expect_tx(&B->v_full[s], rows_load * 256);
-        load_tile(wv, maps.v, &B->v_full[s], sV + s * kTileBytes, base_row, rows_valid, rows_load);
-      }
     }
-  } else if (warp == 5) {
-    // ===================================================== MMA issuer (one thread)
-    if (lane == 0) {
-      const uint32_t idesc_qk = umma_idesc(0), idesc_pv = umma_idesc(1);
-      const uint32_t q_addr = smem_u32(sQ), k_addr = smem_u32(sK), v_addr = smem_u32(sV);
-      auto issue_qk = [&](int j) {
-        const int s = j % kStages;
-        mbar_wait(&B->k_full[s], (j / kStages) & 1);
-        tc_fence_after();
+    RunWalker w{p.runs + ((size_t)bh * p.Nq + g) * p.run_stride, p.koff + (size_t)bh * (p.Nk + 1),
+                p.run_cnt[(size_t)bh * p.Nq + g], 0, 0, 0, 0};
+    w.load();
+    const CUtensorMap* mp = is_k ? maps.k : maps.v;
+    uint64_t* full = is_k ? B->k_full : B->v_full;
+    uint64_t* empty = is_k ? B->k_empty : B->v_empty;
+    unsigned char* ring = (is_k ? sK : sV) + half * kHalfBytes;
+    for (int j = 0; j < jn; ++j) {
+      const int s = j % kStages, use = j / kStages;
+      const int rows_valid = min(kBN, kappa - j * kBN);
+      const int rows_load = rows_valid == kBN ? kBN : (rows_valid + 15) & ~15;
+      if (use > 0) mbar_wait(&empty[s], (use - 1) & 1);
+      if (elect_one()) mbar_expect_tx(&full[s], rows_load * 128);
+      __syncwarp();
+      load_tile(w, mp, &full[s], ring + s * kTileBytes, half * 64, base_row, rows_valid, rows_load);
+    }
+  } else if (warp == 9) {
+    // ===================================================== MMA issuer: the whole warp runs the loop (uniform), one elected lane issues
+    // S and P are double buffered and separate: QK_{j+2} is issued as soon as the softmax threads have pulled S_j into
+    // registers (s_free), PV_j when P_j is complete (p_ready); the softmax of tile j+2 reuses P_b once PV_j is done (p_free).
+    const uint32_t idesc_qk = umma_idesc(0), idesc_pv = umma_idesc(1);
+    // descriptors are built once; a k-step / stage only adds a constant to the 14-bit start-address field (no carry out:
+    // the tiles end below 256 KB), so each MMA costs one add per operand instead of a shift / mask / or chain
+    const uint64_t dq = umma_desc(smem_u32(sQ), 16, 1024), dk = umma_desc(smem_u32(sK), 16, 1024),
+                   dv = umma_desc(smem_u32(sV), kHalfBytes, 1024);
+#ifdef HVA_ATTN_TIMING
+    unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long tprev = clock64();
+#endif
+    auto issue_qk = [&](int j) {
+      const int s = j % kStages, b = j & 1;
+      AMARK(0);
+      mbar_wait(&B->k_full[s], (j / kStages) & 1);
+      AMARK(1);
+      tc_fence_after();
+      const uint64_t dks = dk + (uint64_t)(s * (kTileBytes >> 4));
+      const uint32_t d_s = tmem + kColS + b * 128;
+      if (elect_one()) {
 #pragma unroll
         for (int ks = 0; ks < kD / 16; ++ks) {
-          const uint32_t off = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
-          mma_ss(tmem + kColS, umma_desc(q_addr + off, 16, 1024), umma_desc(k_addr + s * kTileBytes + off, 16, 1024), idesc_qk, ks > 0);
+          const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
+          mma_ss(d_s, dq + off, dks + off, idesc_qk, ks > 0);
         }
-        tc_commit(&B->s_full);
+        tc_commit(&B->s_full[b]);
         tc_commit(&B->k_empty[s]);
-      };
-      mbar_wait(&B->q_full, 0);
-      issue_qk(0);
-      for (int j = 0; j < jn; ++j) {
-        const int s = j % kStages;
-        mbar_wait(&B->p_ready, j & 1);
-        mbar_wait(&B->v_full[s], (j / kStages) & 1);
-        tc_fence_after();
-        const int rows_valid = min(kBN, kappa - j * kBN);
-        const int ksteps = (rows_valid + 15) >> 4;
-        for (int ks = 0; ks < ksteps; ++ks)
-          mma_ts(tmem + kColO, tmem + kColS + ks * 8, umma_desc(v_addr + s * kTileBytes + ks * 2048, kHalfBytes, 1024), idesc_pv,
-                 (j > 0 || ks > 0));
-        tc_commit(&B->v_empty[s]);
-        tc_commit(&B->o_done);
-        if (j + 1 < jn) issue_qk(j + 1);   // S is aliased by P_j: issue order after PV(j) keeps the tensor pipe in order
       }
+      __syncwarp();
+    };
+    mbar_wait(&B->q_full, 0);
+    issue_qk(0);
+    if (jn > 1) issue_qk(1);
+    for (int j = 0; j < jn; ++j) {
+      const int s = j % kStages, b = j & 1;
+      if (j + 2 < jn) {
+        AMARK(0);
+        mbar_wait(&B->s_free[b], (j >> 1) & 1);
+        AMARK(2);
+        issue_qk(j + 2);
+      }
+      AMARK(0);
+      mbar_wait(&B->p_ready[b], (j >> 1) & 1);
+      AMARK(3);
+      mbar_wait(&B->v_full[s], (j / kStages) & 1);
+      AMARK(4);
+      tc_fence_after();
+      const int rows_valid = min(kBN, kappa - j * kBN);
+      const int ksteps = (rows_valid + 15) >> 4;
+      const uint64_t dvs = dv + (uint64_t)(s * (kTileBytes >> 4));
+      const uint32_t a_p = tmem + kColP + b * 64;
+      if (elect_one()) {
+        if (ksteps == 8) {
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks) mma_ts(tmem + kColO, a_p + ks * 8, dvs + ks * (2048 >> 4), idesc_pv, (j > 0 || ks > 0));
+        } else {
+          for (int ks = 0; ks < ksteps; ++ks) mma_ts(tmem + kColO, a_p + ks * 8, dvs + ks * (2048 >> 4), idesc_pv, (j > 0 || ks > 0));
+        }
+        tc_commit(&B->v_empty[s]);
+        tc_commit(&B->p_free[b]);
+      }
+      __syncwarp();
     }
-  } else {
-    // ===================================================== softmax / correction / epilogue (thread = row)
-    const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+#ifdef HVA_ATTN_TIMING
+    AMARK(0);
+    if (p.probe && lane == 0) for (int k = 0; k < 8; ++k) atomicAdd(p.probe + k, tacc[k]);
+#endif
+  } else if (warp < 8) {
+    // ===================================================== softmax / correction / epilogue
+    // thread = (query row, half): row = TMEM lane 32 (warp & 3) + lane, half h = warp >> 2 owns key columns [64h, 64h + 64)
+    const int h = warp >> 2, r = (warp & 3) * 32 + lane;
+    const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
     const float sl2 = p.scale_log2;
     const float2 sl2x2 = make_float2(sl2, sl2);
     float m_ref = -INFINITY;          // reference exponent (log2 units) of the row: P = 2^(s*scale*log2e - m_ref)
     float2 l2 = make_float2(0.f, 0.f);
-    uint32_t v[32];
+    uint32_t va[32], vb[32];
+#ifdef HVA_ATTN_TIMING
+    unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long tprev = clock64();
+#endif
     for (int j = 0; j < jn; ++j) {
-      const uint32_t s_addr = tmem + lane_base + kColS;
+      const int b = j & 1;
+      const uint32_t s_addr = tmem + lane_base + kColS + b * 128;
       const int rows_valid = min(kBN, kappa - j * kBN);
-      mbar_wait(&B->s_full, j & 1);
+      AMARK(0);
+      mbar_wait(&B->s_full[b], (j >> 1) & 1);
+      AMARK(1);
       tc_fence_after();
-      // One pass over S, 32 columns at a time: chunk max -> (rarely) move the reference -> exponentials -> P over S.
-      // The reference only moves when a score exceeds it by > 2^8 (lazy rescale); then l, the P chunks of this tile already
-      // written and O (complete: the commit of S_j covers PV_{j-1}) are rescaled.
+      // half-row maximum; the 64 scores stay in registers (P_j is written over S_j only after both halves have read it)
+      tmem_ld32(s_addr + h * 64, va);
+      tmem_ld32(s_addr + h * 64 + 32, vb);
+      tc_fence_before();
+      mbar_arrive(&B->s_free[b]);          // the scores are in registers: the MMA warp may overwrite S_b with QK_{j+2}
+      if (rows_valid != kBN) {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+          if (h * 64 + i >= rows_valid) va[i] = 0xff800000u;   // -inf: key columns past the packed list
+          if (h * 64 + 32 + i >= rows_valid) vb[i] = 0xff800000u;
+        }
+      }
+      float mx0 = fmaxf(__uint_as_float(va[0]), __uint_as_float(va[1])), mx1 = fmaxf(__uint_as_float(vb[0]), __uint_as_float(vb[1]));
+#pragma unroll
+      for (int i = 2; i < 32; i += 2) {
+        mx0 = fmaxf(mx0, fmaxf(__uint_as_float(va[i]), __uint_as_float(va[i + 1])));
+        mx1 = fmaxf(mx1, fmaxf(__uint_as_float(vb[i]), __uint_as_float(vb[i + 1])));
+      }
+      const float m_half = fmaxf(mx0, mx1);
+      B->xch[h][r] = m_half;
+      tc_fence_before();
+      AMARK(2);
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      AMARK(3);
+      tc_fence_after();
+      const float m_c = fmaxf(m_half, B->xch[h ^ 1][r]) * sl2;
+      // the reference only moves when a score exceeds it by > 2^8 (lazy rescale); both threads of a row take the same decision
+      if (__any_sync(0xffffffffu, m_c - m_ref > kRescaleThreshold)) {
+        const float m_new = fmaxf(m_ref, m_c);
+        const float f = (m_new == m_ref) ? 1.f : ex2(m_ref - m_new);
+        l2.x *= f; l2.y *= f;
+        if (j > 0) {                                   // O columns [64h, 64h + 64) of the row
+          mbar_wait(&B->p_free[(j - 1) & 1], ((j - 1) >> 1) & 1);   // PV_{j-1} complete
+          tc_fence_after();
+          uint32_t o[16];
 #pragma unroll 1
-      for (int c = 0; c < 4; ++c) {
-        tmem_ld32(s_addr + c * 32, v);
-        if (rows_valid != kBN) {
+          for (int cc = 0; cc < 4; ++cc) {
+            tmem_ld16(tmem + lane_base + kColO + h * 64 + cc * 16, o);
 #pragma unroll
-          for (int i = 0; i < 32; ++i)
-            if (c * 32 + i >= rows_valid) v[i] = 0xff800000u;   // -inf: key columns past the packed list
-        }
-        float mx0 = fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1])), mx1 = fmaxf(__uint_as_float(v[2]), __uint_as_float(v[3]));
-#pragma unroll
-        for (int i = 4; i < 32; i += 4) {
-          mx0 = fmaxf(mx0, fmaxf(__uint_as_float(v[i]), __uint_as_float(v[i + 1])));
-          mx1 = fmaxf(mx1, fmaxf(__uint_as_float(v[i + 2]), __uint_as_float(v[i + 3])));
-        }
-        const float m_c = fmaxf(mx0, mx1) * sl2;
-        if (__any_sync(0xffffffffu, m_c - m_ref > kRescaleThreshold)) {   // warp-uniform
-          const float m_new = fmaxf(m_ref, m_c);
-          const float f = (m_new == m_ref) ? 1.f : ex2(m_ref - m_new);
-          l2.x *= f; l2.y *= f;
-          tmem_st_wait();
-          for (int cc = 0; cc < c; ++cc) {          // P chunks of this tile written against the old reference
-            uint32_t pk[16];
-            tmem_ld16(s_addr + cc * 16, pk);
-#pragma unroll
-            for (int i = 0; i < 16; ++i)
-              pk[i] = pack_bf16(__uint_as_float(pk[i] << 16) * f, __uint_as_float(pk[i] & 0xffff0000u) * f);
-            tmem_st16(s_addr + cc * 16, pk);
+            for (int i = 0; i < 16; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+            tmem_st16(tmem + lane_base + kColO + h * 64 + cc * 16, o);
           }
-          if (j > 0) {
-            mbar_wait(&B->o_done, (j - 1) & 1);
-            tc_fence_after();
-            uint32_t o[32];
-#pragma unroll 1
-            for (int cc = 0; cc < 4; ++cc) {
-              tmem_ld32(tmem + lane_base + kColO + cc * 32, o);
-#pragma unroll
-              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-              tmem_st32(tmem + lane_base + kColO + cc * 32, o);
-            }
-          }
-          m_ref = m_new;
         }
-        const float2 nm = make_float2(-m_ref, -m_ref);
+        m_ref = m_new;
+      }
+      AMARK(4);
+      if (j >= 2) { mbar_wait(&B->p_free[b], ((j - 2) >> 1) & 1); tc_fence_after(); }   // PV_{j-2} has read P_b
+      AMARK(5);
+      const uint32_t p_addr = tmem + lane_base + kColP + b * 64;
+      const float2 nm = make_float2(-m_ref, -m_ref);
+      auto exp_chunk = [&](const uint32_t (&vv)[32], int c) {
         uint32_t pk[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-          const float2 x = __ffma2_rn(make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), sl2x2, nm);
+          const float2 x = __ffma2_rn(make_float2(__uint_as_float(vv[2 * i]), __uint_as_float(vv[2 * i + 1])), sl2x2, nm);
           float2 e;
           if ((i & 3) == 3) {
             e = exp2_poly2(x);            // 1 pair in 4 on the FMA pipe: the MUFU rate (16/clk/SM) equals the MMA time of a tile
@@ -284,41 +347,52 @@ __global__ void __launch_bounds__(kThreadsTC, 2) hva_attn_tc_kernel(const __grid
           l2 = __fadd2_rn(l2, e);
           pk[i] = pack_bf16(e.x, e.y);
         }
-        tmem_st16(s_addr + c * 16, pk);
-      }
+        tmem_st16(p_addr + h * 32 + c * 16, pk);
+      };
+      exp_chunk(va, 0);
+      exp_chunk(vb, 1);
       tmem_st_wait();
       tc_fence_before();
-      mbar_arrive(&B->p_ready);
+      mbar_arrive(&B->p_ready[b]);
+      AMARK(6);
     }
-    const float l = l2.x + l2.y;
-    // epilogue: O / l, bf16, row store with the inverse permutation fused (Eq. 4: O = Pi^{q-1} O')
-    mbar_wait(&B->o_done, (jn - 1) & 1);
+#ifdef HVA_ATTN_TIMING
+    if (p.probe && tid == 0) for (int k = 0; k < 8; ++k) atomicAdd(p.probe + 8 + k, tacc[k]);
+#endif
+    // row sum = both halves
+    const float l_half = l2.x + l2.y;
+    B->xch[h][r] = l_half;
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    const float l = l_half + B->xch[h ^ 1][r];
+    // epilogue: O / l, bf16, row store with the inverse permutation fused (Eq. 4: O = Pi^{q-1} O'); 64 columns per thread
+    mbar_wait(&B->p_free[(jn - 1) & 1], ((jn - 1) >> 1) & 1);   // last PV complete
     tc_fence_after();
     const float inv = 1.f / l;
-    const int row = row0 + tid;
+    const int row = row0 + r;
     const bool ok = row < row1;
     size_t orow = 0;
     if (ok) orow = (size_t)base_row + (p.unpermute ? p.perm_q[(size_t)base_row + row] : row);
 #pragma unroll 1
-    for (int c = 0; c < 4; ++c) {
-      tmem_ld32(tmem + lane_base + kColO + c * 32, v);
+    for (int c = 0; c < 2; ++c) {
+      uint32_t o[32];
+      tmem_ld32(tmem + lane_base + kColO + h * 64 + c * 32, o);
       if (ok) {
-        uint4* dst = reinterpret_cast<uint4*>(p.O + orow * kD + c * 32);
+        uint4* dst = reinterpret_cast<uint4*>(p.O + orow * kD + h * 64 + c * 32);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          uint4 o;
-          o.x = pack_bf16(__uint_as_float(v[8 * q + 0]) * inv, __uint_as_float(v[8 * q + 1]) * inv);
-          o.y = pack_bf16(__uint_as_float(v[8 * q + 2]) * inv, __uint_as_float(v[8 * q + 3]) * inv);
-          o.z = pack_bf16(__uint_as_float(v[8 * q + 4]) * inv, __uint_as_float(v[8 * q + 5]) * inv);
-          o.w = pack_bf16(__uint_as_float(v[8 * q + 6]) * inv, __uint_as_float(v[8 * q + 7]) * inv);
-          dst[q] = o;
+          uint4 w;
+          w.x = pack_bf16(__uint_as_float(o[8 * q + 0]) * inv, __uint_as_float(o[8 * q + 1]) * inv);
+          w.y = pack_bf16(__uint_as_float(o[8 * q + 2]) * inv, __uint_as_float(o[8 * q + 3]) * inv);
+          w.z = pack_bf16(__uint_as_float(o[8 * q + 4]) * inv, __uint_as_float(o[8 * q + 5]) * inv);
+          w.w = pack_bf16(__uint_as_float(o[8 * q + 6]) * inv, __uint_as_float(o[8 * q + 7]) * inv);
+          dst[q] = w;
         }
       }
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 5) {
+  if (warp == 9) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
   }
@@ -360,6 +434,10 @@ int hva_attention_tc_launch(const hva_shape* s, float scale, const void* Qp, con
   p.run_cnt = (const int*)(b + L.run_cnt); p.work_cnt = (const int*)(b + L.work_cnt); p.work = (const int*)(b + L.work);
   p.perm_q = (const int*)(b + L.perm_q); p.runs = (const uint32_t*)(b + L.runs);
   p.O = reinterpret_cast<__nv_bfloat16*>(O);
+  {
+    const char* pe = getenv("HVA_ATTN_PROBE");
+    p.probe = pe ? reinterpret_cast<unsigned long long*>(strtoull(pe, nullptr, 0)) : nullptr;
+  }
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(hva_attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemTC) != cudaSuccess)
