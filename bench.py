@@ -138,6 +138,10 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--top-p", type=float, default=None)
     ap.add_argument("--merge-rounds", type=int, default=None)
+    ap.add_argument("--report", default=None, choices=[None, "sweep", "hybrid"],
+                    help="extra reports of BASELINE.json configs[3] / configs[4] instead of the bench line: 'sweep' = top-p x merging "
+                         "with CTA tile occupancy, 'hybrid' = the 50-step anchor / subset sequence (use --config C5)")
+    ap.add_argument("--seq-steps", type=int, default=50)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stages", action="store_true")
     args = ap.parse_args()
@@ -149,6 +153,10 @@ def main():
     b.lib()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the hva path has no CPU fallback")
+    if args.report == "sweep":
+        return report_sweep(b, wl, args)
+    if args.report == "hybrid":
+        return report_hybrid(b, wl, args)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -204,7 +212,7 @@ def main():
                       "l2": "inputs (2.2 GB) larger than L2", "parallelism": "head-sharded replicas, no collective"},
            "clocks": clocks,
            "e2e": {"value": e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
-           "gpu_launches": args.steps * (2 * (1 + 2 * wl.iters) + 1 + 1 + 7 + 3 + 1)}
+           "gpu_launches": args.steps * (2 * (2 + 2 * wl.iters) + 1 + (3 + 2 * int(cfg.merge_rounds)) + 7 + 3 + 1)}
 
     # ---- per-stage times and rooflines (rank 0)
     if rank == 0 and not args.no_stages:
@@ -219,6 +227,110 @@ def main():
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def occupancy(wl, stats):
+    BH, n = wl.B * wl.heads, wl.n
+    tq, tk = wl.tile
+    tiles = sum(s["tiles_executed"] for s in stats)
+    pairs = sum(s["pairs_valid"] for s in stats)
+    padded = tiles * tq * tk
+    return {"groups": sum(s["n_groups"] for s in stats), "theoretical_density": pairs / (BH * float(n) * n),
+            "cta_density": padded / (BH * float(n) * n), "cta_tile_occupancy": pairs / padded,
+            "q_rows_valid_over_padded": sum(s["q_rows_valid"] for s in stats) / sum(s["q_rows_padded"] for s in stats),
+            "k_cols_valid_over_padded": sum(s["k_cols_valid"] for s in stats) / sum(s["k_cols_padded"] for s in stats),
+            "tiles_executed": tiles}
+
+
+def report_sweep(b, wl, args):
+    """BASELINE.json configs[3]: top-p in {0.8, 0.9, 0.95} x merging {off, on}: ms per call and per attention launch, executed
+    and dense-equivalent TFLOP/s, CTA tile occupancy (valid / padded pairs, rows, columns; Eq. 7 l.111, Fig. 5c l.225)."""
+    Q, K, V = [t.cuda().contiguous() for t in inputs.make_qkv(wl)]
+    shape = b.make_shape(wl)
+    O = torch.empty_like(Q)
+    BH, n, D = wl.B * wl.heads, wl.n, wl.D
+    for top_p in (0.8, 0.9, 0.95):
+        for rounds in (0, wl.merge_rounds):
+            cfg = b.make_config(wl, top_p=top_p, merge_rounds=rounds)
+            fwd = b.Forward(shape, cfg)
+            for _ in range(2):
+                fwd(Q, K, V, O)
+            ms = ev_time(lambda: fwd(Q, K, V, O), max(args.steps, 3))
+            occ = occupancy(wl, fwd.stats_dicts())
+            exec_flop = 4.0 * D * wl.tile[0] * wl.tile[1] * occ["tiles_executed"]
+            print(json.dumps({"report": "sweep", "workload": wl.name, "top_p": top_p, "merge_rounds": rounds, "ms_per_call": round(ms, 3),
+                              "executed_tflop": round(exec_flop / 1e12, 2), "dense_equiv_tflops_call": round(4.0 * BH * n * n * D / (ms * 1e-3) / 1e12, 1),
+                              "occupancy": {k: (round(v, 4) if isinstance(v, float) else v) for k, v in occ.items()}}))
+            del fwd
+
+
+def report_hybrid(b, wl, args):
+    """BASELINE.json configs[4]: X_s = 0.98 X_{s-1} + 0.2 fresh_s for Q, K, V; full clustering at anchor steps (every 10th), subset
+    update (l.101-103) in between.  Per step: ms of the whole call and of its clustering part, label agreement with a cold-start
+    full re-clustering of X_s (ours, and the frozen anchor labels for comparison), relative k-means objective."""
+    import math as _m
+    heads = list(range(wl.heads))
+    shape = b.make_shape(wl)
+    cfg = b.make_config(wl, subset_frac=0.15)
+    fwd = b.Forward(shape, cfg, with_state=True)
+    cur = [inputs.make_head(wl, h, 0) for h in heads]                      # per head [3, n, D]
+    rms0 = [c.float().pow(2).mean(dim=(1, 2)).sqrt() for c in cur]
+    from concurrent.futures import ThreadPoolExecutor
+    O = None
+    frozen = None
+    rows = []
+    for s in range(args.seq_steps):
+        if s > 0:
+            with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 8)) as ex:
+                cur = list(ex.map(lambda h: inputs.hybrid_next(wl, cur[h], h, s, rms0[h]), heads))
+        X = torch.stack(cur, dim=1).unsqueeze(1).cuda()                    # [3, 1, heads, n, D]
+        Q, K, V = X[0].contiguous(), X[1].contiguous(), X[2].contiguous()
+        O = torch.empty_like(Q) if O is None else O
+        kind = b.HVA_ANCHOR if s % 10 == 0 else b.HVA_INTERMEDIATE
+        a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); a.record()
+        fwd(Q, K, V, O, step_kind=kind)
+        e.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(e)
+        st = {k: v.clone() for k, v in fwd.state_views().items()}
+        # clustering part of the step, timed on copies of the cache
+        if kind == b.HVA_ANCHOR:
+            def clus():
+                for X_, t in ((Q, "q"), (K, "k")):
+                    r = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X_, want_lowe=True)
+                    b.hva_select_subset(r["lowe"], st["subset_" + t].shape[1])
+            frozen = {t: st["assign_" + t].clone() for t in "qk"}
+        else:
+            prev = prev_state
+            def clus():
+                for X_, t in ((Q, "q"), (K, "k")):
+                    c2 = {k: prev[k + "_" + t].clone() for k in ("assign", "mu", "sums", "sizes")}
+                    b.hva_cluster_update(shape, X_, prev["subset_" + t], c2["assign"], c2["mu"], c2["sums"], c2["sizes"])
+        clus()
+        ms_cl = ev_time(clus, 1)
+        prev_state = st
+        agree, agree_frozen, obj = {}, {}, {}
+        for X_, t in ((Q, "q"), (K, "k")):
+            full = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X_, want_lowe=False, want_sums=False)
+            agree[t] = float((st["assign_" + t] == full["assign"]).float().mean())
+            agree_frozen[t] = float((frozen[t] == full["assign"]).float().mean())
+            Xf = X_[0].float()
+            def J(lab, mu):
+                idx = lab.long().unsqueeze(-1).expand(-1, -1, wl.D)
+                return float((Xf - torch.gather(mu, 1, idx)).pow(2).sum())
+            obj[t] = J(st["assign_" + t], st["mu_" + t]) / J(full["assign"], full["mu"])
+        row = {"report": "hybrid", "step": s, "kind": "anchor" if kind == b.HVA_ANCHOR else "subset", "ms_call": round(ms, 3),
+               "ms_clustering": round(ms_cl, 3), "agree_q": round(agree["q"], 4), "agree_k": round(agree["k"], 4),
+               "agree_frozen_q": round(agree_frozen["q"], 4), "agree_frozen_k": round(agree_frozen["k"], 4),
+               "rel_objective_q": round(obj["q"], 4), "rel_objective_k": round(obj["k"], 4)}
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+    anc = [r for r in rows if r["kind"] == "anchor"]; sub = [r for r in rows if r["kind"] == "subset"]
+    mean = lambda xs, k: round(sum(x[k] for x in xs) / max(len(xs), 1), 4)
+    print(json.dumps({"report": "hybrid-summary", "workload": wl.name, "steps": len(rows), "subset_frac": 0.15,
+                      "anchor": {k: mean(anc, k) for k in ("ms_call", "ms_clustering")},
+                      "subset": {k: mean(sub, k) for k in ("ms_call", "ms_clustering", "agree_q", "agree_k", "agree_frozen_q",
+                                                           "agree_frozen_k", "rel_objective_q", "rel_objective_k")}}))
 
 
 def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
@@ -266,10 +378,7 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
                              "algorithmic_bytes": cl_bytes},
         "roofline_permute": {"bound": "hbm", "kernel": "hva_permute_kernel", "achieved": pm_bytes / (st["permute_qkv"] * 1e-3) / 1e9,
                              "peak": pk["hbm"], "unit": "GB/s", "frac": pm_bytes / (st["permute_qkv"] * 1e-3) / 1e9 / pk["hbm"]},
-        "occupancy": {"groups": sum(s["n_groups"] for s in stats), "theoretical_density": pairs / (BH * float(n) * n),
-                      "cta_density": padded / (BH * float(n) * n), "cta_tile_occupancy": pairs / padded,
-                      "q_rows_valid_over_padded": sum(s["q_rows_valid"] for s in stats) / sum(s["q_rows_padded"] for s in stats),
-                      "k_cols_valid_over_padded": sum(s["k_cols_valid"] for s in stats) / sum(s["k_cols_padded"] for s in stats)},
+        "occupancy": occupancy(wl, stats),
     }
     return rep
 
