@@ -131,6 +131,9 @@ int hva_cluster_update(const hva_shape* s, int32_t Nc, const void* X, const int3
                        int32_t refresh_all, int32_t* assign, float* mu, float* sums, int32_t* sizes,
                        void* ws, size_t ws_bytes, void* stream);
 
+/* Scratch needed by one hva_cluster_update call; 0 on invalid arguments. */
+size_t hva_cluster_update_workspace_bytes(const hva_shape* s, int32_t Nc, int32_t m);
+
 /* S5: M[BH,Nq,Nk] uint8 (Eq. 2-3, l.47-54; min-kc l.334).  fp64 on device from the fp32
  * centroids; order by weight descending, ties -> lower j; smallest prefix with cumulative
  * weight >= top_p * Z; top_p >= 1 -> all ones; at least ceil(min_kc*Nk) kept.  Nk <= 2048. */

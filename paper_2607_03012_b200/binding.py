@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libhva.so")
 HVA_F32, HVA_BF16 = 0, 1
 HVA_ANCHOR, HVA_INTERMEDIATE, HVA_DENSE = 0, 1, 2
 
-EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_cluster_workspace_bytes",
+EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes",
            "hva_plan_describe", "hva_cluster", "hva_select_subset", "hva_cluster_update", "hva_build_mask", "hva_merge",
            "hva_build_plan", "hva_permute", "hva_unpermute", "hva_sparse_attention", "hva_forward", "hva_forward_host"]
 
@@ -59,6 +59,7 @@ def lib():
         L.hva_workspace_bytes.restype = C.c_size_t
         L.hva_state_bytes.restype = C.c_size_t
         L.hva_cluster_workspace_bytes.restype = C.c_size_t
+        L.hva_cluster_update_workspace_bytes.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -162,7 +163,7 @@ def hva_select_subset(lowe, m):
 def hva_cluster_update(shape, X, subset, assign, mu, sums, sizes, refresh_all=0):
     """In place on assign / mu / sums / sizes."""
     BH, m = subset.shape
-    ws = _ws(BH * max(m, 1) * 8 + 512, X.device)
+    ws = _ws(lib().hva_cluster_update_workspace_bytes(C.byref(shape), int(mu.shape[1]), int(m)), X.device)
     _check(lib().hva_cluster_update(C.byref(shape), mu.shape[1], _p(X), _p(subset), int(m), int(refresh_all), _p(assign),
                                     _p(mu), _p(sums), _p(sizes), _p(ws), C.c_size_t(ws.numel()), _stream()))
 

@@ -346,6 +346,15 @@ size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D) {
          2 * hva_align((size_t)BH * g.Nc * D * sizeof(__nv_bfloat16)) + hva_align((size_t)BH * g.Nc * sizeof(float));
 }
 
+int hva_mu_split_launch(int BH, int Nc, int D, const float* mu, void* mu_hi, void* mu_lo, float* musq, cudaStream_t st) {
+  const MuSplit sp{reinterpret_cast<__nv_bfloat16*>(mu_hi), reinterpret_cast<__nv_bfloat16*>(mu_lo), musq};
+  if (D == 128) hva_mu_split_kernel<128><<<dim3(Nc, BH), 128, 0, st>>>(Nc, mu, sp);
+  else if (D == 64) hva_mu_split_kernel<64><<<dim3(Nc, BH), 64, 0, st>>>(Nc, mu, sp);
+  else return HVA_EINVAL;
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
+}
+
 extern "C" size_t hva_cluster_workspace_bytes(const hva_shape* s, const int32_t cell[3], const int32_t win[3]) {
   if (!s || !cell || !win || s->B < 1 || s->heads < 1 || s->T < 1 || s->H < 1 || s->W < 1) return 0;
   for (int a = 0; a < 3; ++a)

@@ -16,3 +16,53 @@ bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype);
 int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, HvaAssignTc* out);
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
                          int* part_cnt, int* assign, float* lowe, float* probe, cudaStream_t st);
+
+// Window-less variant for the hybrid subset step (hybrid_tc.cu): subset tokens against ALL centroids.
+bool hva_subset_tc_supported(int D, int dtype, int Nc);
+int hva_subset_assign_tc_launch(int BH, int n, int Nc, int m, const void* X, const int* subset, const float* mu, const void* mu_hi,
+                                const void* mu_lo, const float* musq, const int* assign, int* oldlab, int* newlab, cudaStream_t st);
+// two-term bf16 split + |mu|^2 of fp32 centroids [BH, Nc, D] (cluster.cu)
+int hva_mu_split_launch(int BH, int Nc, int D, const float* mu, void* mu_hi, void* mu_lo, float* musq, cudaStream_t st);
+
+#ifdef __CUDACC__
+namespace hva_tc_dev {
+// |tensor-pipe dot - exact dot| <= kEpsDot |x| |mu|: split error 2^-18 plus fp32 accumulation of 256 exact
+// products.  Observed on B200 (HVA_CLUSTER_PROBE, tests/test_gpu_parity.py): score error 4.6e-6 |x||mu| including the
+// rounding of the fp32 direct form it is compared with, against the 2 kEpsDot = 6.1e-5 assumed: 13x head room.
+constexpr float kEpsDot = 1.0f / 32768.0f;
+
+// 16-byte chunk q (0..15) of token row r in the swizzled A tile
+__device__ __forceinline__ const uint4* x_chunk(const unsigned char* sA, int half_bytes, int r, int q) {
+  return reinterpret_cast<const uint4*>(sA + (q >> 3) * half_bytes + r * 128 + (((q & 7) ^ (r & 7)) << 4));
+}
+__device__ __forceinline__ void unpack8(const uint4& r, float x[8]) {   // bf16 -> fp32 is a 16-bit shift (exact)
+  x[0] = __uint_as_float(r.x << 16); x[1] = __uint_as_float(r.x & 0xffff0000u);
+  x[2] = __uint_as_float(r.y << 16); x[3] = __uint_as_float(r.y & 0xffff0000u);
+  x[4] = __uint_as_float(r.z << 16); x[5] = __uint_as_float(r.z & 0xffff0000u);
+  x[6] = __uint_as_float(r.w << 16); x[7] = __uint_as_float(r.w & 0xffff0000u);
+}
+
+// exact direct form sum_c (x_c - mu_c)^2, fp32, sequential in c (Eq. 5)
+__device__ __forceinline__ float direct_dist(const unsigned char* sA, int half_bytes, int r, const float* __restrict__ mu) {
+  float acc = 0.f;
+#pragma unroll 4
+  for (int q = 0; q < 16; ++q) {
+    float x[8];
+    unpack8(*x_chunk(sA, half_bytes, r, q), x);
+    const float4 m0 = __ldg(reinterpret_cast<const float4*>(mu) + 2 * q);
+    const float4 m1 = __ldg(reinterpret_cast<const float4*>(mu) + 2 * q + 1);
+    float d;
+    d = x[0] - m0.x; acc = fmaf(d, d, acc);
+    d = x[1] - m0.y; acc = fmaf(d, d, acc);
+    d = x[2] - m0.z; acc = fmaf(d, d, acc);
+    d = x[3] - m0.w; acc = fmaf(d, d, acc);
+    d = x[4] - m1.x; acc = fmaf(d, d, acc);
+    d = x[5] - m1.y; acc = fmaf(d, d, acc);
+    d = x[6] - m1.z; acc = fmaf(d, d, acc);
+    d = x[7] - m1.w; acc = fmaf(d, d, acc);
+  }
+  return acc;
+}
+
+}  // namespace hva_tc_dev
+#endif

@@ -4,6 +4,8 @@
 //                       minimum), then per-centroid deterministic adjustment of sums / sizes / mu
 //                       (DESIGN.md R-H3), or a full refresh of every centroid (R-H3').
 #include "common.cuh"
+#include "cluster_tc.cuh"
+#include <cstdlib>
 
 namespace {
 
@@ -222,20 +224,32 @@ __global__ void __launch_bounds__(D) hva_refresh_kernel(int n, int Nc, const T* 
 
 template <typename T, int D>
 int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, int refresh_all, int* assign, float* mu,
-               float* sums, int* sizes, int* newlab, cudaStream_t st) {
+               float* sums, int* sizes, int* newlab, char* split, int dtype, cudaStream_t st) {
   int* oldlab = newlab + (size_t)BH * (m > 0 ? m : 1);
   const T* x = reinterpret_cast<const T*>(X);
-  size_t smem = (size_t)kCTile * D * 4 + (size_t)kUpdThreads * (D + 16 / sizeof(T)) * sizeof(T);
-  if (cudaFuncSetAttribute(hva_subset_assign_kernel<T, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return HVA_ECUDA;
-  hva_subset_assign_kernel<T, D><<<dim3((m + kUpdThreads - 1) / kUpdThreads, BH), kUpdThreads, smem, st>>>(n, Nc, m, x, subset, mu, assign, oldlab, newlab);
-  HVA_CHECK_LAUNCH();
-  if (!refresh_all) {
+  const char* force = getenv("HVA_CLUSTER_SIMT");
+  if (m > 0 && hva_subset_tc_supported(D, dtype, Nc) && !(force && force[0] == '1')) {
+    // tensor-pipe path: split the cached centroids, then the dense m x N_c x D filter with exact refine (hybrid_tc.cu)
+    char* hi = split;
+    char* lo = hi + hva_align((size_t)BH * Nc * D * 2);
+    float* musq = reinterpret_cast<float*>(lo + hva_align((size_t)BH * Nc * D * 2));
+    HVA_TRY(hva_mu_split_launch(BH, Nc, D, mu, hi, lo, musq, st));
+    HVA_TRY(hva_subset_assign_tc_launch(BH, n, Nc, m, X, subset, mu, hi, lo, musq, assign, oldlab, newlab, st));
+  } else if (m > 0) {
+    size_t smem = (size_t)kCTile * D * 4 + (size_t)kUpdThreads * (D + 16 / sizeof(T)) * sizeof(T);
+    if (cudaFuncSetAttribute(hva_subset_assign_kernel<T, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+      return HVA_ECUDA;
+    hva_subset_assign_kernel<T, D><<<dim3((m + kUpdThreads - 1) / kUpdThreads, BH), kUpdThreads, smem, st>>>(n, Nc, m, x, subset, mu, assign, oldlab, newlab);
+    HVA_CHECK_LAUNCH();
+  }
+  if (!refresh_all && m > 0) {
     hva_subset_apply_kernel<T, D><<<dim3(Nc, BH), D, 0, st>>>(n, Nc, m, x, subset, oldlab, newlab, mu, sums, sizes);
     HVA_CHECK_LAUNCH();
   }
-  hva_subset_commit_kernel<<<dim3((m + 255) / 256, BH), 256, 0, st>>>(n, m, subset, newlab, assign);
-  HVA_CHECK_LAUNCH();
+  if (m > 0) {
+    hva_subset_commit_kernel<<<dim3((m + 255) / 256, BH), 256, 0, st>>>(n, m, subset, newlab, assign);
+    HVA_CHECK_LAUNCH();
+  }
   if (refresh_all) {
     hva_refresh_kernel<T, D><<<dim3(Nc, BH), D, 0, st>>>(n, Nc, x, assign, mu, sums, sizes);
     HVA_CHECK_LAUNCH();
@@ -246,8 +260,13 @@ int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, i
 }  // namespace
 
 size_t hva_hybrid_ws_bytes(int BH, int n, int Nc, int m, int D) {
-  (void)n; (void)Nc; (void)D;
-  return hva_align((size_t)BH * (m > 0 ? m : 1) * 8);
+  (void)n;
+  return hva_align((size_t)BH * (m > 0 ? m : 1) * 8) + 2 * hva_align((size_t)BH * Nc * D * 2) + hva_align((size_t)BH * Nc * 4);
+}
+
+extern "C" size_t hva_cluster_update_workspace_bytes(const hva_shape* s, int32_t Nc, int32_t m) {
+  if (!s || Nc < 1 || m < 0 || s->B < 1 || s->heads < 1) return 0;
+  return hva_hybrid_ws_bytes(s->B * s->heads, s->T * s->H * s->W, Nc, m, s->D);
 }
 
 extern "C" int hva_select_subset(int32_t BH, int32_t n, const float* lowe, int32_t m, int32_t* subset, void* ws,
@@ -272,7 +291,8 @@ extern "C" int hva_cluster_update(const hva_shape* s, int32_t Nc, const void* X,
   if (m == 0 && !refresh_all) return HVA_OK;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   int* newlab = reinterpret_cast<int*>(ws);
-#define HVA_DISPATCH(T, DD) return run_update<T, DD>(BH, n, Nc, m, X, subset, refresh_all, assign, mu, sums, sizes, newlab, st)
+  char* split = reinterpret_cast<char*>(ws) + hva_align((size_t)BH * (m > 0 ? m : 1) * 8);
+#define HVA_DISPATCH(T, DD) return run_update<T, DD>(BH, n, Nc, m, X, subset, refresh_all, assign, mu, sums, sizes, newlab, split, s->dtype, st)
   if (s->dtype == HVA_F32) { if (s->D == 64) HVA_DISPATCH(float, 64); HVA_DISPATCH(float, 128); }
   if (s->D == 64) HVA_DISPATCH(__nv_bfloat16, 64);
   HVA_DISPATCH(__nv_bfloat16, 128);
