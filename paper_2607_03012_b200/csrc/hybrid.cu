@@ -155,47 +155,114 @@ __global__ void __launch_bounds__(kUpdThreads) hva_subset_assign_kernel(int n, i
 }
 
 // ---- per-centroid deterministic adjustment (R-H3): moves are applied in subset order.
-// The CTA of centroid u scans the subset cooperatively (one entry per thread, ballot) and applies the
-// few matching moves sequentially, thread = feature dim.
+// The moved subset entries are bucketed by centroid (count / scan / scatter; the scatter order inside a bucket is
+// arbitrary), the CTA of centroid u then sorts its few entries by subset position and applies them sequentially,
+// thread = feature dim: the result does not depend on the scatter order.
+constexpr int kMoveCap = 1024;   // entries of one centroid sorted in shared memory; beyond that the subset is scanned
+
+__global__ void hva_moves_count_kernel(int Nc, int m, const int* __restrict__ oldlab, const int* __restrict__ newlab,
+                                       int* __restrict__ cnt) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, bh = blockIdx.y;
+  if (i >= m) return;
+  const int ol = oldlab[(size_t)bh * m + i], nl = newlab[(size_t)bh * m + i];
+  if (ol != nl) { atomicAdd(&cnt[(size_t)bh * (Nc + 1) + ol], 1); atomicAdd(&cnt[(size_t)bh * (Nc + 1) + nl], 1); }
+}
+
+// cnt[bh][0..Nc) -> exclusive offsets off[bh][0..Nc] (in place) and a copy as scatter cursors
+__global__ void __launch_bounds__(1024) hva_moves_scan_kernel(int Nc, int* __restrict__ cnt, int* __restrict__ cursor) {
+  const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  __shared__ int s_warp[32];
+  __shared__ int s_carry;
+  if (tid == 0) s_carry = 0;
+  __syncthreads();
+  for (int u0 = 0; u0 <= Nc; u0 += 1024) {
+    const int u = u0 + tid;
+    const int v = u < Nc ? cnt[(size_t)bh * (Nc + 1) + u] : 0;
+    int x = v;
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) s_warp[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+      int w = s_warp[lane], t = w;
+      for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, t, o); if (lane >= o) t += y; }
+      s_warp[lane] = t - w;
+    }
+    __syncthreads();
+    const int excl = s_carry + s_warp[warp] + x - v;
+    if (u <= Nc) { cnt[(size_t)bh * (Nc + 1) + u] = excl; if (u < Nc) cursor[(size_t)bh * Nc + u] = excl; }
+    __syncthreads();
+    if (tid == 1023) s_carry = excl + v;
+    __syncthreads();
+  }
+}
+
+__global__ void hva_moves_scatter_kernel(int Nc, int m, const int* __restrict__ oldlab, const int* __restrict__ newlab,
+                                         int* __restrict__ cursor, int* __restrict__ entries) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, bh = blockIdx.y;
+  if (i >= m) return;
+  const int ol = oldlab[(size_t)bh * m + i], nl = newlab[(size_t)bh * m + i];
+  if (ol != nl) {
+    entries[(size_t)bh * 2 * m + atomicAdd(&cursor[(size_t)bh * Nc + ol], 1)] = i << 1;         // leaves ol
+    entries[(size_t)bh * 2 * m + atomicAdd(&cursor[(size_t)bh * Nc + nl], 1)] = (i << 1) | 1;   // joins nl
+  }
+}
+
 template <typename T, int D>
 __global__ void __launch_bounds__(D) hva_subset_apply_kernel(int n, int Nc, int m, const T* __restrict__ X,
                                                              const int* __restrict__ subset, const int* __restrict__ oldlab,
-                                                             const int* __restrict__ newlab, float* __restrict__ mu,
+                                                             const int* __restrict__ newlab, const int* __restrict__ off,
+                                                             const int* __restrict__ entries, float* __restrict__ mu,
                                                              float* __restrict__ sums, int* __restrict__ sizes) {
   const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x, lane = c & 31, warp = c >> 5;
-  __shared__ unsigned s_bal[D / 32];
-  __shared__ int s_tok[D];
-  __shared__ int s_dir[D];
+  const int e0 = off[(size_t)bh * (Nc + 1) + u], k = off[(size_t)bh * (Nc + 1) + u + 1] - e0;
+  if (k == 0) return;                              // untouched centroid
   const size_t o = ((size_t)bh * Nc + u) * D + c;
   float z = sums[o];
   int cnt = sizes[(size_t)bh * Nc + u];
-  bool touched = false;
-  for (int i0 = 0; i0 < m; i0 += D) {
-    const int i = i0 + c;
-    int ol = -1, nl = -1;
-    if (i < m) { ol = oldlab[(size_t)bh * m + i]; nl = newlab[(size_t)bh * m + i]; }
-    const bool hit = (ol != nl) && (ol == u || nl == u);
-    const unsigned b = __ballot_sync(0xffffffffu, hit);
-    if (lane == 0) s_bal[warp] = b;
-    if (hit) { s_tok[c] = subset[(size_t)bh * m + i]; s_dir[c] = (ol == u) ? -1 : 1; }
+  if (k <= kMoveCap) {
+    __shared__ int s_raw[kMoveCap], s_sorted[kMoveCap];
+    for (int e = c; e < k; e += D) s_raw[e] = entries[(size_t)bh * 2 * m + e0 + e];
     __syncthreads();
-    for (int w = 0; w < D / 32; ++w) {
-      unsigned bits = s_bal[w];
-      while (bits) {
-        int e = w * 32 + __ffs(bits) - 1;
-        bits &= bits - 1;
-        float x = HvaElem<T>::ld(X + ((size_t)bh * n + s_tok[e]) * D + c);
-        if (s_dir[e] < 0) { z -= x; --cnt; } else { z += x; ++cnt; }
-        touched = true;
-      }
+    for (int e = c; e < k; e += D) {               // keys are distinct: rank = number of smaller keys
+      const int key = s_raw[e];
+      int rank = 0;
+      for (int f = 0; f < k; ++f) rank += s_raw[f] < key;
+      s_sorted[rank] = key;
     }
     __syncthreads();
+    for (int e = 0; e < k; ++e) {
+      const int key = s_sorted[e];
+      const float x = HvaElem<T>::ld(X + ((size_t)bh * n + subset[(size_t)bh * m + (key >> 1)]) * D + c);
+      if (key & 1) { z += x; ++cnt; } else { z -= x; --cnt; }
+    }
+  } else {                                         // degenerate: scan the subset in order (one entry per thread, ballot)
+    __shared__ unsigned s_bal[D / 32];
+    __shared__ int s_tok[D];
+    __shared__ int s_dir[D];
+    for (int i0 = 0; i0 < m; i0 += D) {
+      const int i = i0 + c;
+      int ol = -1, nl = -1;
+      if (i < m) { ol = oldlab[(size_t)bh * m + i]; nl = newlab[(size_t)bh * m + i]; }
+      const bool hit = (ol != nl) && (ol == u || nl == u);
+      const unsigned b = __ballot_sync(0xffffffffu, hit);
+      if (lane == 0) s_bal[warp] = b;
+      if (hit) { s_tok[c] = subset[(size_t)bh * m + i]; s_dir[c] = (ol == u) ? -1 : 1; }
+      __syncthreads();
+      for (int w = 0; w < D / 32; ++w) {
+        unsigned bits = s_bal[w];
+        while (bits) {
+          int e = w * 32 + __ffs(bits) - 1;
+          bits &= bits - 1;
+          float x = HvaElem<T>::ld(X + ((size_t)bh * n + s_tok[e]) * D + c);
+          if (s_dir[e] < 0) { z -= x; --cnt; } else { z += x; ++cnt; }
+        }
+      }
+      __syncthreads();
+    }
   }
-  if (touched) {
-    sums[o] = z;
-    if (c == 0) sizes[(size_t)bh * Nc + u] = cnt;
-    if (cnt > 0) mu[o] = __fdiv_rn(z, (float)cnt);
-  }
+  sums[o] = z;
+  if (c == 0) sizes[(size_t)bh * Nc + u] = cnt;
+  if (cnt > 0) mu[o] = __fdiv_rn(z, (float)cnt);
 }
 
 __global__ void hva_subset_commit_kernel(int n, int m, const int* __restrict__ subset, const int* __restrict__ newlab,
@@ -243,7 +310,17 @@ int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, i
     HVA_CHECK_LAUNCH();
   }
   if (!refresh_all && m > 0) {
-    hva_subset_apply_kernel<T, D><<<dim3(Nc, BH), D, 0, st>>>(n, Nc, m, x, subset, oldlab, newlab, mu, sums, sizes);
+    int* off = reinterpret_cast<int*>(split + 2 * hva_align((size_t)BH * Nc * D * 2) + hva_align((size_t)BH * Nc * 4));
+    int* cursor = off + hva_align((size_t)BH * (Nc + 1) * 4) / 4;
+    int* entries = cursor + hva_align((size_t)BH * Nc * 4) / 4;
+    if (cudaMemsetAsync(off, 0, (size_t)BH * (Nc + 1) * 4, st) != cudaSuccess) return HVA_ECUDA;
+    hva_moves_count_kernel<<<dim3((m + 255) / 256, BH), 256, 0, st>>>(Nc, m, oldlab, newlab, off);
+    HVA_CHECK_LAUNCH();
+    hva_moves_scan_kernel<<<BH, 1024, 0, st>>>(Nc, off, cursor);
+    HVA_CHECK_LAUNCH();
+    hva_moves_scatter_kernel<<<dim3((m + 255) / 256, BH), 256, 0, st>>>(Nc, m, oldlab, newlab, cursor, entries);
+    HVA_CHECK_LAUNCH();
+    hva_subset_apply_kernel<T, D><<<dim3(Nc, BH), D, 0, st>>>(n, Nc, m, x, subset, oldlab, newlab, off, entries, mu, sums, sizes);
     HVA_CHECK_LAUNCH();
   }
   if (m > 0) {
@@ -261,7 +338,8 @@ int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, i
 
 size_t hva_hybrid_ws_bytes(int BH, int n, int Nc, int m, int D) {
   (void)n;
-  return hva_align((size_t)BH * (m > 0 ? m : 1) * 8) + 2 * hva_align((size_t)BH * Nc * D * 2) + hva_align((size_t)BH * Nc * 4);
+  return hva_align((size_t)BH * (m > 0 ? m : 1) * 8) + 2 * hva_align((size_t)BH * Nc * D * 2) + hva_align((size_t)BH * Nc * 4) +
+         hva_align((size_t)BH * (Nc + 1) * 4) + hva_align((size_t)BH * Nc * 4) + hva_align((size_t)BH * 2 * (m > 0 ? m : 1) * 4);
 }
 
 extern "C" size_t hva_cluster_update_workspace_bytes(const hva_shape* s, int32_t Nc, int32_t m) {
