@@ -22,7 +22,7 @@ import torch
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
-from paper_2607_03012_b200 import inputs  # noqa: E402
+from paper_2607_03012_b200 import inputs, sharding  # noqa: E402
 
 METRIC = "sparse-attn ms/call + clustering ms/step at 118,800-token HunyuanVideo shape"
 
@@ -187,9 +187,7 @@ def main():
     ms = ev_time(step, args.steps)
     clocks = clk.stop()
     if world > 1:
-        tt = torch.tensor([ms], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+        ms = sharding.max_over_ranks(ms, device="cuda")
         dist.barrier()
     stats = fwd.stats_dicts()
 
@@ -204,7 +202,7 @@ def main():
     nbytes = Q.numel() * Q.element_size()
     del dev4
 
-    out = {"metric": METRIC, "value": ms / world, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+    out = {"metric": METRIC, "value": sharding.whole_job_value(ms, world), "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
            "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
            "config": {"workload": wl.name, "B": wl.B, "heads": wl.heads, "n": wl.n, "D": wl.D, "cell": wl.cell, "iters": wl.iters,
