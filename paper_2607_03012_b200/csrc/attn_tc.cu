@@ -24,8 +24,8 @@ using namespace hva_ptx;
 constexpr int kBM = 128, kBN = 128, kD = 128;
 constexpr int kHalfBytes = 128 * 128;          // one 64-dim half of a 128-row tile: 128 rows x 128 B
 constexpr int kTileBytes = 2 * kHalfBytes;     // 32 KB
-constexpr int kStages = 3;                     // K ring and V ring of three 128-row tiles each
-constexpr int kThreadsTC = 416;                // warps 0-7 softmax (two threads per query row), 9: MMA, 8/10/11/12: TMA
+constexpr int kStagesK = 3, kStagesV = 3;      // K ring and V ring of 128-row tiles (4 + 2 measured the same: the rings are L2-bandwidth bound)
+constexpr int kThreadsTC = 512;                // 4 warpgroups: 0-1 softmax (setmaxnreg 200), 2-3 MMA / TMA warps + idle (setmaxnreg 56)                // warps 0-3 / 4-7 softmax of the even / odd key tiles, 9: MMA, TMA: 8 = K dims 0-63 (+Q), 11 = K dims 64-127, 10 = V
 constexpr int kNumBoxes = 8;                   // box heights 1,2,4,...,128
 constexpr uint32_t kTmemCols = 512;            // S_0, S_1 (fp32 scores), O (fp32), P_0, P_1 (bf16 probabilities)
 constexpr uint32_t kColS = 0, kColO = 256, kColP = 384;   // S_b at kColS + 128 b, P_b at kColP + 64 b
@@ -73,12 +73,16 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
 #endif
 
 struct __align__(8) TcBarriers {
-  uint64_t q_full, k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages], s_full[2], s_free[2], p_ready[2], p_free[2];
+  uint64_t q_full, k_full[kStagesK], k_empty[kStagesK], v_full[kStagesV], v_empty[kStagesV], s_full[2], s_free[2], p_ready[2], p_free[2];
   uint32_t tmem_base;
-  float xch[2][kBM];          // half-row maxima / sums exchanged between the two threads of a query row
+  float xch[2][kBM];          // partial row sums of the two softmax sets
+  float mref[kBM];            // reference exponent of each query row (shared by its two softmax threads)
+  int seq[kBM];               // number of key tiles whose reference decision has been taken, per row
 };
 
-constexpr size_t kSmemTC = 1024 + kTileBytes * (1 + 2 * kStages) + sizeof(TcBarriers);
+constexpr int kAlignSlack = 512;               // the dynamic window is 1024-byte aligned in practice (checked in the kernel)
+constexpr size_t kSmemTC = kAlignSlack + kTileBytes * (1 + kStagesK + kStagesV) + sizeof(TcBarriers);
+static_assert(kSmemTC <= 227 * 1024, "attention tile ring exceeds the shared memory of one SM");
 
 // Walks the group's key runs (maximal runs of consecutive selected key clusters, contiguous in K')
 // and packs them back to back into 128-row tiles (l.109).
@@ -91,29 +95,34 @@ struct RunWalker {
   }
 };
 
+template <int HALVES>
 __device__ __forceinline__ void emit_boxes(const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col, int grow, int dst, int len) {
 #pragma unroll 1
   for (int b = kNumBoxes - 1; b >= 0; --b) {
     const int h = 1 << b;
     if (len & h) {
-      if (elect_one()) tma_load_2d(maps + b, bar, stage + dst * 128, col, grow);
+      if (elect_one()) {
+        tma_load_2d(maps + b, bar, stage + dst * 128, col, grow);
+        if (HALVES == 2) tma_load_2d(maps + b, bar, stage + kHalfBytes + dst * 128, col + 64, grow);
+      }
       grow += h; dst += h;
     }
   }
 }
 
-// one 64-dim half (column `col`) of a packed key tile
+// HALVES = 1: the 64-dim half at column `col` only; 2: both halves
+template <int HALVES>
 __device__ __forceinline__ void load_tile(RunWalker& w, const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col,
                                           int base_row, int rows_valid, int rows_load) {
   int dst = 0;
   while (dst < rows_valid) {
     while (w.used == w.len) { ++w.r; w.load(); }
     int seg = min(w.len - w.used, rows_valid - dst);
-    emit_boxes(maps, bar, stage, col, base_row + w.row0 + w.used, dst, seg);
+    emit_boxes<HALVES>(maps, bar, stage, col, base_row + w.row0 + w.used, dst, seg);
     w.used += seg; dst += seg;
   }
   if (rows_load > rows_valid)   // ragged last tile: round up to the MMA K granule with finite over-read rows
-    emit_boxes(maps, bar, stage, col, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
+    emit_boxes<HALVES>(maps, bar, stage, col, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
 }
 
 __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid_constant__ TcMaps maps, TcParams p) {
@@ -128,12 +137,13 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int base_row = bh * p.n;
 
-  extern __shared__ unsigned char smem_raw[];
-  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  if (smem - smem_raw > kAlignSlack) __trap();
   unsigned char* sQ = smem;
   unsigned char* sK = smem + kTileBytes;
-  unsigned char* sV = smem + kTileBytes * (1 + kStages);
-  TcBarriers* B = reinterpret_cast<TcBarriers*>(smem + kTileBytes * (1 + 2 * kStages));
+  unsigned char* sV = smem + kTileBytes * (1 + kStagesK);
+  TcBarriers* B = reinterpret_cast<TcBarriers*>(smem + kTileBytes * (1 + kStagesK + kStagesV));
 
   if (jn == 0) {   // no key selected: defined as a zero row
     if (tid < kBM && row0 + tid < row1) {
@@ -146,13 +156,11 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
 
   if (tid == 0) {
     mbar_init(&B->q_full, 1);
-    for (int s = 0; s < kStages; ++s) {
-      mbar_init(&B->k_full[s], 2); mbar_init(&B->k_empty[s], 1);     // two producers (one per 64-dim half) per ring
-      mbar_init(&B->v_full[s], 2); mbar_init(&B->v_empty[s], 1);
-    }
+    for (int s = 0; s < kStagesK; ++s) { mbar_init(&B->k_full[s], 2); mbar_init(&B->k_empty[s], 1); }   // two producers (one per
+    for (int s = 0; s < kStagesV; ++s) { mbar_init(&B->v_full[s], 2); mbar_init(&B->v_empty[s], 1); }   // 64-dim half) per ring
     mbar_init(&B->s_full[0], 1); mbar_init(&B->s_full[1], 1);
-    mbar_init(&B->p_ready[0], 256); mbar_init(&B->p_ready[1], 256);
-    mbar_init(&B->s_free[0], 256); mbar_init(&B->s_free[1], 256);
+    mbar_init(&B->p_ready[0], 128); mbar_init(&B->p_ready[1], 128);     // set b = warps 4b..4b+3 owns S_b, P_b
+    mbar_init(&B->s_free[0], 128); mbar_init(&B->s_free[1], 128);
     mbar_init(&B->p_free[0], 1); mbar_init(&B->p_free[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -161,15 +169,17 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&B->tmem_base)), "r"(kTmemCols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
+  if (tid < kBM) { B->mref[tid] = -INFINITY; B->seq[tid] = 0; }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = B->tmem_base;
-
-  if (warp == 8 || warp >= 10) {
+  // register file: 512 threads x 128 at launch; the two softmax warpgroups hold a 128-column row each and take 200, the rest gives back
+  if (warp == 8 || (warp >= 10 && warp <= 12)) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
     // ===================================================== TMA producers (warp-uniform, one elected lane issues):
-    // warp 8: K ring dims 0-63 (+ Q), warp 10: V ring dims 0-63, warp 11: K ring dims 64-127, warp 12: V ring dims 64-127
-    const bool is_k = (warp == 8 || warp == 11);
+    // the K ring is on the critical path (QK_{j+2} is issued two tiles ahead): one warp per 64-dim half; one warp for the V ring
+    const bool is_k = (warp == 8 || warp == 11);   // 8: K dims 0-63 (+Q), 11: K dims 64-127, 10: V dims 0-63, 12: V dims 64-127
     const int half = warp >= 11;
     if (warp == 8 && elect_one()) {
       mbar_expect_tx(&B->q_full, kTileBytes);
@@ -184,15 +194,17 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     uint64_t* empty = is_k ? B->k_empty : B->v_empty;
     unsigned char* ring = (is_k ? sK : sV) + half * kHalfBytes;
     for (int j = 0; j < jn; ++j) {
-      const int s = j % kStages, use = j / kStages;
+      const int ns = is_k ? kStagesK : kStagesV;
+      const int s = j % ns, use = j / ns;
       const int rows_valid = min(kBN, kappa - j * kBN);
       const int rows_load = rows_valid == kBN ? kBN : (rows_valid + 15) & ~15;
       if (use > 0) mbar_wait(&empty[s], (use - 1) & 1);
       if (elect_one()) mbar_expect_tx(&full[s], rows_load * 128);
       __syncwarp();
-      load_tile(w, mp, &full[s], ring + s * kTileBytes, half * 64, base_row, rows_valid, rows_load);
+      load_tile<1>(w, mp, &full[s], ring + s * kTileBytes, half * 64, base_row, rows_valid, rows_load);
     }
   } else if (warp == 9) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
     // ===================================================== MMA issuer: the whole warp runs the loop (uniform), one elected lane issues
     // S and P are double buffered and separate: QK_{j+2} is issued as soon as the softmax threads have pulled S_j into
     // registers (s_free), PV_j when P_j is complete (p_ready); the softmax of tile j+2 reuses P_b once PV_j is done (p_free).
@@ -206,9 +218,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     long long tprev = clock64();
 #endif
     auto issue_qk = [&](int j) {
-      const int s = j % kStages, b = j & 1;
+      const int s = j % kStagesK, b = j & 1;
       AMARK(0);
-      mbar_wait(&B->k_full[s], (j / kStages) & 1);
+      mbar_wait(&B->k_full[s], (j / kStagesK) & 1);
       AMARK(1);
       tc_fence_after();
       const uint64_t dks = dk + (uint64_t)(s * (kTileBytes >> 4));
@@ -228,7 +240,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     issue_qk(0);
     if (jn > 1) issue_qk(1);
     for (int j = 0; j < jn; ++j) {
-      const int s = j % kStages, b = j & 1;
+      const int s = j % kStagesV, b = j & 1;
       if (j + 2 < jn) {
         AMARK(0);
         mbar_wait(&B->s_free[b], (j >> 1) & 1);
@@ -238,7 +250,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
       AMARK(0);
       mbar_wait(&B->p_ready[b], (j >> 1) & 1);
       AMARK(3);
-      mbar_wait(&B->v_full[s], (j / kStages) & 1);
+      mbar_wait(&B->v_full[s], (j / kStagesV) & 1);
       AMARK(4);
       tc_fence_after();
       const int rows_valid = min(kBN, kappa - j * kBN);
@@ -262,76 +274,93 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     if (p.probe && lane == 0) for (int k = 0; k < 8; ++k) atomicAdd(p.probe + k, tacc[k]);
 #endif
   } else if (warp < 8) {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 200;");
     // ===================================================== softmax / correction / epilogue
-    // thread = (query row, half): row = TMEM lane 32 (warp & 3) + lane, half h = warp >> 2 owns key columns [64h, 64h + 64)
-    const int h = warp >> 2, r = (warp & 3) * 32 + lane;
+    // Two sets of 128 threads alternate over the key tiles: set b = warp >> 2 takes the tiles j = b (mod 2), i.e. always
+    // the buffers S_b / P_b; thread = one full query row (TMEM lane 32 (warp & 3) + lane) held in 128 registers.  While one
+    // set loads and reduces its tile the other one is in the MUFU-bound exponentials.  The two threads of a row share the
+    // row's reference exponent through shared memory: decisions are taken in tile order (seq[r] = tiles decided), each
+    // thread keeps its own partial row sum relative to the reference it last saw.
+    const int b = warp >> 2, r = (warp & 3) * 32 + lane;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t s_addr = tmem + lane_base + kColS + b * 128, p_addr = tmem + lane_base + kColP + b * 64;
     const float sl2 = p.scale_log2;
     const float2 sl2x2 = make_float2(sl2, sl2);
-    float m_ref = -INFINITY;          // reference exponent (log2 units) of the row: P = 2^(s*scale*log2e - m_ref)
+    float m_seen = -INFINITY;         // reference (log2 units) the partial sum l2 is relative to: P = 2^(s*scale*log2e - m_ref)
     float2 l2 = make_float2(0.f, 0.f);
-    uint32_t va[32], vb[32];
+    uint32_t v0[32], v1[32], v2[32], v3[32];
+    volatile int* seq = B->seq;
+    volatile float* mref = B->mref;
 #ifdef HVA_ATTN_TIMING
     unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long tprev = clock64();
 #endif
-    for (int j = 0; j < jn; ++j) {
-      const int b = j & 1;
-      const uint32_t s_addr = tmem + lane_base + kColS + b * 128;
+    for (int j = b; j < jn; j += 2) {
       const int rows_valid = min(kBN, kappa - j * kBN);
       AMARK(0);
       mbar_wait(&B->s_full[b], (j >> 1) & 1);
       AMARK(1);
       tc_fence_after();
-      // half-row maximum; the 64 scores stay in registers (P_j is written over S_j only after both halves have read it)
-      tmem_ld32(s_addr + h * 64, va);
-      tmem_ld32(s_addr + h * 64 + 32, vb);
+      tmem_ld32_nowait(s_addr, v0);
+      tmem_ld32_nowait(s_addr + 32, v1);
+      tmem_ld32_nowait(s_addr + 64, v2);
+      tmem_ld32_nowait(s_addr + 96, v3);
+      tmem_ld_wait();
       tc_fence_before();
-      mbar_arrive(&B->s_free[b]);          // the scores are in registers: the MMA warp may overwrite S_b with QK_{j+2}
+      mbar_arrive(&B->s_free[b]);          // the row is in registers: the MMA warp may overwrite S_b with QK_{j+2}
       if (rows_valid != kBN) {
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          if (h * 64 + i >= rows_valid) va[i] = 0xff800000u;   // -inf: key columns past the packed list
-          if (h * 64 + 32 + i >= rows_valid) vb[i] = 0xff800000u;
+        for (int i = 0; i < 32; ++i) {     // -inf: key columns past the packed list
+          if (i >= rows_valid) v0[i] = 0xff800000u;
+          if (32 + i >= rows_valid) v1[i] = 0xff800000u;
+          if (64 + i >= rows_valid) v2[i] = 0xff800000u;
+          if (96 + i >= rows_valid) v3[i] = 0xff800000u;
         }
       }
-      float mx0 = fmaxf(__uint_as_float(va[0]), __uint_as_float(va[1])), mx1 = fmaxf(__uint_as_float(vb[0]), __uint_as_float(vb[1]));
+      float mx0 = fmaxf(__uint_as_float(v0[0]), __uint_as_float(v0[1])), mx1 = fmaxf(__uint_as_float(v1[0]), __uint_as_float(v1[1]));
+      float mx2 = fmaxf(__uint_as_float(v2[0]), __uint_as_float(v2[1])), mx3 = fmaxf(__uint_as_float(v3[0]), __uint_as_float(v3[1]));
 #pragma unroll
       for (int i = 2; i < 32; i += 2) {
-        mx0 = fmaxf(mx0, fmaxf(__uint_as_float(va[i]), __uint_as_float(va[i + 1])));
-        mx1 = fmaxf(mx1, fmaxf(__uint_as_float(vb[i]), __uint_as_float(vb[i + 1])));
+        mx0 = fmaxf(mx0, fmaxf(__uint_as_float(v0[i]), __uint_as_float(v0[i + 1])));
+        mx1 = fmaxf(mx1, fmaxf(__uint_as_float(v1[i]), __uint_as_float(v1[i + 1])));
+        mx2 = fmaxf(mx2, fmaxf(__uint_as_float(v2[i]), __uint_as_float(v2[i + 1])));
+        mx3 = fmaxf(mx3, fmaxf(__uint_as_float(v3[i]), __uint_as_float(v3[i + 1])));
       }
-      const float m_half = fmaxf(mx0, mx1);
-      B->xch[h][r] = m_half;
-      tc_fence_before();
+      const float m_c = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * sl2;
       AMARK(2);
-      asm volatile("bar.sync 1, 256;" ::: "memory");
+      // reference decisions are sequential in j: wait for the partner's decision on tile j-1 (normally long taken)
+      while (seq[r] != j) { }
+      __threadfence_block();
+      float m_ref = mref[r];
       AMARK(3);
-      tc_fence_after();
-      const float m_c = fmaxf(m_half, B->xch[h ^ 1][r]) * sl2;
-      // the reference only moves when a score exceeds it by > 2^8 (lazy rescale); both threads of a row take the same decision
+      if (m_ref != m_seen) { const float f0 = ex2(m_seen - m_ref); l2.x *= f0; l2.y *= f0; m_seen = m_ref; }   // m_seen = -inf: l2 = 0
+      // the reference only moves when a score exceeds it by > 2^8 (lazy rescale); then O (complete up to PV_{j-1}) is rescaled
       if (__any_sync(0xffffffffu, m_c - m_ref > kRescaleThreshold)) {
         const float m_new = fmaxf(m_ref, m_c);
         const float f = (m_new == m_ref) ? 1.f : ex2(m_ref - m_new);
         l2.x *= f; l2.y *= f;
-        if (j > 0) {                                   // O columns [64h, 64h + 64) of the row
-          mbar_wait(&B->p_free[(j - 1) & 1], ((j - 1) >> 1) & 1);   // PV_{j-1} complete
+        if (j > 0) {
+          mbar_wait(&B->p_free[b ^ 1], ((j - 1) >> 1) & 1);   // PV_{j-1} complete
           tc_fence_after();
           uint32_t o[16];
 #pragma unroll 1
-          for (int cc = 0; cc < 4; ++cc) {
-            tmem_ld16(tmem + lane_base + kColO + h * 64 + cc * 16, o);
+          for (int cc = 0; cc < 8; ++cc) {
+            tmem_ld16(tmem + lane_base + kColO + cc * 16, o);
 #pragma unroll
             for (int i = 0; i < 16; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-            tmem_st16(tmem + lane_base + kColO + h * 64 + cc * 16, o);
+            tmem_st16(tmem + lane_base + kColO + cc * 16, o);
           }
+          tmem_st_wait();
+          tc_fence_before();
         }
-        m_ref = m_new;
+        m_ref = m_new; m_seen = m_new;
+        mref[r] = m_new;
       }
+      __threadfence_block();
+      seq[r] = j + 1;
       AMARK(4);
       if (j >= 2) { mbar_wait(&B->p_free[b], ((j - 2) >> 1) & 1); tc_fence_after(); }   // PV_{j-2} has read P_b
       AMARK(5);
-      const uint32_t p_addr = tmem + lane_base + kColP + b * 64;
       const float2 nm = make_float2(-m_ref, -m_ref);
       auto exp_chunk = [&](const uint32_t (&vv)[32], int c) {
         uint32_t pk[16];
@@ -347,10 +376,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
           l2 = __fadd2_rn(l2, e);
           pk[i] = pack_bf16(e.x, e.y);
         }
-        tmem_st16(p_addr + h * 32 + c * 16, pk);
+        tmem_st16(p_addr + c * 16, pk);
       };
-      exp_chunk(va, 0);
-      exp_chunk(vb, 1);
+      exp_chunk(v0, 0); exp_chunk(v1, 1); exp_chunk(v2, 2); exp_chunk(v3, 3);
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(&B->p_ready[b]);
@@ -359,12 +387,17 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
 #ifdef HVA_ATTN_TIMING
     if (p.probe && tid == 0) for (int k = 0; k < 8; ++k) atomicAdd(p.probe + 8 + k, tacc[k]);
 #endif
-    // row sum = both halves
-    const float l_half = l2.x + l2.y;
-    B->xch[h][r] = l_half;
+    // final reference of the row, partial sums of the two sets
+    while (seq[r] != jn) { }
+    __threadfence_block();
+    {
+      const float m_fin = mref[r];
+      if (m_fin != m_seen) { const float f0 = ex2(m_seen - m_fin); l2.x *= f0; l2.y *= f0; }
+    }
+    B->xch[b][r] = l2.x + l2.y;
     asm volatile("bar.sync 1, 256;" ::: "memory");
-    const float l = l_half + B->xch[h ^ 1][r];
-    // epilogue: O / l, bf16, row store with the inverse permutation fused (Eq. 4: O = Pi^{q-1} O'); 64 columns per thread
+    const float l = B->xch[0][r] + B->xch[1][r];
+    // epilogue: O / l, bf16, row store with the inverse permutation fused (Eq. 4: O = Pi^{q-1} O'); set b stores columns [64b, 64b+64)
     mbar_wait(&B->p_free[(jn - 1) & 1], ((jn - 1) >> 1) & 1);   // last PV complete
     tc_fence_after();
     const float inv = 1.f / l;
@@ -375,9 +408,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
 #pragma unroll 1
     for (int c = 0; c < 2; ++c) {
       uint32_t o[32];
-      tmem_ld32(tmem + lane_base + kColO + h * 64 + c * 32, o);
+      tmem_ld32(tmem + lane_base + kColO + b * 64 + c * 32, o);
       if (ok) {
-        uint4* dst = reinterpret_cast<uint4*>(p.O + orow * kD + h * 64 + c * 32);
+        uint4* dst = reinterpret_cast<uint4*>(p.O + orow * kD + b * 64 + c * 32);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           uint4 w;
@@ -389,6 +422,8 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
         }
       }
     }
+  } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");   // idle warps of the last warpgroup
   }
   tc_fence_before();
   __syncthreads();
