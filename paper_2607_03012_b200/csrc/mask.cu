@@ -78,9 +78,13 @@ __global__ void __launch_bounds__(kMaskThreads) hva_mask_kernel(int Nq, int Nk, 
       s_j[j] = j;
     }
     __syncthreads();
-    for (int k = 2; k <= P; k <<= 1) {              // bitonic sort, order `before`
+    // bitonic sort, order `before`.  Warp w owns the contiguous segment [w seg, (w+1) seg), seg = P / 8: every pass with
+    // j < seg stays inside the segment and only needs a warp-level barrier; block barriers around the passes that cross
+    // segments (10 instead of 55 for P = 1024).
+    const int seg = P / (kMaskThreads / 32), wbase = (tid >> 5) * seg, lane = tid & 31;
+    for (int k = 2; k <= P; k <<= 1) {
       for (int j = k >> 1; j > 0; j >>= 1) {
-        for (int a = tid; a < P; a += kMaskThreads) {
+        for (int a = wbase + lane; a < wbase + seg; a += 32) {
           int b = a ^ j;
           if (b > a) {
             double wa = s_w[a], wb = s_w[b];
@@ -90,7 +94,7 @@ __global__ void __launch_bounds__(kMaskThreads) hva_mask_kernel(int Nq, int Nk, 
             if (swap) { s_w[a] = wb; s_w[b] = wa; s_j[a] = jb; s_j[b] = ja; }
           }
         }
-        __syncthreads();
+        if (j >= seg || (j == 1 && k >= seg)) __syncthreads(); else __syncwarp();
       }
     }
     // inclusive scan of the sorted weights: per-thread contiguous chunk, then scan of the chunk sums
