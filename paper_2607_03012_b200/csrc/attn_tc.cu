@@ -95,34 +95,32 @@ struct RunWalker {
   }
 };
 
-template <int HALVES>
-__device__ __forceinline__ void emit_boxes(const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col, int grow, int dst, int len) {
-#pragma unroll 1
-  for (int b = kNumBoxes - 1; b >= 0; --b) {
-    const int h = 1 << b;
-    if (len & h) {
-      if (elect_one()) {
-        tma_load_2d(maps + b, bar, stage + dst * 128, col, grow);
-        if (HALVES == 2) tma_load_2d(maps + b, bar, stage + kHalfBytes + dst * 128, col + 64, grow);
-      }
-      grow += h; dst += h;
-    }
+// One segment of `len` consecutive source rows -> `len` consecutive tile rows.  A TMA box costs ~100 clk of the SM's TMA unit
+// whatever its height (microbenchmark), and the box count paces the rings: instead of the binary decomposition
+// (popcount(len) boxes) a segment takes at most TWO boxes of the largest power of two h <= len, at offsets 0 and len - h;
+// the overlap is written twice with the same bytes.  Returns the bytes issued (for the barrier's expect-tx).
+__device__ __forceinline__ int emit_boxes(const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col, int grow, int dst, int len) {
+  const int b = 31 - __clz(len), h = 1 << b;
+  if (elect_one()) {
+    tma_load_2d(maps + b, bar, stage + dst * 128, col, grow);
+    if (len != h) tma_load_2d(maps + b, bar, stage + (dst + len - h) * 128, col, grow + len - h);
   }
+  return (len != h ? 2 * h : h) * 128;
 }
 
-// HALVES = 1: the 64-dim half at column `col` only; 2: both halves
-template <int HALVES>
-__device__ __forceinline__ void load_tile(RunWalker& w, const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col,
-                                          int base_row, int rows_valid, int rows_load) {
-  int dst = 0;
+// the 64-dim half at column `col` of a packed key tile; returns the bytes issued
+__device__ __forceinline__ int load_tile(RunWalker& w, const CUtensorMap* maps, uint64_t* bar, unsigned char* stage, int col,
+                                         int base_row, int rows_valid, int rows_load) {
+  int dst = 0, bytes = 0;
   while (dst < rows_valid) {
     while (w.used == w.len) { ++w.r; w.load(); }
     int seg = min(w.len - w.used, rows_valid - dst);
-    emit_boxes<HALVES>(maps, bar, stage, col, base_row + w.row0 + w.used, dst, seg);
+    bytes += emit_boxes(maps, bar, stage, col, base_row + w.row0 + w.used, dst, seg);
     w.used += seg; dst += seg;
   }
   if (rows_load > rows_valid)   // ragged last tile: round up to the MMA K granule with finite over-read rows
-    emit_boxes<HALVES>(maps, bar, stage, col, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
+    bytes += emit_boxes(maps, bar, stage, col, base_row + w.row0 + w.used, dst, rows_load - rows_valid);
+  return bytes;
 }
 
 __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid_constant__ TcMaps maps, TcParams p) {
@@ -199,9 +197,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
       const int rows_valid = min(kBN, kappa - j * kBN);
       const int rows_load = rows_valid == kBN ? kBN : (rows_valid + 15) & ~15;
       if (use > 0) mbar_wait(&empty[s], (use - 1) & 1);
-      if (elect_one()) mbar_expect_tx(&full[s], rows_load * 128);
+      const int bytes = load_tile(w, mp, &full[s], ring + s * kTileBytes, half * 64, base_row, rows_valid, rows_load);
+      if (elect_one()) mbar_expect_tx(&full[s], bytes);   // posted after the boxes: the pending arrival keeps the phase open
       __syncwarp();
-      load_tile<1>(w, mp, &full[s], ring + s * kTileBytes, half * 64, base_row, rows_valid, rows_load);
     }
   } else if (warp == 9) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
