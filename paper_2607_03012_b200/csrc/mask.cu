@@ -4,6 +4,7 @@
 // (DESIGN.md R-K3); each CTA scores kRowsPerCta query clusters per pass over mu^k: w_j = s^k_j exp(S_j - max_j S_j); sort by (w desc, j asc) with an in-smem
 // bitonic network; inclusive scan; k = first position with cum >= top_p * Z; keep at least kmin.
 #include "common.cuh"
+#include <cstdlib>
 
 namespace {
 
@@ -127,6 +128,139 @@ __global__ void __launch_bounds__(kMaskThreads) hva_mask_kernel(int Nq, int Nk, 
   }
 }
 
+// ---- warp-per-row variant (Nk <= 1024): 8 query clusters per CTA.  The scores of the 8 rows are computed by the block
+// (thread = key cluster, every mu^k element read once for 8 fp64 dot products); then warp w owns row w: each lane holds E
+// of the row's P = 32 E (weight, j) pairs in registers (position = lane E + i) and the bitonic network runs without shared
+// memory or block barriers: distances < E are register-to-register inside a lane, distances >= E are lane-to-lane shuffles.
+template <int E>
+struct WarpSort {
+  double w[E];
+  int j[E];
+  __device__ __forceinline__ void cex(int a, int b, bool up) {      // positions a < b inside the lane
+    const bool sw = up ? before(w[b], j[b], w[a], j[a]) : before(w[a], j[a], w[b], j[b]);
+    if (sw) { double tw = w[a]; w[a] = w[b]; w[b] = tw; int tj = j[a]; j[a] = j[b]; j[b] = tj; }
+  }
+  __device__ __forceinline__ void sort(int lane) {
+#pragma unroll
+    for (int k = 2; k <= 32 * E; k <<= 1) {
+#pragma unroll
+      for (int d = k >> 1; d > 0; d >>= 1) {
+        if (d >= E) {                                                 // partner lane, same register index
+          const int lm = d / E;
+          const bool up = ((lane * E) & k) == 0, lower = (lane & lm) == 0;
+          const bool keep_first = (lower == up);                      // this position keeps the pair's `before` element
+#pragma unroll
+          for (int i = 0; i < E; ++i) {
+            const double ow = __shfl_xor_sync(0xffffffffu, w[i], lm);
+            const int oj = __shfl_xor_sync(0xffffffffu, j[i], lm);
+            const bool mine_first = before(w[i], j[i], ow, oj);
+            if (mine_first != keep_first) { w[i] = ow; j[i] = oj; }
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < E; ++i) {
+            if ((i & d) == 0) {
+              const bool up = k < E ? ((i & k) == 0) : ((((lane * E) | i) & k) == 0);
+              cex(i, i | d, up);
+            }
+          }
+        }
+      }
+    }
+  }
+};
+
+constexpr int kWarpRows = 8;
+
+template <int D, int E>
+__global__ void __launch_bounds__(256, 2) hva_mask_warp_kernel(int Nq, int Nk, const float* __restrict__ mu_q,
+                                                            const float* __restrict__ mu_k, const int* __restrict__ sizes_k,
+                                                            double scale, double top_p, int kmin, uint8_t* __restrict__ mask) {
+  constexpr int P = 32 * E;
+  const int i0 = blockIdx.x * kWarpRows, bh = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* s_q = reinterpret_cast<double*>(smem_raw);         // [kWarpRows][D]
+  double* s_sc = s_q + kWarpRows * D;                        // [kWarpRows][P] scores S_ij
+  const int nrows = min(kWarpRows, Nq - i0);
+  for (int e = tid; e < kWarpRows * D; e += 256) {
+    const int r = e / D;
+    s_q[e] = r < nrows ? (double)mu_q[((size_t)bh * Nq + i0 + r) * D + (e % D)] : 0.0;
+  }
+  __syncthreads();
+  // S_ij = <mu^q_i, mu^k_j> * scale   (Eq. 2), fp64 accumulation in ascending feature order
+  for (int jj = tid; jj < Nk; jj += 256) {
+    const float4* kr = reinterpret_cast<const float4*>(mu_k + ((size_t)bh * Nk + jj) * D);
+    double a[kWarpRows];
+#pragma unroll
+    for (int r = 0; r < kWarpRows; ++r) a[r] = 0.0;
+#pragma unroll 2
+    for (int c = 0; c < D / 4; ++c) {
+      const float4 v = __ldg(kr + c);
+      const double x0 = v.x, x1 = v.y, x2 = v.z, x3 = v.w;
+#pragma unroll
+      for (int r = 0; r < kWarpRows; ++r) {
+        const double* q = s_q + r * D + 4 * c;
+        a[r] = fma(x0, q[0], a[r]); a[r] = fma(x1, q[1], a[r]); a[r] = fma(x2, q[2], a[r]); a[r] = fma(x3, q[3], a[r]);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < kWarpRows; ++r) s_sc[(size_t)r * P + jj] = a[r] * scale;
+  }
+  __syncthreads();
+  if (warp >= nrows) return;
+  uint8_t* mrow = mask + ((size_t)bh * Nq + i0 + warp) * Nk;
+  const double* sc = s_sc + (size_t)warp * P;
+  WarpSort<E> ws;
+  double smax = -1.0 / 0.0;
+#pragma unroll
+  for (int i = 0; i < E; ++i) {                              // initial placement is arbitrary: key j = 32 i + lane (conflict-free)
+    const int jj = 32 * i + lane;
+    ws.j[i] = jj;
+    ws.w[i] = jj < Nk ? sc[jj] : -1.0 / 0.0;
+    smax = fmax(smax, ws.w[i]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+#pragma unroll
+  for (int i = 0; i < E; ++i)                                // w_j = s^k_j exp(S_j - max); pads (-1) sort last
+    ws.w[i] = ws.j[i] < Nk ? (double)sizes_k[(size_t)bh * Nk + ws.j[i]] * exp(ws.w[i] - smax) : -1.0;
+  ws.sort(lane);
+  // inclusive scan of the sorted weights: sequential inside a lane (positions lane E .. lane E + E - 1), shuffle scan across lanes
+  double run = 0.0;
+#pragma unroll
+  for (int i = 0; i < E; ++i) run += ws.w[i] > 0.0 ? ws.w[i] : 0.0;
+  double incl = run;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const double y = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += y;
+  }
+  const double Z = __shfl_sync(0xffffffffu, incl, 31), thr = top_p * Z;
+  double a = incl - run;
+  int first = Nk;                                            // smallest k with cum_k >= p Z   (Eq. 3)
+#pragma unroll
+  for (int i = 0; i < E; ++i) {
+    a += ws.w[i] > 0.0 ? ws.w[i] : 0.0;
+    if (a >= thr && first == Nk && lane * E + i < Nk) first = lane * E + i + 1;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) first = min(first, __shfl_xor_sync(0xffffffffu, first, o));
+  const int kcut = first < kmin ? kmin : first;
+#pragma unroll
+  for (int i = 0; i < E; ++i)
+    if (ws.j[i] < Nk) mrow[ws.j[i]] = (lane * E + i < kcut) ? 1 : 0;
+}
+
+template <int D, int E>
+int launch_mask_warp(int BH, int Nq, int Nk, const float* mu_q, const float* mu_k, const int* sizes_k, double scale, double top_p,
+                     int kmin, uint8_t* mask, cudaStream_t st) {
+  const size_t smem = (size_t)kWarpRows * D * 8 + (size_t)kWarpRows * 32 * E * 8;
+  if (cudaFuncSetAttribute(hva_mask_warp_kernel<D, E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return HVA_ECUDA;
+  hva_mask_warp_kernel<D, E><<<dim3((Nq + kWarpRows - 1) / kWarpRows, BH), 256, smem, st>>>(Nq, Nk, mu_q, mu_k, sizes_k, scale, top_p, kmin, mask);
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
+}
+
 }  // namespace
 
 extern "C" int hva_build_mask(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, const float* mu_q, const float* mu_k,
@@ -142,6 +276,18 @@ extern "C" int hva_build_mask(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, con
   int kmin = (int)ceil((double)min_kc * (double)Nk);
   size_t smem = (size_t)P * 12 + (size_t)kRowsPerCta * Nk * 8 + (size_t)kRowsPerCta * D * 8 + kMaskThreads * 8 + 16;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const char* force = getenv("HVA_MASK_BLOCKSORT");
+  if (top_p < 1.f && Nk <= 1024 && !(force && force[0] == '1')) {   // warp-per-row register sort
+#define HVA_MASK_WARP(DD)                                                                                                             \
+    do {                                                                                                                              \
+      if (Nk <= 256) return launch_mask_warp<DD, 8>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st);  \
+      if (Nk <= 512) return launch_mask_warp<DD, 16>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st); \
+      return launch_mask_warp<DD, 32>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st);                \
+    } while (0)
+    if (D == 64) HVA_MASK_WARP(64);
+    HVA_MASK_WARP(128);
+#undef HVA_MASK_WARP
+  }
   dim3 grid((Nq + kRowsPerCta - 1) / kRowsPerCta, BH);
   if (smem > 48 * 1024) {
     cudaFuncSetAttribute(hva_mask_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
