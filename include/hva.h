@@ -181,7 +181,10 @@ int hva_forward(const hva_shape* s, const hva_config* c, const void* Q, const vo
                 void* ws, size_t ws_bytes, void* stream);
 
 /* Same as hva_forward with HOST Q,K,V,O (pinned or pageable); allocates nothing: `dev_qkvo` is a
- * caller-owned DEVICE staging buffer of 4*B*heads*n*D elements.  Synchronises the stream. */
+ * caller-owned DEVICE staging buffer of 4*B*heads*n*D elements.  Heads are independent, so with B = 1, >= 8 heads and no
+ * hybrid state the call runs in 4 chunks of heads: the copies of the neighbouring chunks (two library-owned copy streams,
+ * both PCIe directions; pinned host buffers needed for the overlap) run under the kernels of the current one.
+ * Synchronises the stream. */
 int hva_forward_host(const hva_shape* s, const hva_config* c, const void* hQ, const void* hK,
                      const void* hV, void* hO, int32_t step_kind, void* state, void* dev_qkvo,
                      void* ws, size_t ws_bytes, void* stream);

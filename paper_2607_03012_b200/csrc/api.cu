@@ -110,8 +110,9 @@ extern "C" int hva_sparse_attention(const hva_shape* s, const hva_config* c, con
   return hva_attention_simt_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st, c->tile_q);
 }
 
-extern "C" int hva_forward(const hva_shape* s, const hva_config* c, const void* Q, const void* K, const void* V, void* O,
-                           int32_t step_kind, void* state, hva_stats* stats_out, void* ws, size_t ws_bytes, void* stream) {
+namespace {
+int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const void* K, const void* V, void* O, int32_t step_kind,
+                 void* state, hva_stats* stats_out, void* ws, size_t ws_bytes, void* stream, int bh0) {
   if (!valid_shape(s) || !valid_config(c) || !Q || !K || !V || !O || !ws) return HVA_EINVAL;
   if (step_kind != HVA_ANCHOR && step_kind != HVA_INTERMEDIATE && step_kind != HVA_DENSE) return HVA_EINVAL;
   if (step_kind == HVA_INTERMEDIATE && (!state || c->subset_frac <= 0.f)) return HVA_EINVAL;
@@ -162,7 +163,7 @@ extern "C" int hva_forward(const hva_shape* s, const hva_config* c, const void* 
   int32_t* n_groups = (int32_t*)(w + F.n_groups);
   HVA_TRY(hva_build_mask(BH, F.Nq, F.Nk, s->D, (float*)(sb + F.mu[0]), (float*)(sb + F.mu[1]), (int32_t*)(sb + F.sizes[1]),
                          scale, c->top_p, c->min_kc, mask, w + F.scratch, F.scratch_bytes, stream));
-  HVA_TRY(hva_merge(BH, F.Nq, F.Nk, (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), mask, c->tile_q, c->tile_k,
+  HVA_TRY(hva_merge_offset(bh0, BH, F.Nq, F.Nk, (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), mask, c->tile_q, c->tile_k,
                     c->merge_rounds, c->max_q_tiles, c->seed, group_of, n_groups, gmask, w + F.scratch, F.scratch_bytes, stream));
   HVA_TRY(hva_build_plan(BH, n, F.Nq, F.Nk, (int32_t*)(sb + F.assign[0]), (int32_t*)(sb + F.assign[1]),
                          (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), group_of, n_groups, gmask, c->tile_q,
@@ -177,18 +178,76 @@ extern "C" int hva_forward(const hva_shape* s, const hva_config* c, const void* 
   return HVA_OK;
 }
 
+}  // namespace
+
+extern "C" int hva_forward(const hva_shape* s, const hva_config* c, const void* Q, const void* K, const void* V, void* O,
+                           int32_t step_kind, void* state, hva_stats* stats_out, void* ws, size_t ws_bytes, void* stream) {
+  return forward_impl(s, c, Q, K, V, O, step_kind, state, stats_out, ws, ws_bytes, stream, 0);
+}
+
+namespace {
+// copy streams / events of hva_forward_host, created once per process (no device memory is allocated)
+struct HostPipe {
+  cudaStream_t h2d = nullptr, d2h = nullptr;
+  cudaEvent_t in_done[8] = {}, out_ready[8] = {};
+  bool ok = false;
+  HostPipe() {
+    ok = cudaStreamCreateWithFlags(&h2d, cudaStreamNonBlocking) == cudaSuccess &&
+         cudaStreamCreateWithFlags(&d2h, cudaStreamNonBlocking) == cudaSuccess;
+    for (int i = 0; i < 8 && ok; ++i)
+      ok = cudaEventCreateWithFlags(&in_done[i], cudaEventDisableTiming) == cudaSuccess &&
+           cudaEventCreateWithFlags(&out_ready[i], cudaEventDisableTiming) == cudaSuccess;
+  }
+};
+}  // namespace
+
+// Heads are independent instances of the whole pipeline, so the host variant runs the call in chunks of heads: the
+// host-to-device copy of chunk i+1 and the device-to-host copy of chunk i-1 (two copy streams, both PCIe directions)
+// overlap the kernels of chunk i on the caller's stream.  With a hybrid state buffer (per-(b,h) cache) or B > 1 the
+// call is not chunked.
 extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const void* hQ, const void* hK, const void* hV,
                                 void* hO, int32_t step_kind, void* state, void* dev_qkvo, void* ws, size_t ws_bytes,
                                 void* stream) {
   if (!valid_shape(s) || !hQ || !hK || !hV || !hO || !dev_qkvo) return HVA_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  const size_t bytes = (size_t)s->B * s->heads * s->T * s->H * s->W * s->D * (s->dtype == HVA_F32 ? 4 : 2);
+  const size_t es = s->dtype == HVA_F32 ? 4 : 2;
+  const size_t head_bytes = (size_t)s->T * s->H * s->W * s->D * es;
+  const size_t bytes = (size_t)s->B * s->heads * head_bytes;
   char* d = reinterpret_cast<char*>(dev_qkvo);
-  if (cudaMemcpyAsync(d, hQ, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
-  if (cudaMemcpyAsync(d + bytes, hK, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
-  if (cudaMemcpyAsync(d + 2 * bytes, hV, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
-  HVA_TRY(hva_forward(s, c, d, d + bytes, d + 2 * bytes, d + 3 * bytes, step_kind, state, nullptr, ws, ws_bytes, stream));
-  if (cudaMemcpyAsync(hO, d + 3 * bytes, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return HVA_ECUDA;
-  if (cudaStreamSynchronize(st) != cudaSuccess) return HVA_ECUDA;
+  static HostPipe pipe;
+  int nchunk = 1;
+  if (pipe.ok && !state && s->B == 1 && s->heads >= 8) nchunk = 4;
+  if (nchunk == 1) {
+    if (cudaMemcpyAsync(d, hQ, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
+    if (cudaMemcpyAsync(d + bytes, hK, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
+    if (cudaMemcpyAsync(d + 2 * bytes, hV, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
+    HVA_TRY(hva_forward(s, c, d, d + bytes, d + 2 * bytes, d + 3 * bytes, step_kind, state, nullptr, ws, ws_bytes, stream));
+    if (cudaMemcpyAsync(hO, d + 3 * bytes, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return HVA_ECUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return HVA_ECUDA;
+    return HVA_OK;
+  }
+  // the copy streams start after whatever the caller has queued on `st`
+  if (cudaEventRecord(pipe.out_ready[7], st) != cudaSuccess || cudaStreamWaitEvent(pipe.h2d, pipe.out_ready[7], 0) != cudaSuccess ||
+      cudaStreamWaitEvent(pipe.d2h, pipe.out_ready[7], 0) != cudaSuccess)
+    return HVA_ECUDA;
+  const char* src[3] = {(const char*)hQ, (const char*)hK, (const char*)hV};
+  int h0 = 0;
+  for (int i = 0; i < nchunk; ++i) {
+    const int h1 = (int)((long long)s->heads * (i + 1) / nchunk), nh = h1 - h0;
+    const size_t off = (size_t)h0 * head_bytes, cb = (size_t)nh * head_bytes;
+    for (int t = 0; t < 3; ++t)
+      if (cudaMemcpyAsync(d + t * bytes + off, src[t] + off, cb, cudaMemcpyHostToDevice, pipe.h2d) != cudaSuccess) return HVA_ECUDA;
+    if (cudaEventRecord(pipe.in_done[i], pipe.h2d) != cudaSuccess || cudaStreamWaitEvent(st, pipe.in_done[i], 0) != cudaSuccess)
+      return HVA_ECUDA;
+    hva_shape sc = *s;
+    sc.heads = nh;
+    HVA_TRY(forward_impl(&sc, c, d + off, d + bytes + off, d + 2 * bytes + off, d + 3 * bytes + off, step_kind, nullptr, nullptr, ws,
+                         ws_bytes, stream, h0));
+    if (cudaEventRecord(pipe.out_ready[i], st) != cudaSuccess || cudaStreamWaitEvent(pipe.d2h, pipe.out_ready[i], 0) != cudaSuccess)
+      return HVA_ECUDA;
+    if (cudaMemcpyAsync((char*)hO + off, d + 3 * bytes + off, cb, cudaMemcpyDeviceToHost, pipe.d2h) != cudaSuccess) return HVA_ECUDA;
+    h0 = h1;
+  }
+  if (cudaStreamSynchronize(pipe.d2h) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return HVA_ECUDA;
   return HVA_OK;
 }

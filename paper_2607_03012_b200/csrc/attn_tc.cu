@@ -284,6 +284,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     const uint32_t s_addr = tmem + lane_base + kColS + b * 128, p_addr = tmem + lane_base + kColP + b * 64;
     const float sl2 = p.scale_log2;
     const float2 sl2x2 = make_float2(sl2, sl2);
+    const bool row_ok = row0 + r < row1;
     float m_seen = -INFINITY;         // reference (log2 units) the partial sum l2 is relative to: P = 2^(s*scale*log2e - m_ref)
     float2 l2 = make_float2(0.f, 0.f);
     uint32_t v0[32], v1[32], v2[32], v3[32];
@@ -333,7 +334,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
       AMARK(3);
       if (m_ref != m_seen) { const float f0 = ex2(m_seen - m_ref); l2.x *= f0; l2.y *= f0; m_seen = m_ref; }   // m_seen = -inf: l2 = 0
       // the reference only moves when a score exceeds it by > 2^8 (lazy rescale); then O (complete up to PV_{j-1}) is rescaled
-      if (__any_sync(0xffffffffu, m_c - m_ref > kRescaleThreshold)) {
+      // (rows past the end of the group -- the Q tile over-reads its neighbours -- do not vote: they are never stored, and the
+      // bits of the valid rows must not depend on them)
+      if (__any_sync(0xffffffffu, row_ok && m_c - m_ref > kRescaleThreshold)) {
         const float m_new = fmaxf(m_ref, m_c);
         const float f = (m_new == m_ref) ? 1.f : ex2(m_ref - m_new);
         l2.x *= f; l2.y *= f;

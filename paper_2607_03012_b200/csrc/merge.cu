@@ -26,6 +26,7 @@ struct MergeParams {
   int Nq, Nk, Wd;
   const int* sizes_q; const int* sizes_k; const uint8_t* mask;
   int tile_q, tile_k, rounds, max_q_tiles; uint32_t seed;
+  int bh0;   // index of this call's first (batch, head) in the whole problem: the bipartition hash is keyed by the global bh
   int* group_of; int* n_groups; uint8_t* group_mask;
   uint32_t* chi; int* sq; int* kap; int* alive; int* side; int* remap; unsigned long long* best;
 };
@@ -65,13 +66,13 @@ __global__ void __launch_bounds__(256) hva_merge_propose_kernel(MergeParams p, i
   const size_t e0 = (size_t)bh * Nq;
   for (int j = tid; j < Wd * 32; j += 256) s_sk[j] = j < p.Nk ? p.sizes_k[(size_t)bh * p.Nk + j] : 0;
   for (int g = tid; g < Nq; g += 256) {
-    bool isB = p.alive[e0 + g] && hva_side_hash(p.seed, (uint32_t)bh, (uint32_t)r, (uint32_t)g) == 0;
+    bool isB = p.alive[e0 + g] && hva_side_hash(p.seed, (uint32_t)(p.bh0 + bh), (uint32_t)r, (uint32_t)g) == 0;
     s_sq[g] = isB ? p.sq[e0 + g] : 0;
     s_kap[g] = p.kap[e0 + g];
   }
   __syncthreads();
   const int A = blockIdx.x * 8 + (tid >> 5);
-  if (A >= Nq || !p.alive[e0 + A] || hva_side_hash(p.seed, (uint32_t)bh, (uint32_t)r, (uint32_t)A) != 1) return;
+  if (A >= Nq || !p.alive[e0 + A] || hva_side_hash(p.seed, (uint32_t)(p.bh0 + bh), (uint32_t)r, (uint32_t)A) != 1) return;
   const int sA = p.sq[e0 + A], kA = p.kap[e0 + A], rA = cdiv(sA, p.tile_q), cA = rA * cdiv(kA, p.tile_k);
   const uint32_t a0 = lane < Wd ? ~chi[(size_t)A * Wd + lane] : 0u;
   const uint32_t a1 = lane + 32 < Wd ? ~chi[(size_t)A * Wd + lane + 32] : 0u;
@@ -171,7 +172,7 @@ size_t hva_merge_ws_bytes(int BH, int Nq, int Nk) {
   return hva_align((size_t)BH * Nq * Wd * 4) + 5 * hva_align((size_t)BH * Nq * 4) + hva_align((size_t)BH * Nq * 8);
 }
 
-extern "C" int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k,
+int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k,
                          const uint8_t* mask, int32_t tile_q, int32_t tile_k, int32_t rounds, int32_t max_q_tiles,
                          uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask, void* ws,
                          size_t ws_bytes, void* stream) {
@@ -182,7 +183,7 @@ extern "C" int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* size
   MergeParams p;
   p.Nq = Nq; p.Nk = Nk; p.Wd = (Nk + 31) / 32;
   p.sizes_q = sizes_q; p.sizes_k = sizes_k; p.mask = mask;
-  p.tile_q = tile_q; p.tile_k = tile_k; p.rounds = rounds; p.max_q_tiles = max_q_tiles; p.seed = seed;
+  p.tile_q = tile_q; p.tile_k = tile_k; p.rounds = rounds; p.max_q_tiles = max_q_tiles; p.seed = seed; p.bh0 = bh0;
   p.group_of = group_of_cluster; p.n_groups = n_groups; p.group_mask = group_mask;
   char* w = reinterpret_cast<char*>(ws);
   size_t a4 = hva_align((size_t)BH * Nq * 4);
@@ -209,4 +210,12 @@ extern "C" int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* size
   hva_merge_out_kernel<<<dim3(Nq, BH), 256, 0, st>>>(p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
+}
+
+extern "C" int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k,
+                         const uint8_t* mask, int32_t tile_q, int32_t tile_k, int32_t rounds, int32_t max_q_tiles,
+                         uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask, void* ws,
+                         size_t ws_bytes, void* stream) {
+  return hva_merge_offset(0, BH, Nq, Nk, sizes_q, sizes_k, mask, tile_q, tile_k, rounds, max_q_tiles, seed, group_of_cluster, n_groups,
+                          group_mask, ws, ws_bytes, stream);
 }

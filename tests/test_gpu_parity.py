@@ -346,6 +346,22 @@ def test_forward_c2_end_to_end():
     assert flips <= 8
 
 
+def test_forward_host_matches_device_call():
+    """hva_forward_host (HOST buffers; with >= 8 heads it runs in chunks of heads with the copies overlapped on two copy
+    streams) returns the bits of hva_forward on device tensors."""
+    b = _b()
+    for wl, heads in ((inputs.C2, list(range(8))), (inputs.C2, [0, 3, 5])):
+        Q, K, V = inputs.make_qkv(wl, heads)
+        shape = b.make_shape(wl, heads=len(heads))
+        fwd = b.Forward(shape, b.make_config(wl))
+        O_dev = fwd(Q.cuda(), K.cuda(), V.cuda()).cpu()
+        hQ, hK, hV = [t.contiguous().pin_memory() for t in (Q, K, V)]
+        hO = torch.empty_like(hQ).pin_memory()
+        dev4 = torch.empty((4,) + tuple(Q.shape), dtype=Q.dtype, device="cuda")
+        fwd.host(hQ, hK, hV, hO, dev4)
+        assert torch.equal(hO, O_dev)
+
+
 def test_forward_dense_step_is_full_attention():
     b = _b()
     for wl in (inputs.C1, inputs.C2):
