@@ -53,6 +53,12 @@ __device__ __noinline__ float direct_dist_probe(const unsigned char* sA, int hal
   return direct_dist(sA, half_bytes, r, mu);
 }
 
+#ifdef HVA_ASSIGN_TIMING
+#define CMARK(k) do { if (threadIdx.x == 0) { long long _t = clock64(); tacc[k] = (unsigned)(_t - tprev); tprev = _t; } } while (0)
+#else
+#define CMARK(k) do { } while (0)
+#endif
+
 // x / d for 0 <= x, x * d < 2^32 by one multiply-high (m = ceil(2^32 / d); d == 1 is passed as m = 0)
 __device__ __forceinline__ int fast_div(int x, uint32_t m) { return m ? (int)__umulhi((uint32_t)x, m) : x; }
 
@@ -67,6 +73,10 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
   const int ctok = g.kt * g.kh * g.kw, nwin = g.nwin, npad = p.npad;
   const int half_a = p.rows_a * 128, half_b = npad * 128;
+#ifdef HVA_ASSIGN_TIMING
+  unsigned tacc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  long long tprev = clock64();
+#endif
 
   // Shared memory (offsets from a 1024-byte aligned base, kept as shared-space pointers):
   //   sB  [hi | lo][2 halves][npad][128 B]  window centroids, K-major SW128; after MMA 1 the hi part is reused for
@@ -121,27 +131,29 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   tc_fence_before();
   __syncthreads();
+  CMARK(0);
   tc_fence_after();
   const uint32_t tmem = B->tmem_base;
 
-  if (tid == 0) {
+  if (warp == 0) {
+    // warp-uniform up to the elected lane: descriptors built once in uniform registers, a k-step only adds a constant to the
+    // start-address field (a lane-0-only loop spends ~100 clk per MMA on descriptor arithmetic and R2UR moves)
     mbar_wait(&B->full, 0);
     tc_fence_after();
     const uint32_t idesc = umma_idesc_bf16(128, (uint32_t)npad, 0, 0);
-    const uint32_t a_addr = smem_u32(sA), hi_addr = smem_u32(sBhi), lo_addr = smem_u32(sBlo);
+    const uint64_t da = umma_desc(smem_u32(sA), 16, 1024), dhi = umma_desc(smem_u32(sBhi), 16, 1024), dlo = umma_desc(smem_u32(sBlo), 16, 1024);
+    const uint32_t ha = (uint32_t)half_a >> 4, hb = (uint32_t)half_b >> 4;
+    if (elect_one()) {
 #pragma unroll
-    for (int ks = 0; ks < kD / 16; ++ks) {
-      const uint32_t oa = (ks >> 2) * half_a + (ks & 3) * 32, ob = (ks >> 2) * half_b + (ks & 3) * 32;
-      mma_ss(tmem, umma_desc(a_addr + oa, 16, 1024), umma_desc(hi_addr + ob, 16, 1024), idesc, ks > 0);
-    }
+      for (int ks = 0; ks < kD / 16; ++ks)
+        mma_ss(tmem, da + ((ks >> 2) * ha + (ks & 3) * 2), dhi + ((ks >> 2) * hb + (ks & 3) * 2), idesc, ks > 0);
 #pragma unroll
-    for (int ks = 0; ks < kD / 16; ++ks) {
-      const uint32_t oa = (ks >> 2) * half_a + (ks & 3) * 32, ob = (ks >> 2) * half_b + (ks & 3) * 32;
-      mma_ss(tmem, umma_desc(a_addr + oa, 16, 1024), umma_desc(lo_addr + ob, 16, 1024), idesc, 1);
+      for (int ks = 0; ks < kD / 16; ++ks)
+        mma_ss(tmem, da + ((ks >> 2) * ha + (ks & 3) * 2), dlo + ((ks >> 2) * hb + (ks & 3) * 2), idesc, 1);
+      tc_commit(&B->mma_done);
     }
-    tc_commit(&B->mma_done);
+    __syncwarp();
   }
-  __syncwarp();
 
   // ---- token geometry; an upper bound of |x|^2 and the filter margin while the MMAs run
   const int li = tid;
@@ -159,6 +171,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     c_max = fmaxf(fmaxf(c_max, fmaxf(c4.x, c4.y)), fmaxf(c4.z, c4.w));
   }
   mbar_wait(&B->full, 0);
+  CMARK(1);
   // |x|^2 only scales the margin: packed bf16 FMAs (4 x 2 accumulators of 16 non-negative terms each: relative
   // error < 16 * 2^-8), inflated by 1/8 so that it is an upper bound
   float xsq = 0.f;
@@ -183,7 +196,9 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   const float xm = sqrtf(xsq * c_max);
   const float margin = 2.f * (2.f * kEpsDot * xm + 6e-7f * (c_max + 2.f * xm));
 
+  CMARK(2);
   mbar_wait(&B->mma_done, 0);
+  CMARK(3);
   tc_fence_after();
   // the B tiles are dead: clear the one-hot tile that aliases the hi part (filled after the labels are known)
   for (int i = tid; i < (2 * half_b) / 16; i += kThreads) reinterpret_cast<uint4*>(sP)[i] = make_uint4(0, 0, 0, 0);
@@ -269,6 +284,8 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
       p.lowe[(size_t)bh * g.n + tok] = rho;
     }
   }
+  CMARK(5);
+#ifndef HVA_ASSIGN_TIMING
   if (p.probe) {   // debug: observed filter error against the exact direct form
     float worst = 0.f, xx = 0.f;
     if (valid) {
@@ -293,8 +310,10 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     if (xx > xsq) worst = 1.f;   // the packed-bf16 |x|^2 must be an upper bound
     atomicMax(reinterpret_cast<int*>(p.probe), __float_as_int(worst));
   }
+#endif
   tc_fence_before();
   __syncthreads();        // one-hot tile cleared, every score read
+  CMARK(6);
 
   // ---- one-hot tile P^T[slot, token] = 1 and the slot counts
   {
@@ -307,23 +326,31 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncthreads();
+  CMARK(7);
   tc_fence_after();
 
   // ---- MMA 2: z^T[dim, slot] = sum_token x[token, dim] P^T[slot, token]   (Alg. 2 line 20): A = the token tile read
   // MN-major (M = 128 feature dims), B = the one-hot tile, D overwrites the score columns; TMEM lane = feature dim
-  if (tid == 0) {
+  if (warp == 0) {
     const uint32_t idesc = umma_idesc_bf16(128, (uint32_t)npad, 1, 0);
-    const uint32_t p_addr = smem_u32(sP), x_addr = smem_u32(sA);
+    const uint64_t dx = umma_desc(smem_u32(sA), half_a, 1024), dp = umma_desc(smem_u32(sP), 16, 1024);
+    const uint32_t hb = (uint32_t)half_b >> 4;
     const int ksteps = p.rows_a >> 4;
-    for (int ks = 0; ks < ksteps; ++ks)
-      mma_ss(tmem, umma_desc(x_addr + ks * 2048, half_a, 1024), umma_desc(p_addr + (ks >> 2) * half_b + (ks & 3) * 32, 16, 1024),
-             idesc, ks > 0);
-    tc_commit(&B->sum_done);
+    if (elect_one()) {
+      if (ksteps == 8) {
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) mma_ss(tmem, dx + ks * (2048 >> 4), dp + ((ks >> 2) * hb + (ks & 3) * 2), idesc, ks > 0);
+      } else {
+        for (int ks = 0; ks < ksteps; ++ks) mma_ss(tmem, dx + ks * (2048 >> 4), dp + ((ks >> 2) * hb + (ks & 3) * 2), idesc, ks > 0);
+      }
+      tc_commit(&B->sum_done);
+    }
+    __syncwarp();
   }
-  __syncwarp();
   const size_t pbase = ((size_t)bh * g.Nc + cell) * nwin;
   for (int v = tid; v < nwin; v += kThreads) p.part_cnt[pbase + v] = s_cnt[v];
   mbar_wait(&B->sum_done, 0);
+  CMARK(8);
   tc_fence_after();
   // thread = feature dim: a warp stores 32 consecutive floats of a partial row (coalesced)
   float* prow = p.part + pbase * kD + tid;
@@ -336,6 +363,10 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   }
   tc_fence_before();
   __syncthreads();
+  CMARK(9);
+#ifdef HVA_ASSIGN_TIMING
+  if (threadIdx.x == 0 && p.probe) for (int k = 0; k < 10; ++k) atomicAdd(p.probe + 16 + k, (float)tacc[k]);
+#endif
   if (warp == 0) { tc_fence_after(); tmem_dealloc(tmem, p.tmem_cols); }
 }
 
