@@ -210,7 +210,7 @@ def main():
                       "l2": "inputs (2.2 GB) larger than L2", "parallelism": "head-sharded replicas, no collective"},
            "clocks": clocks,
            "e2e": {"value": e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
-           "gpu_launches": args.steps * (2 * (2 + 2 * wl.iters) + 1 + (3 + 2 * int(cfg.merge_rounds)) + 7 + 3 + 1)}
+           "gpu_launches": args.steps * (2 * (2 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 7 + 3 + 1)}
 
     # ---- per-stage times and rooflines (rank 0)
     if rank == 0 and not args.no_stages:

@@ -151,6 +151,9 @@ int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const 
               uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask,
               void* ws, size_t ws_bytes, void* stream);
 
+/* Scratch needed by one hva_merge call; 0 on invalid arguments. */
+size_t hva_merge_workspace_bytes(int32_t BH, int32_t Nq, int32_t Nk);
+
 /* S7: canonical permutations (Eq. 1, l.37; R-P1) and the attention work list.  perm_k sorts
  * tokens by (a^k, l); perm_q by (gid(a^q), a^q, l).  `plan` is an opaque device buffer of
  * hva_plan_describe().total bytes.  Labels need not be window-local (hybrid steps). */

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libhva.so")
 HVA_F32, HVA_BF16 = 0, 1
 HVA_ANCHOR, HVA_INTERMEDIATE, HVA_DENSE = 0, 1, 2
 
-EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes",
+EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes", "hva_merge_workspace_bytes",
            "hva_plan_describe", "hva_cluster", "hva_select_subset", "hva_cluster_update", "hva_build_mask", "hva_merge",
            "hva_build_plan", "hva_permute", "hva_unpermute", "hva_sparse_attention", "hva_forward", "hva_forward_host"]
 
@@ -60,6 +60,7 @@ def lib():
         L.hva_state_bytes.restype = C.c_size_t
         L.hva_cluster_workspace_bytes.restype = C.c_size_t
         L.hva_cluster_update_workspace_bytes.restype = C.c_size_t
+        L.hva_merge_workspace_bytes.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -183,7 +184,7 @@ def hva_merge(sizes_q, sizes_k, mask, tile_q, tile_k, rounds, seed=0, max_q_tile
     group_of = torch.empty((BH, Nq), dtype=torch.int32, device=dev)
     n_groups = torch.empty((BH,), dtype=torch.int32, device=dev)
     gmask = torch.empty((BH, Nq, Nk), dtype=torch.uint8, device=dev)
-    ws = _ws(BH * Nq * ((Nk + 31) // 32) * 4 + 6 * (BH * Nq * 8 + 256) + 4096, dev)
+    ws = _ws(lib().hva_merge_workspace_bytes(BH, Nq, Nk), dev)
     _check(lib().hva_merge(BH, Nq, Nk, _p(sizes_q), _p(sizes_k), _p(mask), int(tile_q), int(tile_k), int(rounds),
                            int(max_q_tiles), C.c_uint32(seed), _p(group_of), _p(n_groups), _p(gmask), _p(ws),
                            C.c_size_t(ws.numel()), _stream()))

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhva.so")
-SOURCES = ["api.cu", "cluster.cu", "cluster_tc.cu", "hybrid.cu", "hybrid_tc.cu", "mask.cu", "merge.cu", "plan.cu", "attn_simt.cu", "attn_tc.cu"]
+SOURCES = ["api.cu", "cluster.cu", "cluster_tc.cu", "hybrid.cu", "hybrid_tc.cu", "mask.cu", "merge.cu", "merge_tc.cu", "plan.cu", "attn_simt.cu", "attn_tc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 

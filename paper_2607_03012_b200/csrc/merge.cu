@@ -11,6 +11,7 @@
 //   3. per-B conflict resolution with a 64-bit atomicMin on (dC, gid(A)) (line 14; order-free),
 //   4. accepted pairs are applied in parallel (lines 15-16): gid = min, s^q = sum, chi = OR.
 #include "common.cuh"
+#include <cstdlib>
 
 namespace {
 
@@ -101,6 +102,36 @@ __global__ void __launch_bounds__(256) hva_merge_propose_kernel(MergeParams p, i
   }
 }
 
+// Alg. 1 lines 6-13 for round r with the pairwise overlaps I[A][B] precomputed on the tensor pipe (merge_tc.cu):
+// kappa(A u B) = kappa(A) + kappa(B) - I[A][B].  One warp per A in side 1, lanes over B (coalesced row of I); the warp's
+// best (dC, gid(B)) is the lexicographic minimum == first minimum in ascending gid(B) with strict '<' (line 13).
+__global__ void __launch_bounds__(256) hva_merge_propose_inter_kernel(MergeParams p, int r, const int* __restrict__ inter, int Nqp) {
+  const int bh = blockIdx.y, tid = threadIdx.x, lane = tid & 31, Nq = p.Nq;
+  const size_t e0 = (size_t)bh * Nq;
+  const int A = blockIdx.x * 8 + (tid >> 5);
+  if (A >= Nq || !p.alive[e0 + A] || hva_side_hash(p.seed, (uint32_t)(p.bh0 + bh), (uint32_t)r, (uint32_t)A) != 1) return;
+  const int sA = p.sq[e0 + A], kA = p.kap[e0 + A], rA = cdiv(sA, p.tile_q), cA = rA * cdiv(kA, p.tile_k);
+  const int* row = inter + ((size_t)bh * Nqp + A) * Nqp;
+  int best_dc = 0, best_B = 0x7fffffff;
+  for (int B = lane; B < Nq; B += 32) {
+    if (!p.alive[e0 + B] || hva_side_hash(p.seed, (uint32_t)(p.bh0 + bh), (uint32_t)r, (uint32_t)B) != 0) continue;
+    const int sB = p.sq[e0 + B], kB = p.kap[e0 + B], rB = cdiv(sB, p.tile_q), cB = rB * cdiv(kB, p.tile_k);
+    const int rU = cdiv(sA + sB, p.tile_q);
+    if (p.max_q_tiles > 0 && rU > p.max_q_tiles) continue;
+    if (rU >= rA + rB) continue;                                      // no row tile saved => dC >= 0 (R-M6)
+    const int dc = rU * cdiv(kA + kB - row[B], p.tile_k) - cA - cB;   // Eq. 10 in tile units
+    if (dc < best_dc) { best_dc = dc; best_B = B; }                   // ascending B per lane: strict '<' keeps the lower gid
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const int odc = __shfl_xor_sync(0xffffffffu, best_dc, o), oB = __shfl_xor_sync(0xffffffffu, best_B, o);
+    if (odc < best_dc || (odc == best_dc && oB < best_B)) { best_dc = odc; best_B = oB; }
+  }
+  if (lane == 0 && best_dc < 0) {
+    unsigned long long key = ((unsigned long long)(uint32_t)(best_dc + 0x40000000) << 32) | (uint32_t)A;
+    atomicMin(&p.best[e0 + best_B], key);                             // line 14: best A per B, ties -> lower gid(A)
+  }
+}
+
 // Alg. 1 lines 15-16: accepted pairs are disjoint, applied in parallel.  One CTA per (b, head); warp per pair.
 __global__ void __launch_bounds__(1024) hva_merge_apply_kernel(MergeParams p) {
   const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, Nq = p.Nq, Wd = p.Wd;
@@ -167,9 +198,25 @@ __global__ void __launch_bounds__(256) hva_merge_out_kernel(MergeParams p) {
 
 }  // namespace
 
+// tensor-pipe overlap matrix (merge_tc.cu)
+size_t hva_merge_inter_bytes(int BH, int Nq);
+int hva_merge_nterms_launch(int BH, int Nk, const int* sizes_k, int* nterms, cudaStream_t st);
+int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, cudaStream_t st);
+
+static bool merge_use_inter(int Nq) {
+  const char* force = getenv("HVA_MERGE_SIMT");
+  return Nq <= 2048 && !(force && force[0] == '1');
+}
+
 size_t hva_merge_ws_bytes(int BH, int Nq, int Nk) {
   size_t Wd = (Nk + 31) / 32;
-  return hva_align((size_t)BH * Nq * Wd * 4) + 5 * hva_align((size_t)BH * Nq * 4) + hva_align((size_t)BH * Nq * 8);
+  return hva_align((size_t)BH * Nq * Wd * 4) + 5 * hva_align((size_t)BH * Nq * 4) + hva_align((size_t)BH * Nq * 8) +
+         (Nq <= 2048 ? hva_merge_inter_bytes(BH, Nq) : 0);
+}
+
+extern "C" size_t hva_merge_workspace_bytes(int32_t BH, int32_t Nq, int32_t Nk) {
+  if (BH < 1 || Nq < 1 || Nk < 1) return 0;
+  return hva_merge_ws_bytes(BH, Nq, Nk);
 }
 
 int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k,
@@ -193,14 +240,24 @@ int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int3
   p.alive = reinterpret_cast<int*>(w); w += a4;
   p.side = reinterpret_cast<int*>(w); w += a4;
   p.remap = reinterpret_cast<int*>(w); w += a4;
-  p.best = reinterpret_cast<unsigned long long*>(w);
+  p.best = reinterpret_cast<unsigned long long*>(w); w += hva_align((size_t)BH * Nq * 8);
+  const bool use_inter = rounds > 0 && merge_use_inter(Nq);
+  const int Nqp = (Nq + 127) / 128 * 128;
+  int* inter = reinterpret_cast<int*>(w);
+  int* nterms = reinterpret_cast<int*>(w + hva_align((size_t)BH * Nqp * Nqp * 4));
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const dim3 gw((Nq + 7) / 8, BH);
   hva_merge_init_kernel<<<gw, 256, 0, st>>>(p);
   HVA_CHECK_LAUNCH();
   const size_t smem = ((size_t)p.Wd * 32 + 2 * (size_t)Nq) * sizeof(int);
+  if (use_inter) HVA_TRY(hva_merge_nterms_launch(BH, Nk, sizes_k, nterms, st));
   for (int r = 1; r <= rounds; ++r) {
-    hva_merge_propose_kernel<<<gw, 256, smem, st>>>(p, r);
+    if (use_inter) {
+      HVA_TRY(hva_merge_inter_launch(BH, Nq, Nk, p.chi, sizes_k, nterms, inter, st));
+      hva_merge_propose_inter_kernel<<<gw, 256, 0, st>>>(p, r, inter, Nqp);
+    } else {
+      hva_merge_propose_kernel<<<gw, 256, smem, st>>>(p, r);
+    }
     HVA_CHECK_LAUNCH();
     hva_merge_apply_kernel<<<BH, 1024, 0, st>>>(p);
     HVA_CHECK_LAUNCH();
