@@ -24,6 +24,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 from paper_2607_03012_b200 import inputs, sharding  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one hva_attn_tc_kernel launch at C4 (top-p 0.9, merging on), from the `ncu --set full`
+# capture summarised in profiles/r1c_ncu_full.md (11.64 GB + 0.78 GB); algorithmic minimum 2.9 GB (Q', K', V' once + O)
+ATTN_DRAM_BYTES_C4 = 12.41e9
+
 METRIC = "sparse-attn ms/call + clustering ms/step at 118,800-token HunyuanVideo shape"
 
 
@@ -370,7 +374,8 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
         "stages_ms": {k: round(v, 4) for k, v in st.items()},
         "roofline": {"bound": "tensor", "kernel": "hva_attn_tc_kernel", "achieved": ach, "peak": pk["tf_sust"], "unit": "TFLOP/s",
                      "frac": ach / pk["tf_sust"], "frac_of_burst": ach / pk["tf_burst"], "peak_source": pk["src"] + " (sustained)",
-                     "traffic": None, "executed_tflop": exec_flop / 1e12, "dense_equiv_tflops": dense_flop / t_att / 1e12},
+                     "traffic": ATTN_DRAM_BYTES_C4 if (wl.name == "C4-hunyuan" and abs(float(cfg.top_p) - 0.9) < 1e-6 and int(cfg.merge_rounds) == 3) else None,
+                     "executed_tflop": exec_flop / 1e12, "dense_equiv_tflops": dense_flop / t_att / 1e12},
         "roofline_cluster": {"bound": "hbm", "kernel": "hva_assign_tc_kernel+hva_finalize_kernel", "achieved": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9,
                              "peak": pk["hbm"], "unit": "GB/s", "frac": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9 / pk["hbm"],
                              "algorithmic_bytes": cl_bytes},
