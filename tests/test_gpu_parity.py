@@ -165,6 +165,41 @@ def test_cluster_tensor_pipe_equals_direct_form(wl, monkeypatch):
                 assert 0 < float(probe.item()) < 2.0 ** -14 / 8, float(probe.item())
 
 
+def test_tensor_pipe_exact_ties_take_the_first_minimum():
+    """Degenerate inputs for the filter-and-refine kernels: few distinct token values, so most centroids coincide and every
+    candidate of a token ties EXACTLY.  All of them are contenders (the many-contender path of both kernels: in-window exact
+    refine, and the warp-cooperative exact scan of the subset step); the result must be the first minimum in ascending
+    centroid id, as in the oracle (R-C1)."""
+    b = _b()
+    wl = dataclasses.replace(inputs.C2, name="ties", heads=2, T=6, H=8, W=16, cell=(2, 4, 4), seed=21)
+    rng = np.random.default_rng(21)
+    vals = torch.from_numpy(rng.standard_normal((3, wl.D)).astype(np.float32)).to(torch.bfloat16)      # three distinct rows
+    pick = torch.from_numpy(rng.integers(0, 3, size=(1, 2, wl.n)))
+    X = vals[pick].contiguous()                                                                         # [1, 2, n, D]
+    Xd = X.cuda()
+    shape = b.make_shape(wl, heads=2)
+    g = b.hva_cluster(shape, wl.cell, wl.win, 2, Xd)
+    torch.cuda.synchronize()
+    Nc = wl.n_clusters
+    for hi in range(2):
+        x64 = inputs.to_f64(X[0, hi])
+        orc = oracle.local_window_kmeans(x64, _lat(wl), wl.cell, wl.win, 2)
+        assert np.array_equal(g["assign"][hi].cpu().numpy(), orc["assign"])
+        assert np.array_equal(g["sizes"][hi].cpu().numpy(), orc["sizes"])
+    # subset step: every token, all N_c candidates, centroids that coincide exactly
+    sub = torch.arange(wl.n, dtype=torch.int32).repeat(2, 1).cuda()
+    mu32 = g["mu"].clone(); mu32[:, 1::2] = mu32[:, 0::2][:, : mu32[:, 1::2].shape[1]]                  # duplicate centroids pairwise
+    assign, mu, sums, sizes = g["assign"].clone(), mu32.clone(), g["sums"].clone(), g["sizes"].clone()
+    b.hva_cluster_update(shape, Xd, sub, assign, mu, sums, sizes, 1)
+    torch.cuda.synchronize()
+    for hi in range(2):
+        x64 = inputs.to_f64(X[0, hi])
+        a, *_ = oracle.subset_update(x64, g["assign"][hi].cpu().numpy().astype(np.int64), mu32[hi].cpu().numpy().astype(np.float64),
+                                     g["sums"][hi].cpu().numpy().astype(np.float64), g["sizes"][hi].cpu().numpy().astype(np.int64),
+                                     np.arange(wl.n), refresh_all=True)
+        assert np.array_equal(assign[hi].cpu().numpy(), a)
+
+
 def _oracle_stage_inputs(wl, heads, f64):
     """Oracle clustering of Q and K per head (the 'teacher' for the downstream stages)."""
     out = []
