@@ -48,6 +48,18 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
   int* run_cnt = P.run_cnt + (size_t)bh * Nq;
   int* qb = qbase + (size_t)bh * Nq;
   __shared__ int s_ng;
+  // the serial parts below are chains of dependent loads: run them on shared-memory copies (global latency made this kernel
+  // 0.67 ms at C4)
+  extern __shared__ int s_stage[];
+  int* s_sq = s_stage;            // [Nq]
+  int* s_gof = s_sq + Nq;         // [Nq]
+  int* s_sk = s_gof + Nq;         // [Nk]
+  int* s_goff = s_sk + Nk;        // [Nq + 1]
+  int* s_kap = s_goff + Nq + 1;   // [Nq]
+  for (int u = tid; u < Nq; u += blockDim.x) { s_sq[u] = sizes_q[(size_t)bh * Nq + u]; s_gof[u] = group_of[(size_t)bh * Nq + u]; }
+  for (int j = tid; j < Nk; j += blockDim.x) s_sk[j] = sizes_k[(size_t)bh * Nk + j];
+  __syncthreads();
+  sq = s_sq; sk = s_sk; gof = s_gof;
   // Q' row offset of query cluster u: clusters ordered by (gid(u), u)   (R-P1)
   for (int u = tid; u < Nq; u += blockDim.x) {
     int gu = gof[u], off = 0;
@@ -73,27 +85,47 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
   }
   __syncthreads();
   const int ng = s_ng;
-  for (int k = tid; k < ng; k += blockDim.x) goff[k] = qb[gid[k]];   // leader = first cluster of its group
-  if (tid == 0) goff[ng] = n;
+  for (int k = tid; k < ng; k += blockDim.x) { const int o = qb[gid[k]]; goff[k] = o; s_goff[k] = o; }   // leader = first cluster of its group
+  if (tid == 0) { goff[ng] = n; s_goff[ng] = n; }
   // packed key runs of each group: maximal runs of consecutive selected key clusters (l.109)
   const uint8_t* gm = group_mask + (size_t)bh * Nq * Nk;
   for (int k = warp; k < ng; k += blockDim.x / 32) {
     uint16_t* r16 = reinterpret_cast<uint16_t*>(P.runs + ((size_t)bh * Nq + k) * P.run_stride);
+    const uint8_t* grow = gm + (size_t)k * Nk;
     int nstart = 0, nend = 0, kap = 0;
-    for (int j0 = 0; j0 < Nk; j0 += 32) {
-      int j = j0 + lane;
-      int bit = (j < Nk) ? gm[(size_t)k * Nk + j] : 0;
-      int prev = (j > 0 && j < Nk) ? gm[(size_t)k * Nk + j - 1] : 0;
-      int next = (j + 1 < Nk) ? gm[(size_t)k * Nk + j + 1] : 0;
-      unsigned ms = __ballot_sync(0xffffffffu, bit && !prev), me = __ballot_sync(0xffffffffu, bit && !next);
-      unsigned lt = (1u << lane) - 1;
-      if (bit && !prev) r16[2 * (nstart + __popc(ms & lt))] = (uint16_t)j;
-      if (bit && !next) r16[2 * (nend + __popc(me & lt)) + 1] = (uint16_t)j;
-      nstart += __popc(ms); nend += __popc(me);
-      kap += bit ? sk[j] : 0;
+    unsigned carry = 0;                                   // last key of the previous 1024-key block selected?
+    for (int jb = 0; jb < Nk; jb += 1024) {
+      // pack up to 1024 mask bytes into 32 ballot words (independent loads, one latency), lane l then owns word l
+      unsigned mine = 0;
+#pragma unroll 8
+      for (int w = 0; w < 32; ++w) {
+        const int j = jb + 32 * w + lane;
+        const int bit = (j < Nk) ? grow[j] : 0;
+        const unsigned word = __ballot_sync(0xffffffffu, bit);
+        kap += bit ? sk[j] : 0;
+        if (w == lane) mine = word;
+      }
+      const unsigned prev_w = __shfl_up_sync(0xffffffffu, mine, 1), next_w = __shfl_down_sync(0xffffffffu, mine, 1);
+      const unsigned prev_bit = lane == 0 ? carry : (prev_w >> 31);
+      unsigned next_bit = lane == 31 ? 0u : (next_w & 1u);
+      if (lane == 31 && jb + 1024 < Nk) next_bit = grow[jb + 1024] ? 1u : 0u;
+      unsigned starts = mine & ~((mine << 1) | prev_bit), ends = mine & ~((mine >> 1) | (next_bit << 31));
+      // exclusive prefix of the run counts over the lanes
+      int cs = __popc(starts), ce = __popc(ends), ps = cs, pe = ce;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int ys = __shfl_up_sync(0xffffffffu, ps, o), ye = __shfl_up_sync(0xffffffffu, pe, o);
+        if (lane >= o) { ps += ys; pe += ye; }
+      }
+      const int tot_s = __shfl_sync(0xffffffffu, ps, 31), tot_e = __shfl_sync(0xffffffffu, pe, 31);
+      int os = nstart + ps - cs, oe = nend + pe - ce;
+      while (starts) { const int bpos = __ffs(starts) - 1; starts &= starts - 1; r16[2 * os++] = (uint16_t)(jb + 32 * lane + bpos); }
+      while (ends) { const int bpos = __ffs(ends) - 1; ends &= ends - 1; r16[2 * oe++ + 1] = (uint16_t)(jb + 32 * lane + bpos); }
+      nstart += tot_s; nend += tot_e;
+      carry = __shfl_sync(0xffffffffu, mine, 31) >> 31;
     }
     for (int o = 16; o > 0; o >>= 1) kap += __shfl_xor_sync(0xffffffffu, kap, o);
-    if (lane == 0) { run_cnt[k] = nstart; kappa[k] = kap; }
+    if (lane == 0) { run_cnt[k] = nstart; kappa[k] = kap; s_kap[k] = kap; }
   }
   __syncthreads();
   if (tid == 0) {  // work list (group, q-tile) in group order + statistics (Eq. 7-8; Fig. 5c terms)
@@ -101,7 +133,7 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
     hva_stats s = {};
     int wc = 0;
     for (int k = 0; k < ng; ++k) {
-      int rows = goff[k + 1] - goff[k], kp = kappa[k];
+      int rows = s_goff[k + 1] - s_goff[k], kp = s_kap[k];
       int rt = (rows + tile_q - 1) / tile_q, kt = (kp + tile_k - 1) / tile_k;
       for (int t = 0; t < rt; ++t) work[wc++] = k | (t << 16);
       s.q_rows_valid += rows; s.q_rows_padded += (int64_t)rt * tile_q;
@@ -255,7 +287,10 @@ extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, con
   const int ntile = (n + kTile - 1) / kTile, Ncmax = Nq > Nk ? Nq : Nk;
   int* hist = reinterpret_cast<int*>(ws);
   int* qbase = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + hva_align((size_t)BH * ntile * Ncmax * 4));
-  hva_plan_groups_kernel<<<BH, 1024, 0, st>>>(n, Nq, Nk, sizes_q, sizes_k, group_of_cluster, group_mask, tile_q, tile_k,
+  const size_t gsmem = sizeof(int) * (4 * (size_t)Nq + Nk + 1);
+  if (gsmem > 48 * 1024 && cudaFuncSetAttribute(hva_plan_groups_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem) != cudaSuccess)
+    return HVA_EUNSUPPORTED;
+  hva_plan_groups_kernel<<<BH, 1024, gsmem, st>>>(n, Nq, Nk, sizes_q, sizes_k, group_of_cluster, group_mask, tile_q, tile_k,
                                               P, qbase);
   HVA_CHECK_LAUNCH();
   dim3 gsort((ntile + kSortWarps - 1) / kSortWarps, BH);
