@@ -496,3 +496,15 @@ def test_c4_full_size_sampled():
         assert s["q_rows_valid"] == wl.n and 0 < s["n_groups"] <= wl.n_clusters
         assert s["pairs_valid"] <= wl.n * wl.n and s["q_rows_padded"] >= wl.n
     assert torch.isfinite(O.float()).all()
+
+
+def test_c3_full_size_sampled():
+    """C3 (Wan2.1-14B shape, 40 heads x 75 600 tokens, 630 clusters): the same full-size check on a second lattice
+    (T = 21 gives 7 temporal cells, N_k = 630 exercises the 1024-wide register sort with 394 pad entries and the
+    5-block merge contraction)."""
+    wl = inputs.C3
+    fwd, dev, O, flips = _forward_vs_oracle(wl, list(range(wl.heads)), rows_per_head=32, check_heads=[17])
+    assert flips <= 20, flips
+    for s in fwd.stats_dicts():
+        assert s["q_rows_valid"] == wl.n and 0 < s["n_groups"] <= wl.n_clusters
+    assert torch.isfinite(O.float()).all()
