@@ -30,6 +30,11 @@ constexpr int kNumBoxes = 8;                   // box heights 1,2,4,...,128
 constexpr uint32_t kTmemCols = 512;            // S_0, S_1 (fp32 scores), O (fp32), P_0, P_1 (bf16 probabilities)
 constexpr uint32_t kColS = 0, kColO = 256, kColP = 384;   // S_b at kColS + 128 b, P_b at kColP + 64 b
 constexpr float kRescaleThreshold = 8.0f;      // log2 units
+// Share of the exponentials taken off MUFU (16/clk/SM = 1024 clk per 128x128 tile, the MMA time of a tile) by the software
+// exp2 below.  It paid while the softmax paced the kernel (1 pair in 4: 96 -> 92 ms); with two softmax sets and the
+// tensor pipe as the pace-maker under the power cap the extra FMA work only costs energy: 0 / 1 / 2 of 8 pairs =
+// 77.5 / 78.9 / 79.8 ms per call at C4.
+constexpr int kPolyPairs = 0;
 
 struct TcMaps {
   CUtensorMap q;
@@ -369,8 +374,8 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
         for (int i = 0; i < 16; ++i) {
           const float2 x = __ffma2_rn(make_float2(__uint_as_float(vv[2 * i]), __uint_as_float(vv[2 * i + 1])), sl2x2, nm);
           float2 e;
-          if ((i & 3) == 3) {
-            e = exp2_poly2(x);            // 1 pair in 4 on the FMA pipe: the MUFU rate (16/clk/SM) equals the MMA time of a tile
+          if (kPolyPairs > 0 && (i & 7) < kPolyPairs) {
+            e = exp2_poly2(x);            // software exponential on the FMA pipe for kPolyPairs of every 8 pairs
           } else {
             e.x = ex2(x.x); e.y = ex2(x.y);
           }
