@@ -508,3 +508,28 @@ def test_c3_full_size_sampled():
     for s in fwd.stats_dicts():
         assert s["q_rows_valid"] == wl.n and 0 < s["n_groups"] <= wl.n_clusters
     assert torch.isfinite(O.float()).all()
+
+
+def test_forward_different_q_and_k_grids_wide_windows_min_kc():
+    """Paper-setting structure (Table 2, App. A of SURVEY.md): different cell sizes for Q and K (N_q != N_k), (3,8,8)
+    windows clipped to the grid (32 and 48 candidates per token: several 32-column TMEM chunks in the assignment kernel),
+    min-kc > 0 -- end to end through hva_forward against the oracle's forward pass."""
+    b = _b()
+    wl = dataclasses.replace(inputs.C2, name="qk-grids", heads=2, T=8, H=16, W=16, seed=31)
+    cell_q, cell_k, win = (4, 4, 4), (2, 4, 4), (3, 8, 8)
+    Q, K, V = inputs.make_qkv(wl, [0, 1])
+    cfg = b.make_config(wl, min_kc=0.15)
+    i3 = type(cfg.cell_q)
+    cfg.cell_q, cfg.cell_k, cfg.win_q, cfg.win_k = i3(*cell_q), i3(*cell_k), i3(*win), i3(*win)
+    fwd = b.Forward(b.make_shape(wl, heads=2), cfg)
+    O = fwd(Q.cuda(), K.cuda(), V.cuda())
+    torch.cuda.synchronize()
+    scale32 = float(np.float32(1.0 / math.sqrt(wl.D)))
+    for hi in range(2):
+        f = [inputs.to_f64(t[0, hi]) for t in (Q, K, V)]
+        r = oracle.forward_head(f[0], f[1], f[2], _lat(wl), cell_q, win, cell_k, win, wl.iters, wl.tile, float(np.float32(wl.top_p)),
+                                wl.merge_rounds, seed=wl.seed, bh=hi, min_kc=float(np.float32(0.15)), scale=scale32)
+        assert fwd.stats_dicts()[hi]["n_groups"] == len(r["gids"])
+        got = O[0, hi].float().cpu().numpy().astype(np.float64)[r["rows"]]
+        assert np.abs(got - r["O"]).max() <= 2e-2
+        assert np.linalg.norm(got - r["O"]) / np.linalg.norm(r["O"]) <= 1e-2
