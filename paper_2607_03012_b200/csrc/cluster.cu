@@ -231,7 +231,7 @@ __device__ __forceinline__ void axis_cells(int u, int w, int K, int& lo, int& cn
 template <int D>
 __global__ void __launch_bounds__(D) hva_finalize_kernel(HvaGrid g, const float* __restrict__ part,
                                                          const int* __restrict__ part_cnt, float* __restrict__ mu,
-                                                         int* __restrict__ sizes, float* __restrict__ sums, MuSplit sp) {
+                                                         int* __restrict__ sizes, float* __restrict__ sums, MuSplit sp, int csplit) {
   const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
   const int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
   __shared__ unsigned s_idx[1024];     // at most nwin <= 1024 home cells have u in their window (checked by hva_cluster)
@@ -241,18 +241,19 @@ __global__ void __launch_bounds__(D) hva_finalize_kernel(HvaGrid g, const float*
     axis_cells(ut, g.wt, g.Kt, lt, nt);
     axis_cells(uh, g.wh, g.Kh, lh, nh);
     axis_cells(uw, g.ww, g.Kw, lw, nw);
-    const int total = nt * nh * nw;
+    const int total = nt * nh * nw * csplit;      // (home cell, t-tile of the cell) partials, ascending cell then tile
     int m = 0, n = 0;
     for (int e0 = 0; e0 < total; e0 += 32) {
       const int e = e0 + c;
       int k = 0;
       unsigned idx = 0;
       if (e < total) {
-        const int gt = lt + e / (nh * nw), gh = lh + (e / nw) % nh, gw = lw + e % nw;
+        const int ce = e / csplit, chunk = e - ce * csplit;
+        const int gt = lt + ce / (nh * nw), gh = lh + (ce / nw) % nh, gw = lw + ce % nw;
         const int cell = (gt * g.Kh + gh) * g.Kw + gw;
         const int slot = ((ut - hva_win_start(gt, g.wt, g.Kt)) * g.wh + (uh - hva_win_start(gh, g.wh, g.Kh))) * g.ww +
                          (uw - hva_win_start(gw, g.ww, g.Kw));
-        idx = (unsigned)(((size_t)bh * g.Nc + cell) * g.nwin + slot);
+        idx = (unsigned)((((size_t)bh * g.Nc + cell) * csplit + chunk) * g.nwin + slot);
         k = part_cnt[idx];
       }
       const unsigned bal = __ballot_sync(0xffffffffu, k > 0);
@@ -333,7 +334,7 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
       hva_assign_kernel<T, D><<<grid, kThreads, smem, st>>>(p);
       HVA_CHECK_LAUNCH();
     }
-    hva_finalize_kernel<D><<<grid, D, 0, st>>>(g, ws.part, ws.part_cnt, mu, sizes, last ? sums : nullptr, last ? none : sp);
+    hva_finalize_kernel<D><<<grid, D, 0, st>>>(g, ws.part, ws.part_cnt, mu, sizes, last ? sums : nullptr, last ? none : sp, tc ? atc.csplit : 1);
     HVA_CHECK_LAUNCH();
   }
   return HVA_OK;
@@ -342,7 +343,8 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
 }  // namespace
 
 size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D) {
-  return hva_align((size_t)BH * g.Nc * g.nwin * D * sizeof(float)) + hva_align((size_t)BH * g.Nc * g.nwin * sizeof(int)) +
+  const size_t cs = (size_t)hva_assign_tc_csplit(g);
+  return hva_align((size_t)BH * g.Nc * cs * g.nwin * D * sizeof(float)) + hva_align((size_t)BH * g.Nc * cs * g.nwin * sizeof(int)) +
          2 * hva_align((size_t)BH * g.Nc * D * sizeof(__nv_bfloat16)) + hva_align((size_t)BH * g.Nc * sizeof(float));
 }
 
@@ -373,13 +375,14 @@ extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int3
   if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
   HvaGrid g = hva_make_grid(s, cell, win);
   int BH = s->B * s->heads;
-  if (g.nwin > 1024 || (size_t)BH * g.Nc * g.nwin >= (1ull << 32)) return HVA_EUNSUPPORTED;
+  if ((size_t)g.nwin * hva_assign_tc_csplit(g) > 1024 || (size_t)BH * g.Nc * g.nwin * hva_assign_tc_csplit(g) >= (1ull << 32)) return HVA_EUNSUPPORTED;
   if (ws_bytes < hva_cluster_ws_bytes(g, BH, s->D)) return HVA_EWORKSPACE;
   ClusterWs cw;
   {
     char* w = reinterpret_cast<char*>(ws);
-    cw.part = reinterpret_cast<float*>(w); w += hva_align((size_t)BH * g.Nc * g.nwin * s->D * sizeof(float));
-    cw.part_cnt = reinterpret_cast<int*>(w); w += hva_align((size_t)BH * g.Nc * g.nwin * sizeof(int));
+    const size_t cs = (size_t)hva_assign_tc_csplit(g);
+    cw.part = reinterpret_cast<float*>(w); w += hva_align((size_t)BH * g.Nc * cs * g.nwin * s->D * sizeof(float));
+    cw.part_cnt = reinterpret_cast<int*>(w); w += hva_align((size_t)BH * g.Nc * cs * g.nwin * sizeof(int));
     cw.hi = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
     cw.lo = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
     cw.musq = reinterpret_cast<float*>(w);

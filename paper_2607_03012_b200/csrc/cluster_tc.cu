@@ -38,7 +38,8 @@ struct AssignTcParams {
   int* assign;         // [BH, n] or null
   float* lowe;         // [BH, n] or null
   int npad;            // window candidates padded to the MMA N granule (16)
-  int rows_a;          // cell tokens padded to the MMA K granule (16 rows)
+  int rows_a;          // tile tokens padded to the MMA K granule (16 rows)
+  int csplit, ct;      // a cell of more than 128 tokens is split along t into csplit tiles of ct time slices (one CTA each)
   uint32_t m_khw, m_kw, m_whw, m_ww;   // fast_div multipliers for k_h k_w, k_w, w_h w_w, w_w
   uint32_t tmem_cols;
   float* probe;        // debug: max |score_tc - score_exact| / (|x| max|mu|), or null
@@ -68,10 +69,12 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
                                                                  const __grid_constant__ CUtensorMap map_lo, AssignTcParams p) {
   const HvaGrid& g = p.g;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int uw = blockIdx.x, uh = blockIdx.y, bh = blockIdx.z / g.Kt, ut = blockIdx.z - bh * g.Kt;
+  const int uw = blockIdx.x, uh = blockIdx.y;
+  const int chunk = blockIdx.z % p.csplit, zz = blockIdx.z / p.csplit, bh = zz / g.Kt, ut = zz - bh * g.Kt;
+  const int dt0 = chunk * p.ct;                        // first time slice of this tile inside the cell
   const int cell = (ut * g.Kh + uh) * g.Kw + uw;
   const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
-  const int ctok = g.kt * g.kh * g.kw, nwin = g.nwin, npad = p.npad;
+  const int ctok = p.ct * g.kh * g.kw, nwin = g.nwin, npad = p.npad;   // token rows of this tile
   const int half_a = p.rows_a * 128, half_b = npad * 128;
 #ifdef HVA_ASSIGN_TIMING
   unsigned tacc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -102,8 +105,8 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     mbar_fence_init();
     // the loads need nothing but the barrier: issue them before any other set-up work
     mbar_expect_tx(&B->full, (uint32_t)(2 * ctok * 128 + 4 * nwin * 128));
-    tma_load_5d(&map_x, &B->full, sA, 0, uw * g.kw, uh * g.kh, ut * g.kt, bh);
-    tma_load_5d(&map_x, &B->full, sA + half_a, 64, uw * g.kw, uh * g.kh, ut * g.kt, bh);
+    tma_load_5d(&map_x, &B->full, sA, 0, uw * g.kw, uh * g.kh, ut * g.kt + dt0, bh);
+    tma_load_5d(&map_x, &B->full, sA + half_a, 64, uw * g.kw, uh * g.kh, ut * g.kt + dt0, bh);
     tma_load_5d(&map_hi, &B->full, sBhi, 0, sw, sh, st, bh);
     tma_load_5d(&map_hi, &B->full, sBhi + half_b, 64, sw, sh, st, bh);
     tma_load_5d(&map_lo, &B->full, sBlo, 0, sw, sh, st, bh);
@@ -161,8 +164,8 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   size_t tok = 0;
   {
     const int dt = fast_div(li, p.m_khw), r = li - dt * g.kh * g.kw, dh = fast_div(r, p.m_kw), dw = r - dh * g.kw;
-    const int t = ut * g.kt + dt, h = uh * g.kh + dh, w = uw * g.kw + dw;
-    if (li < ctok && t < g.T && h < g.H && w < g.W) { lab = 0; tok = (size_t)(t * g.H + h) * g.W + w; }
+    const int t = ut * g.kt + dt0 + dt, h = uh * g.kh + dh, w = uw * g.kw + dw;
+    if (li < ctok && dt0 + dt < g.kt && t < g.T && h < g.H && w < g.W) { lab = 0; tok = (size_t)(t * g.H + h) * g.W + w; }
   }
   const bool valid = lab == 0;
   float c_max = 0.f;
@@ -347,7 +350,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     }
     __syncwarp();
   }
-  const size_t pbase = ((size_t)bh * g.Nc + cell) * nwin;
+  const size_t pbase = (((size_t)bh * g.Nc + cell) * p.csplit + chunk) * nwin;
   for (int v = tid; v < nwin; v += kThreads) p.part_cnt[pbase + v] = s_cnt[v];
   mbar_wait(&B->sum_done, 0);
   CMARK(8);
@@ -373,8 +376,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
 }  // namespace
 
 bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype) {
-  const int ctok = g.kt * g.kh * g.kw;
-  return dtype == HVA_BF16 && D == kD && ctok <= 128 && g.nwin <= 256 && g.kt <= 256 && g.kh <= 256 && g.kw <= 256 &&
+  return dtype == HVA_BF16 && D == kD && g.kh * g.kw <= 128 && g.nwin <= 256 && g.kt <= 256 && g.kh <= 256 && g.kw <= 256 &&
          g.wt <= 256 && g.wh <= 256 && g.ww <= 256;
 }
 
@@ -395,7 +397,9 @@ bool make_map5(CUtensorMap* m, const void* base, int BH, int d3, int d2, int d1,
 }  // namespace
 
 int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, HvaAssignTc* a) {
-  const int ctok = g.kt * g.kh * g.kw;
+  a->ct = hva_assign_tc_slices(g);
+  a->csplit = (g.kt + a->ct - 1) / a->ct;
+  const int ctok = a->ct * g.kh * g.kw;
   a->npad = (g.nwin + 15) & ~15;
   a->rows_a = (ctok + 15) & ~15;
   a->tmem_cols = 32;
@@ -406,8 +410,8 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
   bytes = std::max(bytes, 4 * half_b + half_a + 16384);
   bytes += 1024;
   a->smem = bytes;
-  if (bytes > 227 * 1024 || (long long)g.Kt * BH > 65535 || g.Kh > 65535) return HVA_EUNSUPPORTED;
-  if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, g.kt, g.kh, g.kw)) return HVA_ECUDA;
+  if (bytes > 227 * 1024 || (long long)g.Kt * BH * a->csplit > 65535 || g.Kh > 65535) return HVA_EUNSUPPORTED;
+  if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, a->ct, g.kh, g.kw)) return HVA_ECUDA;
   if (!make_map5(&a->map_hi, mu_hi, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
   if (!make_map5(&a->map_lo, mu_lo, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
   if (cudaFuncSetAttribute(hva_assign_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
@@ -418,9 +422,9 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
                          int* part_cnt, int* assign, float* lowe, float* probe, cudaStream_t st) {
   auto magic = [](int d) -> uint32_t { return d <= 1 ? 0u : (uint32_t)(((1ull << 32) + d - 1) / d); };
-  AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, magic(g.kh * g.kw), magic(g.kw), magic(g.wh * g.ww),
+  AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, a.csplit, a.ct, magic(g.kh * g.kw), magic(g.kw), magic(g.wh * g.ww),
                    magic(g.ww), a.tmem_cols, probe};
-  hva_assign_tc_kernel<<<dim3(g.Kw, g.Kh, g.Kt * BH), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  hva_assign_tc_kernel<<<dim3(g.Kw, g.Kh, g.Kt * BH * a.csplit), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }

@@ -5,12 +5,25 @@
 
 struct HvaAssignTc {
   CUtensorMap map_x, map_hi, map_lo;
-  int npad, rows_a;
+  int npad, rows_a, csplit, ct;
   uint32_t tmem_cols;
   size_t smem;
 };
 
-// bf16, D = 128, cell of at most 128 tokens, window of at most 256 centroids
+// time slices of a cell per CTA tile (<= 128 token rows): a cell of more than 128 tokens is split along t
+static inline int hva_assign_tc_slices(const HvaGrid& g) {
+  const int per = g.kh * g.kw;
+  int ct = per > 0 ? 128 / per : 1;
+  if (ct < 1) ct = 1;
+  return ct < g.kt ? ct : g.kt;
+}
+static inline int hva_assign_tc_csplit(const HvaGrid& g) {
+  if (g.kh * g.kw > 128) return 1;   // not a tensor-pipe shape: the CUDA-core kernel takes whole cells
+  const int ct = hva_assign_tc_slices(g);
+  return (g.kt + ct - 1) / ct;
+}
+
+// bf16, D = 128, k_h k_w <= 128 (a tile of whole time slices fits 128 rows), window of at most 256 centroids
 bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype);
 // X[BH,T,H,W,128] bf16; mu_hi / mu_lo [BH,Kt,Kh,Kw,128] bf16 (two-term split of the fp32 centroids)
 int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, HvaAssignTc* out);

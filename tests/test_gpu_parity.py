@@ -127,8 +127,9 @@ def test_cluster_non_dividing_lattice_and_wide_window():
 def test_cluster_tensor_pipe_edge_shapes():
     # tcgen05 assignment path (bf16, D=128): non-dividing lattice with zero-filled TMA rows (R-C4), even window (R-C3),
     # windows of 12 / 48 / 75 candidates (one and several 32-column TMEM chunks), cell of exactly 128 tokens
+    # ... and cells of more than 128 tokens, split along t into several CTA tiles (the paper's (11,5,5) Q cells: 275 tokens)
     for T, H, W, cell, win in ((5, 7, 9, (2, 3, 4), (3, 4, 3)), (6, 13, 21, (2, 3, 5), (3, 4, 4)), (8, 16, 16, (2, 8, 8), (3, 2, 2)),
-                               (10, 11, 12, (2, 2, 2), (3, 5, 5))):
+                               (10, 11, 12, (2, 2, 2), (3, 5, 5)), (23, 10, 10, (11, 5, 5), (3, 8, 8)), (9, 16, 8, (4, 8, 8), (3, 3, 3))):
         wl = dataclasses.replace(inputs.C2, name="edge-tc", heads=2, T=T, H=H, W=W, cell=cell, win=win, seed=12)
         assert run_cluster_parity(wl, [0, 1], 1) <= 1
 
