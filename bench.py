@@ -146,6 +146,10 @@ def main():
                     help="extra reports of BASELINE.json configs[3] / configs[4] instead of the bench line: 'sweep' = top-p x merging "
                          "with CTA tile occupancy, 'hybrid' = the 50-step anchor / subset sequence (use --config C5)")
     ap.add_argument("--seq-steps", type=int, default=50)
+    ap.add_argument("--cell-q", default=None, help="k_t,k_h,k_w of the Q grid (default: the workload's); e.g. the paper's 11,5,5")
+    ap.add_argument("--cell-k", default=None, help="k_t,k_h,k_w of the K grid; e.g. the paper's 11,3,3")
+    ap.add_argument("--win", default=None, help="w_t,w_h,w_w of both windows; e.g. the paper's 3,8,8")
+    ap.add_argument("--min-kc", type=float, default=0.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stages", action="store_true")
     args = ap.parse_args()
@@ -176,7 +180,13 @@ def main():
     hQ, hK, hV = [t.contiguous().pin_memory() for t in inputs.make_qkv(wl_r)]
     Q, K, V = hQ.cuda(), hK.cuda(), hV.cuda()
     shape = b.make_shape(wl)
-    cfg = b.make_config(wl, top_p=args.top_p, merge_rounds=args.merge_rounds)
+    cfg = b.make_config(wl, top_p=args.top_p, merge_rounds=args.merge_rounds, min_kc=args.min_kc)
+    i3 = type(cfg.cell_q)
+    tri = lambda t: i3(*[int(x) for x in t.split(",")])
+    if args.cell_q: cfg.cell_q = tri(args.cell_q)
+    if args.cell_k: cfg.cell_k = tri(args.cell_k)
+    if args.win: cfg.win_q = cfg.win_k = tri(args.win)
+    custom = bool(args.cell_q or args.cell_k or args.win or args.min_kc)
     fwd = b.Forward(shape, cfg)
     O = torch.empty_like(Q)
     step = lambda: fwd(Q, K, V, O)
@@ -209,7 +219,8 @@ def main():
     out = {"metric": METRIC, "value": sharding.whole_job_value(ms, world), "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
            "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
-           "config": {"workload": wl.name, "B": wl.B, "heads": wl.heads, "n": wl.n, "D": wl.D, "cell": wl.cell, "iters": wl.iters,
+           "config": {"workload": wl.name + ("+custom-grids" if custom else ""), "B": wl.B, "heads": wl.heads, "n": wl.n, "D": wl.D,
+                      "cell_q": list(cfg.cell_q), "cell_k": list(cfg.cell_k), "win": list(cfg.win_q), "min_kc": float(cfg.min_kc), "iters": wl.iters,
                       "top_p": float(cfg.top_p), "merge_rounds": int(cfg.merge_rounds), "tile": wl.tile,
                       "l2": "inputs (2.2 GB) larger than L2", "parallelism": "head-sharded replicas, no collective"},
            "clocks": clocks,
@@ -219,7 +230,7 @@ def main():
     # ---- per-stage times and rooflines (rank 0)
     if rank == 0 and not args.no_stages:
         out.update(stage_report(b, wl, shape, cfg, Q, K, V, stats, pk))
-    if rank == 0 and not args.no_cpu_baseline:
+    if rank == 0 and not args.no_cpu_baseline and not custom:
         t, cpu_ms = oracle_sample(wl, attn_rows=32, merge_rounds=1 if wl.n > 50000 else None)
         out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": os.cpu_count(), "kind": "oracle",
                                "sample": "one head of %s: oracle clustering Q,K %.1fs, mask %.2fs, merge(1 round) %.1fs, plan %.2fs, "
@@ -340,13 +351,14 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
     es = Q.element_size()
     reps = 3
     st = {}
-    cq = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, Q, want_lowe=False)
-    ck = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, K, want_lowe=False)
-    st["cluster_qk"] = ev_time(lambda: (b.hva_cluster(shape, wl.cell, wl.win, wl.iters, Q, want_lowe=False),
-                                        b.hva_cluster(shape, wl.cell, wl.win, wl.iters, K, want_lowe=False)), reps)
+    cell_q, cell_k, win_q, win_k = list(cfg.cell_q), list(cfg.cell_k), list(cfg.win_q), list(cfg.win_k)
+    cq = b.hva_cluster(shape, cell_q, win_q, wl.iters, Q, want_lowe=False)
+    ck = b.hva_cluster(shape, cell_k, win_k, wl.iters, K, want_lowe=False)
+    st["cluster_qk"] = ev_time(lambda: (b.hva_cluster(shape, cell_q, win_q, wl.iters, Q, want_lowe=False),
+                                        b.hva_cluster(shape, cell_k, win_k, wl.iters, K, want_lowe=False)), reps)
     scale = 1.0 / math.sqrt(D)
-    M = b.hva_build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(cfg.top_p))
-    st["mask"] = ev_time(lambda: b.hva_build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(cfg.top_p)), reps)
+    M = b.hva_build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(cfg.top_p), float(cfg.min_kc))
+    st["mask"] = ev_time(lambda: b.hva_build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(cfg.top_p), float(cfg.min_kc)), reps)
     mg = lambda: b.hva_merge(cq["sizes"], ck["sizes"], M, wl.tile[0], wl.tile[1], int(cfg.merge_rounds), seed=wl.seed)
     gof, ng, gm = mg()
     st["merge"] = ev_time(mg, reps)
