@@ -360,10 +360,14 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   for (int v0 = 0; v0 < nwin; v0 += 32) {
     uint32_t raw[32];
     tmem_ld32(trow + v0, raw);
+    // non-empty slots of this chunk as one ballot word: the stores below are then a bit test + STG with an immediate offset
+    const unsigned nz = __ballot_sync(0xffffffffu, v0 + lane < nwin && s_cnt[v0 + lane] > 0);
+    float* pr = prow + (size_t)v0 * kD;
 #pragma unroll
     for (int j = 0; j < 32; ++j)
-      if (v0 + j < nwin && s_cnt[v0 + j] > 0) prow[(size_t)(v0 + j) * kD] = __uint_as_float(raw[j]);
+      if ((nz >> j) & 1u) pr[j * kD] = __uint_as_float(raw[j]);
   }
+  CMARK(4);
   tc_fence_before();
   __syncthreads();
   CMARK(9);
