@@ -222,21 +222,30 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
       sv[j + 3] = v0 + j + 3 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 3]), c4.w) : kInf;
     }
   };
-  // pass 1: smallest and second smallest filter score (two independent chains, merged)
+  // pass 1: smallest filter score, and the second smallest when the Lowe ratio is wanted (independent chains, merged);
+  // 3-input min keeps the chains short
+  const bool want2 = p.lowe != nullptr;
   float s1 = kInf, s2 = kInf, r1 = kInf, r2 = kInf;
   for (int v0 = 0; v0 < nwin; v0 += 32) {
     load_scores(v0);
+    if (want2) {
 #pragma unroll
-    for (int j = 0; j < 32; j += 2) {
-      s2 = fminf(s2, fmaxf(s1, sv[j]));
-      s1 = fminf(s1, sv[j]);
-      r2 = fminf(r2, fmaxf(r1, sv[j + 1]));
-      r1 = fminf(r1, sv[j + 1]);
+      for (int j = 0; j < 32; j += 2) {
+        s2 = fminf(s2, fmaxf(s1, sv[j]));
+        s1 = fminf(s1, sv[j]);
+        r2 = fminf(r2, fmaxf(r1, sv[j + 1]));
+        r1 = fminf(r1, sv[j + 1]);
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 32; j += 4) {
+        s1 = fminf(s1, fminf(sv[j], sv[j + 1]));
+        r1 = fminf(r1, fminf(sv[j + 2], sv[j + 3]));
+      }
     }
   }
   s2 = fminf(fminf(s2, r2), fmaxf(s1, r1));
   s1 = fminf(s1, r1);
-  const bool want2 = p.lowe != nullptr;
   const float thr = (want2 ? s2 : s1) + margin;     // s2 = +inf (single candidate): every candidate is a contender
   // pass 2: contenders = candidates with score <= thr.  A single contender (without the Lowe ratio) is the direct-form
   // argmin; otherwise the exact direct form decides among them, ascending candidate id, strict '<'  (R-C1)
