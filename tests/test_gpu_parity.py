@@ -534,3 +534,19 @@ def test_forward_different_q_and_k_grids_wide_windows_min_kc():
         got = O[0, hi].float().cpu().numpy().astype(np.float64)[r["rows"]]
         assert np.abs(got - r["O"]).max() <= 2e-2
         assert np.linalg.norm(got - r["O"]) / np.linalg.norm(r["O"]) <= 1e-2
+
+
+def test_batch_dimension_is_folded_into_heads():
+    """B > 1: every (batch, head) is an independent instance, bh = b * heads + head (also the key of the merge hash):
+    the same data viewed as [B=2, heads=2] and as [B=1, heads=4] gives the same bits."""
+    b = _b()
+    wl = inputs.C2
+    Q, K, V = [t.cuda().contiguous() for t in inputs.make_qkv(wl, [0, 1, 2, 3])]
+    cfg = b.make_config(wl)
+    O4 = b.Forward(b.make_shape(wl, heads=4), cfg)(Q, K, V)
+    sh = b.make_shape(wl, heads=2)
+    sh.B = 2
+    view = lambda t: t.view(2, 2, wl.n, wl.D)
+    O22 = b.Forward(sh, cfg)(view(Q), view(K), view(V))
+    torch.cuda.synchronize()
+    assert torch.equal(O4.view(-1), O22.view(-1))
