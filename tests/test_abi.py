@@ -1,0 +1,61 @@
+"""CPU-side checks of the C-ABI boundary (no compute without a GPU): libhva.so builds, loads, exports every symbol that
+include/hva.h declares (and the Python binding lists the same set), the host-only entry points answer, and the argument
+checks return the documented error codes before anything touches CUDA."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2607_03012_b200 import binding as b, build, inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "hva.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(hva_[a-z_0-9]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build(force=False)
+    return b.lib()
+
+
+def test_every_declared_symbol_is_exported_and_bound(lib):
+    names = _declared()
+    assert len(names) >= 20
+    for n in names:
+        assert getattr(lib, n) is not None, n
+    assert sorted(b.EXPORTS) == names                      # the binding covers exactly the header
+
+
+def test_host_only_entry_points(lib):
+    assert lib.hva_version() >= 100
+    assert lib.hva_strerror(0) == b"ok" and b"invalid" in lib.hva_strerror(-1)
+    wl = inputs.C4
+    shape, cfg = b.make_shape(wl), b.make_config(wl)
+    assert b.hva_num_clusters(shape, wl.cell) == 990       # 11 x 9 x 10 (BASELINE.json configs[3])
+    ws, st = b.hva_workspace_bytes(shape, cfg), lib.hva_state_bytes(C.byref(shape), C.byref(cfg))
+    assert ws > 3 * wl.heads * wl.n * wl.D * 2 and 0 < st < ws          # Q', K', V' live in the workspace
+    L = b.hva_plan_describe(24, wl.n, 990, 990, 128)
+    assert L.work_cap >= -(-wl.n // 128) + 990 and L.total > 3 * 24 * wl.n * 4
+    assert lib.hva_cluster_workspace_bytes(C.byref(shape), (C.c_int32 * 3)(*wl.cell), (C.c_int32 * 3)(*wl.win)) > 0
+    assert lib.hva_merge_workspace_bytes(24, 990, 990) > 24 * 990 * 31 * 4
+    assert lib.hva_cluster_update_workspace_bytes(C.byref(shape), 990, 17820) > 24 * 17820 * 8
+
+
+def test_argument_checks_return_error_codes_without_cuda(lib):
+    wl = inputs.C2
+    shape, cfg = b.make_shape(wl), b.make_config(wl)
+    null = C.c_void_p(0)
+    assert lib.hva_forward(C.byref(shape), C.byref(cfg), null, null, null, null, 0, null, null, null, C.c_size_t(0), null) == -1
+    assert lib.hva_cluster(C.byref(shape), (C.c_int32 * 3)(1, 1, 1), (C.c_int32 * 3)(3, 3, 3), 0, null, null, null, null, null, null,
+                           null, null, C.c_size_t(0), null) == -1
+    assert lib.hva_build_mask(1, 8, 8, 48, null, null, null, C.c_float(1.0), C.c_float(0.9), C.c_float(0.0), null, null, C.c_size_t(0), null) == -1
+    bad = b.make_shape(wl)
+    bad.D = 96
+    assert lib.hva_workspace_bytes(C.byref(bad), C.byref(cfg)) == 0
+    assert lib.hva_merge_workspace_bytes(0, 8, 8) == 0
