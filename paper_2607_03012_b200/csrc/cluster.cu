@@ -290,7 +290,7 @@ size_t assign_smem_bytes(const HvaGrid& g, int D, int esize) {
 }
 
 struct ClusterWs {
-  float* part; int* part_cnt; __nv_bfloat16 *hi, *lo; float* musq;
+  float* part; int* part_cnt; __nv_bfloat16 *hi, *lo; float* musq; int* counter;
 };
 
 template <typename T, int D>
@@ -328,7 +328,7 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
     bool last = (it == iters - 1);
     if (tc) {
       HVA_TRY(hva_assign_tc_launch(atc, g, BH, mu, ws.musq, ws.part, ws.part_cnt, last ? assign : nullptr, last ? lowe : nullptr,
-                                   probe, st));
+                                   ws.counter, probe, st));
     } else {
       ClusterParams p{g, BH, X, mu, ws.part, ws.part_cnt, last ? assign : nullptr, last ? lowe : nullptr};
       hva_assign_kernel<T, D><<<grid, kThreads, smem, st>>>(p);
@@ -345,7 +345,7 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
 size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D) {
   const size_t cs = (size_t)hva_assign_tc_csplit(g);
   return hva_align((size_t)BH * g.Nc * cs * g.nwin * D * sizeof(float)) + hva_align((size_t)BH * g.Nc * cs * g.nwin * sizeof(int)) +
-         2 * hva_align((size_t)BH * g.Nc * D * sizeof(__nv_bfloat16)) + hva_align((size_t)BH * g.Nc * sizeof(float));
+         2 * hva_align((size_t)BH * g.Nc * D * sizeof(__nv_bfloat16)) + hva_align((size_t)BH * g.Nc * sizeof(float)) + hva_align(sizeof(int));
 }
 
 int hva_mu_split_launch(int BH, int Nc, int D, const float* mu, void* mu_hi, void* mu_lo, float* musq, cudaStream_t st) {
@@ -385,7 +385,8 @@ extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int3
     cw.part_cnt = reinterpret_cast<int*>(w); w += hva_align((size_t)BH * g.Nc * cs * g.nwin * sizeof(int));
     cw.hi = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
     cw.lo = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
-    cw.musq = reinterpret_cast<float*>(w);
+    cw.musq = reinterpret_cast<float*>(w); w += hva_align((size_t)BH * g.Nc * sizeof(float));
+    cw.counter = reinterpret_cast<int*>(w);
   }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
 #define HVA_DISPATCH(T, DD) return run_cluster<T, DD>(g, BH, iters, X, mu_init, assign, mu, sizes, sums, lowe, cw, s->dtype, st)

@@ -22,6 +22,8 @@
 #include "ptx.cuh"
 #include "cluster_tc.cuh"
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
 
 namespace {
 using namespace hva_ptx;
@@ -42,12 +44,16 @@ struct AssignTcParams {
   int csplit, ct;      // a cell of more than 128 tokens is split along t into csplit tiles of ct time slices (one CTA each)
   uint32_t m_khw, m_kw, m_whw, m_ww;   // fast_div multipliers for k_h k_w, k_w, w_h w_w, w_w
   uint32_t tmem_cols;
+  int one_pass;        // 2 npad <= 256: one MMA pass over [hi; lo] stacked as 2 npad score columns (the token tile is read once)
+  int n_items;         // K_w * K_h * K_t * BH * csplit tiles: a CTA starts with tile blockIdx.x and draws the following ones
+  int* counter;        // from this device counter (zero at launch), so that the SMs finish together
   float* probe;        // debug: max |score_tc - score_exact| / (|x| max|mu|), or null
 };
 
 struct __align__(8) AssignTcBars {
   uint64_t full, mma_done, sum_done;
   uint32_t tmem_base;
+  int next;
 };
 
 __device__ __noinline__ float direct_dist_probe(const unsigned char* sA, int half_bytes, int r, const float* mu) {
@@ -55,7 +61,7 @@ __device__ __noinline__ float direct_dist_probe(const unsigned char* sA, int hal
 }
 
 #ifdef HVA_ASSIGN_TIMING
-#define CMARK(k) do { if (threadIdx.x == 0) { long long _t = clock64(); tacc[k] = (unsigned)(_t - tprev); tprev = _t; } } while (0)
+#define CMARK(k) do { if (threadIdx.x == 0) { long long _t = clock64(); tacc[k] += (unsigned)(_t - tprev); tprev = _t; } } while (0)
 #else
 #define CMARK(k) do { } while (0)
 #endif
@@ -63,18 +69,16 @@ __device__ __noinline__ float direct_dist_probe(const unsigned char* sA, int hal
 // x / d for 0 <= x, x * d < 2^32 by one multiply-high (m = ceil(2^32 / d); d == 1 is passed as m = 0)
 __device__ __forceinline__ int fast_div(int x, uint32_t m) { return m ? (int)__umulhi((uint32_t)x, m) : x; }
 
-// One CTA per home cell: grid = (K_w, K_h, K_t * BH), 128 threads, thread = token row of the cell = TMEM lane.
-__global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_constant__ CUtensorMap map_x,
+// Persistent CTAs (as many as fit the SMs, 4 per SM at the 3x5x8 cells) draw the tiles (home cell x time split) in raster
+// order from a device counter; 128 threads, thread = token row of the tile = TMEM lane.  Per-CTA set-up (TMEM allocation,
+// barriers, the CTA launch itself: ~2.5K clk, during which a kernel that allocates TMEM starts no other CTA on the SM)
+// is paid once, and the loads of the next tile are issued as soon as the sums MMA has released the tiles, under the epilogue.
+__global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_hi,
                                                                  const __grid_constant__ CUtensorMap map_lo, AssignTcParams p) {
   const HvaGrid& g = p.g;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int uw = blockIdx.x, uh = blockIdx.y;
-  const int chunk = blockIdx.z % p.csplit, zz = blockIdx.z / p.csplit, bh = zz / g.Kt, ut = zz - bh * g.Kt;
-  const int dt0 = chunk * p.ct;                        // first time slice of this tile inside the cell
-  const int cell = (ut * g.Kh + uh) * g.Kw + uw;
-  const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
-  const int ctok = p.ct * g.kh * g.kw, nwin = g.nwin, npad = p.npad;   // token rows of this tile
+  const int ctok = p.ct * g.kh * g.kw, nwin = g.nwin, npad = p.npad;   // token rows of a tile
   const int half_a = p.rows_a * 128, half_b = npad * 128;
 #ifdef HVA_ASSIGN_TIMING
   unsigned tacc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -82,38 +86,84 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
 #endif
 
   // Shared memory (offsets from a 1024-byte aligned base, kept as shared-space pointers):
-  //   sB  [hi | lo][2 halves][npad][128 B]  window centroids, K-major SW128; after MMA 1 the hi part is reused for
+  //   sB  [2 halves][hi | lo][npad][128 B]  window centroids, K-major SW128 (hi and lo rows of a half are contiguous: one
+  //       B operand of 2 npad rows); after MMA 1 the first half is reused for
   //       sP [2 halves][npad][128 B], the one-hot tile P^T (rows = slots, K = tokens; B of MMA 2, K-major)
-  //   sA  [2 halves][rows_a][128 B]         the cell's tokens (A of MMA 1, K-major; A of MMA 2, MN-major)
+  //   sA  [2 halves][rows_a][128 B]         the tile's tokens (A of MMA 1, K-major; A of MMA 2, MN-major)
   // MMA 1 reads 128 token rows: rows past the tile alias whatever follows inside the allocation and only feed TMEM
   // lanes nobody reads.
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-  unsigned char* sBhi = smem;
-  unsigned char* sBlo = sBhi + 2 * half_b;
+  unsigned char* sBhi = smem;                 // per 64-dim half: [hi rows | lo rows], halves 2 half_b apart
+  unsigned char* sBlo = sBhi + half_b;
   unsigned char* sP = smem;
   unsigned char* sA = smem + 4 * half_b;
   float* s_c = reinterpret_cast<float*>(sA + 2 * half_a);     // [npad] |mu_v|^2
   int* s_u = reinterpret_cast<int*>(s_c + npad);              // [npad] centroid id of window slot v
-  int* s_cnt = s_u + npad;                                    // [npad] tokens of the cell assigned to slot v
+  int* s_cnt = s_u + npad;                                    // [npad] tokens of the tile assigned to slot v
   AssignTcBars* B = reinterpret_cast<AssignTcBars*>(s_cnt + npad);
 
+  // The SM starts the CTAs of a kernel that contains tcgen05.alloc one at a time: the next CTA does not begin before this one
+  // has given the allocation permit back (measured: a CTA that never reaches the relinquish keeps the whole SM to itself).
+  // So the allocation is the first thing the CTA does, on a warp of its own, while thread 0 sets up the loads.
+  if (warp == 1) tmem_alloc(&B->tmem_base, p.tmem_cols);
+
+  // tile -> (cell coordinates, time split, batch*head); thread 0 issues the six boxes of a tile
+  struct Tile { int uw, uh, ut, bh, chunk; };
+  auto decode = [&](int item) {
+    Tile t;
+    const int khw = g.Kw * g.Kh, z = item / khw, r = item - z * khw;
+    t.uh = r / g.Kw; t.uw = r - t.uh * g.Kw;
+    t.chunk = z % p.csplit;
+    const int zz = z / p.csplit;
+    t.bh = zz / g.Kt; t.ut = zz - t.bh * g.Kt;
+    return t;
+  };
+  // the six boxes of a tile, two per call: part 0 = tokens, part 1 = hi, part 2 = lo (a 5-D box costs its issuing thread
+  // ~150 clk, so the parts go to different warps); the expect-tx may be posted after bytes have landed
+  auto issue = [&](const Tile& t, int part) {
+    if (part == 0) {
+      const int t0 = t.ut * g.kt + t.chunk * p.ct;
+      mbar_expect_tx(&B->full, (uint32_t)(2 * ctok * 128 + 4 * nwin * 128));
+      tma_load_5d(&map_x, &B->full, sA, 0, t.uw * g.kw, t.uh * g.kh, t0, t.bh);
+      tma_load_5d(&map_x, &B->full, sA + half_a, 64, t.uw * g.kw, t.uh * g.kh, t0, t.bh);
+    } else {
+      const int st = hva_win_start(t.ut, g.wt, g.Kt), sh = hva_win_start(t.uh, g.wh, g.Kh), sw = hva_win_start(t.uw, g.ww, g.Kw);
+      const CUtensorMap* m = part == 1 ? &map_hi : &map_lo;
+      unsigned char* dst = part == 1 ? sBhi : sBlo;
+      tma_load_5d(m, &B->full, dst, 0, sw, sh, st, t.bh);
+      tma_load_5d(m, &B->full, dst + 2 * half_b, 64, sw, sh, st, t.bh);
+    }
+  };
   if (tid == 0) {
     mbar_init(&B->full, 1);
     mbar_init(&B->mma_done, 1);
     mbar_init(&B->sum_done, 1);
     mbar_fence_init();
-    // the loads need nothing but the barrier: issue them before any other set-up work
-    mbar_expect_tx(&B->full, (uint32_t)(2 * ctok * 128 + 4 * nwin * 128));
-    tma_load_5d(&map_x, &B->full, sA, 0, uw * g.kw, uh * g.kh, ut * g.kt + dt0, bh);
-    tma_load_5d(&map_x, &B->full, sA + half_a, 64, uw * g.kw, uh * g.kh, ut * g.kt + dt0, bh);
-    tma_load_5d(&map_hi, &B->full, sBhi, 0, sw, sh, st, bh);
-    tma_load_5d(&map_hi, &B->full, sBhi + half_b, 64, sw, sh, st, bh);
-    tma_load_5d(&map_lo, &B->full, sBlo, 0, sw, sh, st, bh);
-    tma_load_5d(&map_lo, &B->full, sBlo + half_b, 64, sw, sh, st, bh);
+    if ((int)blockIdx.x < p.n_items) {   // the loads need nothing but the barrier
+      const Tile t = decode(blockIdx.x);
+      issue(t, 0); issue(t, 1); issue(t, 2);
+    }
   }
-  __syncwarp();
-  if (warp == 0) tmem_alloc(&B->tmem_base, p.tmem_cols);
+  // token rows ctok .. rows_a-1 take part in MMA 2 (K granule 16) with zero weight: they must be finite; TMA never writes them
+  for (int i = tid; i < (p.rows_a - ctok) * 16; i += kThreads) {
+    const int r = ctok + (i >> 4), q = i & 15;
+    *reinterpret_cast<uint4*>(sA + (q >> 3) * half_a + r * 128 + ((q & 7) << 4)) = make_uint4(0, 0, 0, 0);
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  // position of this thread's token inside a tile
+  const int li = tid;
+  const int ldt = fast_div(li, p.m_khw), lr = li - ldt * g.kh * g.kw, ldh = fast_div(lr, p.m_kw), ldw = lr - ldh * g.kw;
+  const float kInf = __int_as_float(0x7f800000);
+  uint32_t ph = 0;
+
+  for (int item = blockIdx.x, next_item = 0; item < p.n_items; item = next_item, ph ^= 1u) {
+  const Tile T = decode(item);
+  if (tid == 96) B->next = (int)gridDim.x + atomicAdd(p.counter, 1);   // the tile after this one; published by the barrier below
+  const int uw = T.uw, uh = T.uh, ut = T.ut, bh = T.bh, chunk = T.chunk;
+  const int dt0 = chunk * p.ct;                        // first time slice of this tile inside the cell
+  const int cell = (ut * g.Kh + uh) * g.Kw + uw;
+  const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
   // window slot -> centroid id (ascending == delta_t-major, Alg. 2 line 18), |mu|^2   (warps 1..3)
   for (int v = tid - 32; v < npad; v += kThreads - 32) {
     if (v < 0) continue;
@@ -126,46 +176,41 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     }
     s_u[v] = u; s_c[v] = c; s_cnt[v] = 0;
   }
-  // token rows ctok .. rows_a-1 take part in MMA 2 (K granule 16) with zero weight: they must be finite; TMA never writes them
-  for (int i = tid; i < (p.rows_a - ctok) * 16; i += kThreads) {
-    const int r = ctok + (i >> 4), q = i & 15;
-    *reinterpret_cast<uint4*>(sA + (q >> 3) * half_a + r * 128 + ((q & 7) << 4)) = make_uint4(0, 0, 0, 0);
-  }
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   tc_fence_before();
   __syncthreads();
   CMARK(0);
   tc_fence_after();
   const uint32_t tmem = B->tmem_base;
+  next_item = B->next;
 
   if (warp == 0) {
     // warp-uniform up to the elected lane: descriptors built once in uniform registers, a k-step only adds a constant to the
     // start-address field (a lane-0-only loop spends ~100 clk per MMA on descriptor arithmetic and R2UR moves)
-    mbar_wait(&B->full, 0);
+    mbar_wait(&B->full, ph);
     tc_fence_after();
-    const uint32_t idesc = umma_idesc_bf16(128, (uint32_t)npad, 0, 0);
+    const uint32_t idesc = umma_idesc_bf16(128, (uint32_t)(p.one_pass ? 2 * npad : npad), 0, 0);
     const uint64_t da = umma_desc(smem_u32(sA), 16, 1024), dhi = umma_desc(smem_u32(sBhi), 16, 1024), dlo = umma_desc(smem_u32(sBlo), 16, 1024);
-    const uint32_t ha = (uint32_t)half_a >> 4, hb = (uint32_t)half_b >> 4;
+    const uint32_t ha = (uint32_t)half_a >> 4, hb = (uint32_t)(2 * half_b) >> 4;
     if (elect_one()) {
 #pragma unroll
       for (int ks = 0; ks < kD / 16; ++ks)
         mma_ss(tmem, da + ((ks >> 2) * ha + (ks & 3) * 2), dhi + ((ks >> 2) * hb + (ks & 3) * 2), idesc, ks > 0);
+      if (!p.one_pass) {
 #pragma unroll
-      for (int ks = 0; ks < kD / 16; ++ks)
-        mma_ss(tmem, da + ((ks >> 2) * ha + (ks & 3) * 2), dlo + ((ks >> 2) * hb + (ks & 3) * 2), idesc, 1);
+        for (int ks = 0; ks < kD / 16; ++ks)
+          mma_ss(tmem, da + ((ks >> 2) * ha + (ks & 3) * 2), dlo + ((ks >> 2) * hb + (ks & 3) * 2), idesc, 1);
+      }
       tc_commit(&B->mma_done);
     }
     __syncwarp();
   }
 
   // ---- token geometry; an upper bound of |x|^2 and the filter margin while the MMAs run
-  const int li = tid;
   int lab = -1;
   size_t tok = 0;
   {
-    const int dt = fast_div(li, p.m_khw), r = li - dt * g.kh * g.kw, dh = fast_div(r, p.m_kw), dw = r - dh * g.kw;
-    const int t = ut * g.kt + dt0 + dt, h = uh * g.kh + dh, w = uw * g.kw + dw;
-    if (li < ctok && dt0 + dt < g.kt && t < g.T && h < g.H && w < g.W) { lab = 0; tok = (size_t)(t * g.H + h) * g.W + w; }
+    const int t = ut * g.kt + dt0 + ldt, h = uh * g.kh + ldh, w = uw * g.kw + ldw;
+    if (li < ctok && dt0 + ldt < g.kt && t < g.T && h < g.H && w < g.W) { lab = 0; tok = (size_t)(t * g.H + h) * g.W + w; }
   }
   const bool valid = lab == 0;
   float c_max = 0.f;
@@ -173,7 +218,7 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
     const float4 c4 = *reinterpret_cast<const float4*>(s_c + v);
     c_max = fmaxf(fmaxf(c_max, fmaxf(c4.x, c4.y)), fmaxf(c4.z, c4.w));
   }
-  mbar_wait(&B->full, 0);
+  mbar_wait(&B->full, ph);
   CMARK(1);
   // |x|^2 only scales the margin: packed bf16 FMAs (4 x 2 accumulators of 16 non-negative terms each: relative
   // error < 16 * 2^-8), inflated by 1/8 so that it is an upper bound
@@ -200,26 +245,37 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   const float margin = 2.f * (2.f * kEpsDot * xm + 6e-7f * (c_max + 2.f * xm));
 
   CMARK(2);
-  mbar_wait(&B->mma_done, 0);
+  mbar_wait(&B->mma_done, ph);
   CMARK(3);
   tc_fence_after();
   // the B tiles are dead: clear the one-hot tile that aliases the hi part (filled after the labels are known)
   for (int i = tid; i < (2 * half_b) / 16; i += kThreads) reinterpret_cast<uint4*>(sP)[i] = make_uint4(0, 0, 0, 0);
 
-  const float kInf = __int_as_float(0x7f800000);
   const uint32_t trow = tmem + ((uint32_t)(warp * 32) << 16);
   float sv[32];
   // scores of one 32-candidate chunk: sv[j] = |mu_v|^2 - 2 x.mu_v, +inf past the window
   auto load_scores = [&](int v0) {
-    uint32_t raw[32];
-    tmem_ld32(trow + v0, raw);
 #pragma unroll
-    for (int j = 0; j < 32; j += 4) {
-      const float4 c4 = *reinterpret_cast<const float4*>(s_c + v0 + j);   // npad is a multiple of 16
-      sv[j] = v0 + j < nwin ? fmaf(-2.f, __uint_as_float(raw[j]), c4.x) : kInf;
-      sv[j + 1] = v0 + j + 1 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 1]), c4.y) : kInf;
-      sv[j + 2] = v0 + j + 2 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 2]), c4.z) : kInf;
-      sv[j + 3] = v0 + j + 3 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 3]), c4.w) : kInf;
+    for (int h = 0; h < 32; h += 16) {
+      uint32_t raw[16], rlo[16];
+      if (p.one_pass) {      // x.hi in columns [0, npad), x.lo in [npad, 2 npad)
+        tmem_ld16_nowait(trow + v0 + h, raw);
+        tmem_ld16_nowait(trow + npad + v0 + h, rlo);
+        tmem_ld_wait16(raw);
+        tmem_ld_wait16(rlo);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) raw[j] = __float_as_uint(__uint_as_float(raw[j]) + __uint_as_float(rlo[j]));
+      } else {
+        tmem_ld16(trow + v0 + h, raw);
+      }
+#pragma unroll
+      for (int j = 0; j < 16; j += 4) {
+        const float4 c4 = *reinterpret_cast<const float4*>(s_c + v0 + h + j);   // npad is a multiple of 16
+        sv[h + j] = v0 + h + j < nwin ? fmaf(-2.f, __uint_as_float(raw[j]), c4.x) : kInf;
+        sv[h + j + 1] = v0 + h + j + 1 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 1]), c4.y) : kInf;
+        sv[h + j + 2] = v0 + h + j + 2 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 2]), c4.z) : kInf;
+        sv[h + j + 3] = v0 + h + j + 3 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 3]), c4.w) : kInf;
+      }
     }
   };
   // pass 1: smallest filter score, and the second smallest when the Lowe ratio is wanted (independent chains, merged);
@@ -329,11 +385,10 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
 
   // ---- one-hot tile P^T[slot, token] = 1 and the slot counts
   {
-    const unsigned m = __match_any_sync(0xffffffffu, lab);
     if (lab >= 0) {
       *reinterpret_cast<__nv_bfloat16*>(sP + (li >> 6) * half_b + lab * 128 + (((((li & 63) >> 3) ^ (lab & 7))) << 4) + (li & 7) * 2) =
           __float2bfloat16_rn(1.0f);
-      if ((m & ((1u << lane) - 1u)) == 0) atomicAdd(&s_cnt[lab], __popc(m));
+      atomicAdd(&s_cnt[lab], 1);     // (a warp-wide match.any to combine equal labels first costs more than the conflicts)
     }
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -361,9 +416,12 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   }
   const size_t pbase = (((size_t)bh * g.Nc + cell) * p.csplit + chunk) * nwin;
   for (int v = tid; v < nwin; v += kThreads) p.part_cnt[pbase + v] = s_cnt[v];
-  mbar_wait(&B->sum_done, 0);
+  mbar_wait(&B->sum_done, ph);
   CMARK(8);
   tc_fence_after();
+  // both tiles are dead (every generic read of sA happened before the one-hot barrier, MMA 2 has finished): the next tile's
+  // loads run under the epilogue
+  if (lane == 0 && warp != 1 && next_item < p.n_items) issue(decode(next_item), warp == 0 ? 0 : warp - 1);
   // thread = feature dim: a warp stores 32 consecutive floats of a partial row (coalesced)
   float* prow = p.part + pbase * kD + tid;
   for (int v0 = 0; v0 < nwin; v0 += 32) {
@@ -378,12 +436,14 @@ __global__ void __launch_bounds__(kThreads) hva_assign_tc_kernel(const __grid_co
   }
   CMARK(4);
   tc_fence_before();
-  __syncthreads();
+  __syncthreads();     // s_cnt and the TMEM columns are free for the next tile
   CMARK(9);
+  }   // tiles
 #ifdef HVA_ASSIGN_TIMING
   if (threadIdx.x == 0 && p.probe) for (int k = 0; k < 10; ++k) atomicAdd(p.probe + 16 + k, (float)tacc[k]);
 #endif
-  if (warp == 0) { tc_fence_after(); tmem_dealloc(tmem, p.tmem_cols); }
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(B->tmem_base, p.tmem_cols); }
 }
 
 }  // namespace
@@ -415,29 +475,46 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
   const int ctok = a->ct * g.kh * g.kw;
   a->npad = (g.nwin + 15) & ~15;
   a->rows_a = (ctok + 15) & ~15;
+  a->one_pass = 2 * a->npad <= 256;
   a->tmem_cols = 32;
-  while ((int)a->tmem_cols < a->npad) a->tmem_cols <<= 1;
+  while ((int)a->tmem_cols < (a->one_pass ? 2 : 1) * a->npad) a->tmem_cols <<= 1;
   const size_t half_a = (size_t)a->rows_a * 128, half_b = (size_t)a->npad * 128;
   size_t bytes = 4 * half_b + 2 * half_a + 3 * sizeof(int) * (size_t)a->npad + sizeof(AssignTcBars) + 16;
   // MMA 1 reads 128 token rows of its A operand: keep the over-read inside the allocation
   bytes = std::max(bytes, 4 * half_b + half_a + 16384);
   bytes += 1024;
   a->smem = bytes;
-  if (bytes > 227 * 1024 || (long long)g.Kt * BH * a->csplit > 65535 || g.Kh > 65535) return HVA_EUNSUPPORTED;
+  if (bytes > 227 * 1024 || (long long)g.Kw * g.Kh * g.Kt * BH * a->csplit > 0x7fffffffLL) return HVA_EUNSUPPORTED;
   if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, a->ct, g.kh, g.kw)) return HVA_ECUDA;
   if (!make_map5(&a->map_hi, mu_hi, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
   if (!make_map5(&a->map_lo, mu_lo, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
   if (cudaFuncSetAttribute(hva_assign_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
     return HVA_ECUDA;
+  // resident CTAs per SM from the shared-memory, register and TMEM budgets (the runtime's occupancy query answers 1 for a
+  // kernel that allocates TMEM, whatever it allocates)
+  int dev = 0, sms = 0, smem_sm = 0, smem_res = 0, regs_sm = 0;
+  cudaFuncAttributes fa;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&smem_res, cudaDevAttrReservedSharedMemoryPerBlock, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev) != cudaSuccess ||
+      cudaFuncGetAttributes(&fa, hva_assign_tc_kernel) != cudaSuccess)
+    return HVA_ECUDA;
+  const int regs_cta = ((fa.numRegs + 7) & ~7) * kThreads;
+  int per_sm = std::min({(int)((size_t)smem_sm / (bytes + (size_t)smem_res)), regs_sm / std::max(regs_cta, 1), 512 / (int)a->tmem_cols});
+  if (per_sm < 1) return HVA_EUNSUPPORTED;
+  a->grid = sms * per_sm;
+  if (getenv("HVA_DEBUG")) fprintf(stderr, "assign_tc: %d SMs x %d CTAs, smem %zu, tmem %u\n", sms, per_sm, bytes, a->tmem_cols);
   return HVA_OK;
 }
 
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
-                         int* part_cnt, int* assign, float* lowe, float* probe, cudaStream_t st) {
+                         int* part_cnt, int* assign, float* lowe, int* counter, float* probe, cudaStream_t st) {
   auto magic = [](int d) -> uint32_t { return d <= 1 ? 0u : (uint32_t)(((1ull << 32) + d - 1) / d); };
   AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, a.csplit, a.ct, magic(g.kh * g.kw), magic(g.kw), magic(g.wh * g.ww),
-                   magic(g.ww), a.tmem_cols, probe};
-  hva_assign_tc_kernel<<<dim3(g.Kw, g.Kh, g.Kt * BH * a.csplit), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+                   magic(g.ww), a.tmem_cols, a.one_pass, g.Kw * g.Kh * g.Kt * BH * a.csplit, counter, probe};
+  if (cudaMemsetAsync(counter, 0, sizeof(int), st) != cudaSuccess) return HVA_ECUDA;
+  hva_assign_tc_kernel<<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }

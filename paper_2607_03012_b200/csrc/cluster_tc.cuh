@@ -8,6 +8,8 @@ struct HvaAssignTc {
   int npad, rows_a, csplit, ct;
   uint32_t tmem_cols;
   size_t smem;
+  int one_pass;        // one MMA pass over the stacked [hi; lo] centroid tile
+  int grid;            // resident CTAs (SMs x CTAs per SM): the kernel is persistent
 };
 
 // time slices of a cell per CTA tile (<= 128 token rows): a cell of more than 128 tokens is split along t
@@ -28,7 +30,7 @@ bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype);
 // X[BH,T,H,W,128] bf16; mu_hi / mu_lo [BH,Kt,Kh,Kw,128] bf16 (two-term split of the fp32 centroids)
 int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, HvaAssignTc* out);
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
-                         int* part_cnt, int* assign, float* lowe, float* probe, cudaStream_t st);
+                         int* part_cnt, int* assign, float* lowe, int* counter, float* probe, cudaStream_t st);
 
 // Window-less variant for the hybrid subset step (hybrid_tc.cu): subset tokens against ALL centroids.
 bool hva_subset_tc_supported(int D, int dtype, int Nc);
