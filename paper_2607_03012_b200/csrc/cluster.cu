@@ -225,62 +225,113 @@ __device__ __forceinline__ void axis_cells(int u, int w, int K, int& lo, int& cn
 }
 
 // mu_u <- z_u / n_u if n_u > 0 else mu_u   (Alg. 2 lines 22-23).  z_u = sum over the home cells g whose
-// window contains u of part[g][slot(u in g)], in ascending cell order (fixed => deterministic).  Warp 0 lists the
-// non-empty (cell, slot) partials of u in shared memory (ordered ballot compaction); every thread (= feature dim)
-// then adds its column over that list.
+// window contains u of part[g][slot(u in g)], in ascending cell order (fixed => deterministic).  One warp per centroid,
+// four centroids per block, no shared memory and no block barrier: the lanes read the counts of up to 32 (cell, slot)
+// partials at once, the non-empty ones are then walked in order (ballot bits), four row loads in flight, each lane adding
+// its D/32 feature dims.
+constexpr int kFinWarps = 4;
 template <int D>
-__global__ void __launch_bounds__(D) hva_finalize_kernel(HvaGrid g, const float* __restrict__ part,
-                                                         const int* __restrict__ part_cnt, float* __restrict__ mu,
-                                                         int* __restrict__ sizes, float* __restrict__ sums, MuSplit sp, int csplit) {
-  const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
+__global__ void __launch_bounds__(32 * kFinWarps) hva_finalize_kernel(HvaGrid g, const float* __restrict__ part,
+                                                                      const int* __restrict__ part_cnt, float* __restrict__ mu,
+                                                                      int* __restrict__ sizes, float* __restrict__ sums, MuSplit sp,
+                                                                      int csplit) {
+  constexpr int V = D / 32;
+  const int lane = threadIdx.x & 31, u = blockIdx.x * kFinWarps + (threadIdx.x >> 5), bh = blockIdx.y;
+  if (u >= g.Nc) return;
   const int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
-  __shared__ unsigned s_idx[1024];     // at most nwin <= 1024 home cells have u in their window (checked by hva_cluster)
-  __shared__ int s_m, s_n;
-  if (c < 32) {
-    int lt, nt, lh, nh, lw, nw;
-    axis_cells(ut, g.wt, g.Kt, lt, nt);
-    axis_cells(uh, g.wh, g.Kh, lh, nh);
-    axis_cells(uw, g.ww, g.Kw, lw, nw);
-    const int total = nt * nh * nw * csplit;      // (home cell, t-tile of the cell) partials, ascending cell then tile
-    int m = 0, n = 0;
-    for (int e0 = 0; e0 < total; e0 += 32) {
-      const int e = e0 + c;
-      int k = 0;
-      unsigned idx = 0;
-      if (e < total) {
-        const int ce = e / csplit, chunk = e - ce * csplit;
-        const int gt = lt + ce / (nh * nw), gh = lh + (ce / nw) % nh, gw = lw + ce % nw;
-        const int cell = (gt * g.Kh + gh) * g.Kw + gw;
-        const int slot = ((ut - hva_win_start(gt, g.wt, g.Kt)) * g.wh + (uh - hva_win_start(gh, g.wh, g.Kh))) * g.ww +
-                         (uw - hva_win_start(gw, g.ww, g.Kw));
-        idx = (unsigned)((((size_t)bh * g.Nc + cell) * csplit + chunk) * g.nwin + slot);
-        k = part_cnt[idx];
-      }
-      const unsigned bal = __ballot_sync(0xffffffffu, k > 0);
-      if (k > 0) s_idx[m + __popc(bal & ((1u << c) - 1u))] = idx;
-      m += __popc(bal);
+  int lt, nt, lh, nh, lw, nw;
+  axis_cells(ut, g.wt, g.Kt, lt, nt);
+  axis_cells(uh, g.wh, g.Kh, lh, nh);
+  axis_cells(uw, g.ww, g.Kw, lw, nw);
+  const int total = nt * nh * nw * csplit;      // (home cell, t-tile of the cell) partials, ascending cell then tile
+  float z[V];
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) k += __shfl_xor_sync(0xffffffffu, k, o);
-      n += k;
+  for (int i = 0; i < V; ++i) z[i] = 0.f;
+  int n = 0;
+  auto row = [&](unsigned id, float (&r)[V]) {
+    const float* q = part + (size_t)id * D + lane * V;
+    if constexpr (V == 4) { const float4 t = *reinterpret_cast<const float4*>(q); r[0] = t.x; r[1] = t.y; r[2] = t.z; r[3] = t.w; }
+    else { const float2 t = *reinterpret_cast<const float2*>(q); r[0] = t.x; r[1] = t.y; }
+  };
+  for (int e0 = 0; e0 < total; e0 += 32) {
+    const int e = e0 + lane;
+    int k = 0;
+    unsigned idx = 0;
+    if (e < total) {
+      const int ce = e / csplit, chunk = e - ce * csplit;
+      const int gt = lt + ce / (nh * nw), gh = lh + (ce / nw) % nh, gw = lw + ce % nw;
+      const int cell = (gt * g.Kh + gh) * g.Kw + gw;
+      const int slot = ((ut - hva_win_start(gt, g.wt, g.Kt)) * g.wh + (uh - hva_win_start(gh, g.wh, g.Kh))) * g.ww +
+                       (uw - hva_win_start(gw, g.ww, g.Kw));
+      idx = (unsigned)((((size_t)bh * g.Nc + cell) * csplit + chunk) * g.nwin + slot);
+      k = part_cnt[idx];
     }
-    if (c == 0) { s_m = m; s_n = n; }
+    unsigned bal = __ballot_sync(0xffffffffu, k > 0);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) k += __shfl_xor_sync(0xffffffffu, k, o);
+    n += k;
+    while (bal) {      // ascending partial order, up to four rows in flight
+      unsigned id[4];
+      int cnt = 0;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int b = bal ? __ffs(bal) - 1 : 0;
+        id[j] = __shfl_sync(0xffffffffu, idx, b);
+        if (bal) { ++cnt; bal &= bal - 1; }
+      }
+      float r[4][V];
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (j < cnt) row(id[j], r[j]);
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (j < cnt) {
+#pragma unroll
+          for (int i = 0; i < V; ++i) z[i] += r[j][i];
+        }
+    }
   }
-  __syncthreads();
-  const int m = s_m, n = s_n;
-  float z = 0.f;
-  int e = 0;
-  for (; e + 4 <= m; e += 4) {
-    const float p0 = part[(size_t)s_idx[e] * D + c], p1 = part[(size_t)s_idx[e + 1] * D + c];
-    const float p2 = part[(size_t)s_idx[e + 2] * D + c], p3 = part[(size_t)s_idx[e + 3] * D + c];
-    z += p0; z += p1; z += p2; z += p3;
+  const size_t o = ((size_t)bh * g.Nc + u) * D + lane * V;
+  float m[V];
+  float q = 0.f;
+  auto ld = [&](const float* a, float (&r)[V]) {
+    if constexpr (V == 4) { const float4 t = *reinterpret_cast<const float4*>(a); r[0] = t.x; r[1] = t.y; r[2] = t.z; r[3] = t.w; }
+    else { const float2 t = *reinterpret_cast<const float2*>(a); r[0] = t.x; r[1] = t.y; }
+  };
+  auto stv = [&](float* a, const float (&r)[V]) {
+    if constexpr (V == 4) *reinterpret_cast<float4*>(a) = make_float4(r[0], r[1], r[2], r[3]);
+    else *reinterpret_cast<float2*>(a) = make_float2(r[0], r[1]);
+  };
+  if (n > 0) {
+#pragma unroll
+    for (int i = 0; i < V; ++i) m[i] = __fdiv_rn(z[i], (float)n);
+    stv(mu + o, m);
+  } else {
+    ld(mu + o, m);
   }
-  for (; e < m; ++e) z += part[(size_t)s_idx[e] * D + c];
-  size_t o = ((size_t)bh * g.Nc + u) * D + c;
-  float mval = mu[o];
-  if (n > 0) { mval = __fdiv_rn(z, (float)n); mu[o] = mval; }
-  if (sums) sums[o] = z;
-  if (c == 0) sizes[(size_t)bh * g.Nc + u] = n;
-  mu_split_store<D>(sp, (size_t)bh * g.Nc + u, c, mval);
+  if (sums) stv(sums + o, z);
+#pragma unroll
+  for (int i = 0; i < V; ++i) q = fmaf(m[i], m[i], q);
+  if (lane == 0) sizes[(size_t)bh * g.Nc + u] = n;
+  if (sp.hi) {
+    __nv_bfloat162 h2[V / 2], l2[V / 2];
+#pragma unroll
+    for (int i = 0; i < V; i += 2) {
+      const __nv_bfloat16 h0 = __float2bfloat16_rn(m[i]), h1 = __float2bfloat16_rn(m[i + 1]);
+      h2[i / 2] = __nv_bfloat162(h0, h1);
+      l2[i / 2] = __nv_bfloat162(__float2bfloat16_rn(m[i] - __bfloat162float(h0)), __float2bfloat16_rn(m[i + 1] - __bfloat162float(h1)));
+    }
+    if constexpr (V == 4) {
+      *reinterpret_cast<uint2*>(sp.hi + o) = *reinterpret_cast<const uint2*>(h2);
+      *reinterpret_cast<uint2*>(sp.lo + o) = *reinterpret_cast<const uint2*>(l2);
+    } else {
+      *reinterpret_cast<__nv_bfloat162*>(sp.hi + o) = h2[0];
+      *reinterpret_cast<__nv_bfloat162*>(sp.lo + o) = l2[0];
+    }
+#pragma unroll
+    for (int s2 = 16; s2 > 0; s2 >>= 1) q += __shfl_xor_sync(0xffffffffu, q, s2);
+    if (lane == 0) sp.musq[(size_t)bh * g.Nc + u] = q;
+  }
 }
 
 size_t assign_smem_bytes(const HvaGrid& g, int D, int esize) {
@@ -334,7 +385,7 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
       hva_assign_kernel<T, D><<<grid, kThreads, smem, st>>>(p);
       HVA_CHECK_LAUNCH();
     }
-    hva_finalize_kernel<D><<<grid, D, 0, st>>>(g, ws.part, ws.part_cnt, mu, sizes, last ? sums : nullptr, last ? none : sp, tc ? atc.csplit : 1);
+    hva_finalize_kernel<D><<<dim3((g.Nc + kFinWarps - 1) / kFinWarps, BH), 32 * kFinWarps, 0, st>>>(g, ws.part, ws.part_cnt, mu, sizes, last ? sums : nullptr, last ? none : sp, tc ? atc.csplit : 1);
     HVA_CHECK_LAUNCH();
   }
   return HVA_OK;
