@@ -142,9 +142,10 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--top-p", type=float, default=None)
     ap.add_argument("--merge-rounds", type=int, default=None)
-    ap.add_argument("--report", default=None, choices=[None, "sweep", "hybrid"],
+    ap.add_argument("--report", default=None, choices=[None, "sweep", "hybrid", "selfbase"],
                     help="extra reports of BASELINE.json configs[3] / configs[4] instead of the bench line: 'sweep' = top-p x merging "
-                         "with CTA tile occupancy, 'hybrid' = the 50-step anchor / subset sequence (use --config C5)")
+                         "with CTA tile occupancy, 'hybrid' = the 50-step anchor / subset sequence (use --config C5), 'selfbase' = "
+                         "on-box self-baselines: the dense (HVA_DENSE) call next to the sparse one, clustering over window sizes")
     ap.add_argument("--seq-steps", type=int, default=50)
     ap.add_argument("--cell-q", default=None, help="k_t,k_h,k_w of the Q grid (default: the workload's); e.g. the paper's 11,5,5")
     ap.add_argument("--cell-k", default=None, help="k_t,k_h,k_w of the K grid; e.g. the paper's 11,3,3")
@@ -165,6 +166,8 @@ def main():
         return report_sweep(b, wl, args)
     if args.report == "hybrid":
         return report_hybrid(b, wl, args)
+    if args.report == "selfbase":
+        return report_selfbase(b, wl, args)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -275,6 +278,46 @@ def report_sweep(b, wl, args):
                               "executed_tflop": round(exec_flop / 1e12, 2), "dense_equiv_tflops_call": round(4.0 * BH * n * n * D / (ms * 1e-3) / 1e12, 1),
                               "occupancy": {k: (round(v, 4) if isinstance(v, float) else v) for k, v in occ.items()}}))
             del fwd
+
+
+def report_selfbase(b, wl, args):
+    """(a) the dense tcgen05 FlashAttention call (HVA_DENSE: what warm-up steps / layers run,
+    l.324) next to the sparse call on the same inputs and box -> an on-box speed-up figure (the paper's own: Table 1 / l.11,
+    other hardware); (b) hva_cluster of one tensor over window sizes (our analogue of Fig. 4b, l.85)."""
+    Q, K, V = [t.cuda().contiguous() for t in inputs.make_qkv(wl)]
+    shape = b.make_shape(wl)
+    O = torch.empty_like(Q)
+    BH, n, D = wl.B * wl.heads, wl.n, wl.D
+    reps = max(args.steps, 3)
+    fwd = b.Forward(shape, b.make_config(wl, top_p=args.top_p, merge_rounds=args.merge_rounds, min_kc=args.min_kc))
+    for _ in range(2):
+        fwd(Q, K, V, O)
+    ms_sparse = ev_time(lambda: fwd(Q, K, V, O), reps)
+    fwd(Q, K, V, O, step_kind=b.HVA_DENSE)
+    ms_dense = ev_time(lambda: fwd(Q, K, V, O, step_kind=b.HVA_DENSE), reps)
+    dense_flop = 4.0 * BH * float(n) * n * D
+    print(json.dumps({"report": "selfbase", "workload": wl.name, "top_p": float(fwd.cfg.top_p), "merge_rounds": int(fwd.cfg.merge_rounds),
+                      "sparse_ms_per_call": round(ms_sparse, 3), "dense_ms_per_call": round(ms_dense, 3),
+                      "dense_tflops": round(dense_flop / (ms_dense * 1e-3) / 1e12, 1), "speedup_over_dense": round(ms_dense / ms_sparse, 3)}))
+    del fwd
+    K3 = [-(-d // k) for d, k in zip((wl.T, wl.H, wl.W), wl.cell)]
+    for win in ((1, 1, 1), (3, 3, 3), (3, 5, 5), (5, 5, 5), (3, 8, 8)):
+        nwin = 1
+        for w_, k_ in zip(win, K3):
+            nwin *= min(w_, k_)
+        run = lambda: b.hva_cluster(shape, wl.cell, win, wl.iters, K, want_sums=False, want_lowe=False)
+        out = run()
+        ms = ev_time(run, reps)
+        # k-means objective per token (fp64 on the device, from the labels and centroids the call returned)
+        J = 0.0
+        for h in range(BH):
+            x = K.view(BH, n, D)[h].double()
+            J += float(((x - out["mu"][h].double()[out["assign"][h].long()]) ** 2).sum())
+        gb = wl.iters * BH * n * D * K.element_size() + BH * n * 4
+        print(json.dumps({"report": "selfbase-window", "workload": wl.name, "tensor": "K", "win": list(win), "candidates": nwin,
+                          "iters": wl.iters, "ms": round(ms, 3), "algorithmic_GBps": round(gb / (ms * 1e-3) / 1e9, 1),
+                          "objective_per_token": round(J / (BH * n), 5)}))
+        del out
 
 
 def report_hybrid(b, wl, args):
