@@ -112,6 +112,25 @@ def oracle_sample(wl, head=0, attn_rows=32, merge_rounds=None):
     return t, per_head * wl.heads * 1e3
 
 
+def oracle_threads():
+    """Threads the oracle actually uses: it is single-process numpy, so its BLAS pool (else 1)."""
+    try:
+        from threadpoolctl import threadpool_info
+        return max([int(i.get("num_threads", 1)) for i in threadpool_info()] or [1])
+    except Exception:
+        return 1
+
+
+def workload_config(wl, cell_q, cell_k, win, min_kc, top_p, merge_rounds, custom=False):
+    """The `config` object of the JSON line: the same keys for both arms."""
+    in_gb = 3 * wl.B * wl.heads * wl.n * wl.D * (2 if wl.dtype == "bf16" else 4) / 1e9
+    return {"workload": wl.name + ("+custom-grids" if custom else ""), "B": wl.B, "heads": wl.heads, "n": wl.n, "D": wl.D,
+            "cell_q": list(cell_q), "cell_k": list(cell_k), "win": list(win), "min_kc": min_kc, "iters": wl.iters,
+            "top_p": top_p, "merge_rounds": merge_rounds, "tile": wl.tile,
+            "l2": "inputs (%.2g GB) %s L2" % (in_gb, "larger than" if in_gb > 0.3 else "NOT larger than"),
+            "parallelism": "head-sharded replicas, no collective"}
+
+
 def run_reference(args, wl):
     """--impl reference: the oracle timed on the host cores, each step a bounded sample, extrapolated to ms/call."""
     rank = int(os.environ.get("RANK", "0"))
@@ -123,12 +142,13 @@ def run_reference(args, wl):
         if i >= args.warmup:
             vals.append(ms)
     v = float(np.mean(vals))
-    cores = os.cpu_count()
+    cores = oracle_threads()
     sample = ("per step: one head of %s through oracle clustering (Q,K), mask, 1 merge round, plan and 16 attention rows; "
               "extrapolated x heads and x n/16 rows" % wl.name)
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-                      "dtype": "f64", "data": "synthetic", "config": {"workload": wl.name},
+                      "dtype": "f64", "data": "synthetic",
+                      "config": workload_config(wl, wl.cell, wl.cell, wl.win, 0.0, float(np.float32(wl.top_p)), wl.merge_rounds),
                       "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample},
                       "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
@@ -222,10 +242,8 @@ def main():
     out = {"metric": METRIC, "value": sharding.whole_job_value(ms, world), "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
            "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
-           "config": {"workload": wl.name + ("+custom-grids" if custom else ""), "B": wl.B, "heads": wl.heads, "n": wl.n, "D": wl.D,
-                      "cell_q": list(cfg.cell_q), "cell_k": list(cfg.cell_k), "win": list(cfg.win_q), "min_kc": float(cfg.min_kc), "iters": wl.iters,
-                      "top_p": float(cfg.top_p), "merge_rounds": int(cfg.merge_rounds), "tile": wl.tile,
-                      "l2": "inputs (2.2 GB) larger than L2", "parallelism": "head-sharded replicas, no collective"},
+           "config": workload_config(wl, list(cfg.cell_q), list(cfg.cell_k), list(cfg.win_q), float(cfg.min_kc), float(cfg.top_p),
+                                     int(cfg.merge_rounds), custom),
            "clocks": clocks,
            "e2e": {"value": e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
            "gpu_launches": args.steps * (2 * (2 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 7 + 3 + 1)}
@@ -235,7 +253,7 @@ def main():
         out.update(stage_report(b, wl, shape, cfg, Q, K, V, stats, pk))
     if rank == 0 and not args.no_cpu_baseline and not custom:
         t, cpu_ms = oracle_sample(wl, attn_rows=32, merge_rounds=1 if wl.n > 50000 else None)
-        out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": os.cpu_count(), "kind": "oracle",
+        out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": oracle_threads(), "kind": "oracle",
                                "sample": "one head of %s: oracle clustering Q,K %.1fs, mask %.2fs, merge(1 round) %.1fs, plan %.2fs, "
                                          "32 attention rows %.2fs; extrapolated x%d heads, x n/32 rows" % (
                                              wl.name, t["cluster"], t["mask"], t["merge"], t["plan"], t["attn_rows"], wl.heads)}
