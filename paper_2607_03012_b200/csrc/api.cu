@@ -216,8 +216,18 @@ extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const v
   const size_t bytes = (size_t)s->B * s->heads * head_bytes;
   char* d = reinterpret_cast<char*>(dev_qkvo);
   static HostPipe pipe;
-  int nchunk = 1;
-  if (pipe.ok && !state && s->B == 1 && s->heads >= 8) nchunk = 4;   // 8 chunks measured the same (91.4 vs 91.2-92.4 ms at C4)
+  // chunk boundaries: the first chunk's H2D copy and the last chunk's D2H copy are the only transfers no kernel covers, so
+  // both end chunks are small (heads / 12) and the heads between them go in three equal parts
+  int nchunk = 1, bound[8] = {0, s->heads};
+  if (pipe.ok && !state && s->B == 1 && s->heads >= 8) {
+    const int edge = s->heads / 12 > 0 ? s->heads / 12 : 1, mid = s->heads - 2 * edge;
+    nchunk = 5;
+    bound[1] = edge;
+    bound[2] = edge + mid / 3;
+    bound[3] = edge + (2 * mid) / 3;
+    bound[4] = edge + mid;
+    bound[5] = s->heads;
+  }
   if (nchunk == 1) {
     if (cudaMemcpyAsync(d, hQ, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
     if (cudaMemcpyAsync(d + bytes, hK, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
@@ -232,9 +242,8 @@ extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const v
       cudaStreamWaitEvent(pipe.d2h, pipe.start, 0) != cudaSuccess)
     return HVA_ECUDA;
   const char* src[3] = {(const char*)hQ, (const char*)hK, (const char*)hV};
-  int h0 = 0;
   for (int i = 0; i < nchunk; ++i) {
-    const int h1 = (int)((long long)s->heads * (i + 1) / nchunk), nh = h1 - h0;
+    const int h0 = bound[i], h1 = bound[i + 1], nh = h1 - h0;
     const size_t off = (size_t)h0 * head_bytes, cb = (size_t)nh * head_bytes;
     for (int t = 0; t < 3; ++t)
       if (cudaMemcpyAsync(d + t * bytes + off, src[t] + off, cb, cudaMemcpyHostToDevice, pipe.h2d) != cudaSuccess) return HVA_ECUDA;
@@ -247,7 +256,6 @@ extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const v
     if (cudaEventRecord(pipe.out_ready[i], st) != cudaSuccess || cudaStreamWaitEvent(pipe.d2h, pipe.out_ready[i], 0) != cudaSuccess)
       return HVA_ECUDA;
     if (cudaMemcpyAsync((char*)hO + off, d + 3 * bytes + off, cb, cudaMemcpyDeviceToHost, pipe.d2h) != cudaSuccess) return HVA_ECUDA;
-    h0 = h1;
   }
   if (cudaStreamSynchronize(pipe.d2h) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return HVA_ECUDA;
   return HVA_OK;
