@@ -185,8 +185,10 @@ int hva_forward(const hva_shape* s, const hva_config* c, const void* Q, const vo
 
 /* Same as hva_forward with HOST Q,K,V,O (pinned or pageable); allocates nothing: `dev_qkvo` is a
  * caller-owned DEVICE staging buffer of 4*B*heads*n*D elements.  Heads are independent, so with B = 1, >= 8 heads and no
- * hybrid state the call runs in 4 chunks of heads: the copies of the neighbouring chunks (two library-owned copy streams,
- * both PCIe directions; pinned host buffers needed for the overlap) run under the kernels of the current one.
+ * hybrid state the call runs in 5 chunks of heads (two small end chunks of heads/12 heads, three equal parts between them:
+ * only the first chunk's H2D copy and the last chunk's D2H copy are not covered by kernels): the copies of the neighbouring
+ * chunks (two library-owned copy streams, both PCIe directions; pinned host buffers needed for the overlap) run under the
+ * kernels of the current one.  Chunked and unchunked calls give the same bits (the merge hash is keyed by the global head).
  * Synchronises the stream. */
 int hva_forward_host(const hva_shape* s, const hva_config* c, const void* hQ, const void* hK,
                      const void* hV, void* hO, int32_t step_kind, void* state, void* dev_qkvo,
