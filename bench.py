@@ -162,7 +162,7 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--top-p", type=float, default=None)
     ap.add_argument("--merge-rounds", type=int, default=None)
-    ap.add_argument("--report", default=None, choices=[None, "sweep", "hybrid", "selfbase"],
+    ap.add_argument("--report", default=None, choices=[None, "sweep", "hybrid", "selfbase", "assign-phases"],
                     help="extra reports of BASELINE.json configs[3] / configs[4] instead of the bench line: 'sweep' = top-p x merging "
                          "with CTA tile occupancy, 'hybrid' = the 50-step anchor / subset sequence (use --config C5), 'selfbase' = "
                          "on-box self-baselines: the dense (HVA_DENSE) call next to the sparse one, clustering over window sizes")
@@ -188,6 +188,8 @@ def main():
         return report_hybrid(b, wl, args)
     if args.report == "selfbase":
         return report_selfbase(b, wl, args)
+    if args.report == "assign-phases":
+        return report_assign_phases(b, wl, args)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -336,6 +338,34 @@ def report_selfbase(b, wl, args):
                           "iters": wl.iters, "ms": round(ms, 3), "algorithmic_GBps": round(gb / (ms * 1e-3) / 1e9, 1),
                           "objective_per_token": round(J / (BH * n), 5)}))
         del out
+
+
+def report_assign_phases(b, wl, args):
+    """Per-phase clock64 breakdown of hva_assign_tc_kernel.  Diagnostic, not a bench number: needs the library built with
+    `HVA_NVCC_FLAGS=-DHVA_ASSIGN_TIMING python paper_2607_03012_b200/build.py --force` (thread 0 of every CTA adds its clocks per
+    phase to the HVA_CLUSTER_PROBE buffer); the product build leaves the buffer at zero and this report says so."""
+    heads = list(range(min(8, wl.heads)))
+    _, K, _ = inputs.make_qkv(wl, heads=heads)
+    X = K.cuda().contiguous()
+    shape = b.make_shape(wl, heads=len(heads))
+    names = ["setup", "tile_wait", "xsq", "mma1_wait", "epilogue", "scan_refine_store", "sync", "onehot_fence", "sums_mma", "end_sync"]
+    cells = 1
+    for d, k in zip((wl.T, wl.H, wl.W), wl.cell):
+        cells *= -(-d // k)
+    for lowe, iters in ((False, 1), (True, 1), (False, wl.iters)):
+        b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe, want_sums=False)
+        probe = torch.zeros(32, dtype=torch.float32, device="cuda")
+        os.environ["HVA_CLUSTER_PROBE"] = str(probe.data_ptr())
+        try:
+            b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe, want_sums=False)
+            torch.cuda.synchronize()
+        finally:
+            del os.environ["HVA_CLUSTER_PROBE"]
+        pr = probe.cpu().numpy()
+        ntiles = cells * len(heads) * iters
+        clk = {n: int(round(float(pr[16 + k]) / ntiles)) for k, n in enumerate(names)}
+        print(json.dumps({"report": "assign-phases", "workload": wl.name, "heads": len(heads), "iters": iters, "lowe_ratio": lowe,
+                          "timing_build": bool(pr[16:26].sum() > 0), "clk_per_tile": clk, "clk_per_tile_sum": int(sum(clk.values()))}))
 
 
 def report_hybrid(b, wl, args):

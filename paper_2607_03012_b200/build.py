@@ -12,6 +12,9 @@ LIB = os.path.join(HERE, "libhva.so")
 SOURCES = ["api.cu", "cluster.cu", "cluster_tc.cu", "hybrid.cu", "hybrid_tc.cu", "mask.cu", "merge.cu", "merge_tc.cu", "plan.cu", "attn_simt.cu", "attn_tc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
+# extra nvcc flags for diagnostic builds, e.g. HVA_NVCC_FLAGS=-DHVA_ASSIGN_TIMING (per-phase clock64 build of the assignment
+# kernel read by `bench.py --report assign-phases`); use --force, and rebuild without it afterwards
+FLAGS += os.environ.get("HVA_NVCC_FLAGS", "").split()
 
 
 def _stale(out, deps):
