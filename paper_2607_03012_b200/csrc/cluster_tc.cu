@@ -45,6 +45,7 @@ struct AssignTcParams {
   uint32_t m_khw, m_kw, m_whw, m_ww;   // fast_div multipliers for k_h k_w, k_w, w_h w_w, w_w
   uint32_t tmem_cols;
   int one_pass;        // 2 npad <= 256: one MMA pass over [hi; lo] stacked as 2 npad score columns (the token tile is read once)
+  unsigned long long d_khw, d_kw, d_cs, d_kt;   // fast_div64 multipliers of the tile decode: K_h K_w, K_w, csplit, K_t
   int n_items;         // K_w * K_h * K_t * BH * csplit tiles: a CTA starts with tile blockIdx.x and draws the following ones
   int* counter;        // from this device counter (zero at launch), so that the SMs finish together
   float* probe;        // debug: max |score_tc - score_exact| / (|x| max|mu|), or null
@@ -68,6 +69,9 @@ __device__ __noinline__ float direct_dist_probe(const unsigned char* sA, int hal
 
 // x / d for 0 <= x, x * d < 2^32 by one multiply-high (m = ceil(2^32 / d); d == 1 is passed as m = 0)
 __device__ __forceinline__ int fast_div(int x, uint32_t m) { return m ? (int)__umulhi((uint32_t)x, m) : x; }
+// x / d for every 0 <= x < 2^31 and d >= 1 by one 64-bit multiply-high (m = ceil(2^64 / d); d == 1 is passed as m = 0):
+// m d = 2^64 + e with e < d, so x m / 2^64 = x / d + x e / (d 2^64), and the excess is below 2^-32 < 1 / d
+__device__ __forceinline__ int fast_div64(int x, unsigned long long m) { return m ? (int)__umul64hi((unsigned long long)(uint32_t)x, m) : x; }
 
 // Persistent CTAs (as many as fit the SMs, 4 per SM at the 3x5x8 cells) draw the tiles (home cell x time split) in raster
 // order from a device counter; 128 threads, thread = token row of the tile = TMEM lane.  Per-CTA set-up (TMEM allocation,
@@ -112,11 +116,12 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
   struct Tile { int uw, uh, ut, bh, chunk; };
   auto decode = [&](int item) {
     Tile t;
-    const int khw = g.Kw * g.Kh, z = item / khw, r = item - z * khw;
-    t.uh = r / g.Kw; t.uw = r - t.uh * g.Kw;
-    t.chunk = z % p.csplit;
-    const int zz = z / p.csplit;
-    t.bh = zz / g.Kt; t.ut = zz - t.bh * g.Kt;
+    // (a runtime integer division is ~45 instructions; the decode runs twice per tile and warp: 14 % of the kernel's instructions)
+    const int khw = g.Kw * g.Kh, z = fast_div64(item, p.d_khw), r = item - z * khw;
+    t.uh = fast_div64(r, p.d_kw); t.uw = r - t.uh * g.Kw;
+    const int zz = fast_div64(z, p.d_cs);
+    t.chunk = z - zz * p.csplit;
+    t.bh = fast_div64(zz, p.d_kt); t.ut = zz - t.bh * g.Kt;
     return t;
   };
   // the six boxes of a tile, two per call: part 0 = tokens, part 1 = hi, part 2 = lo (a 5-D box costs its issuing thread
@@ -511,8 +516,10 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
                          int* part_cnt, int* assign, float* lowe, int* counter, float* probe, cudaStream_t st) {
   auto magic = [](int d) -> uint32_t { return d <= 1 ? 0u : (uint32_t)(((1ull << 32) + d - 1) / d); };
+  auto magic64 = [](int d) -> unsigned long long { return d <= 1 ? 0ull : ~0ull / (unsigned long long)d + 1ull; };
   AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, a.npad, a.rows_a, a.csplit, a.ct, magic(g.kh * g.kw), magic(g.kw), magic(g.wh * g.ww),
-                   magic(g.ww), a.tmem_cols, a.one_pass, g.Kw * g.Kh * g.Kt * BH * a.csplit, counter, probe};
+                   magic(g.ww), a.tmem_cols, a.one_pass, magic64(g.Kw * g.Kh), magic64(g.Kw), magic64(a.csplit), magic64(g.Kt),
+                   g.Kw * g.Kh * g.Kt * BH * a.csplit, counter, probe};
   if (cudaMemsetAsync(counter, 0, sizeof(int), st) != cudaSuccess) return HVA_ECUDA;
   hva_assign_tc_kernel<<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   HVA_CHECK_LAUNCH();
