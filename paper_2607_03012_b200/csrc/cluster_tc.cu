@@ -155,6 +155,12 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
     const int r = ctok + (i >> 4), q = i & 15;
     *reinterpret_cast<uint4*>(sA + (q >> 3) * half_a + r * 128 + ((q & 7) << 4)) = make_uint4(0, 0, 0, 0);
   }
+  // rows nwin .. npad-1 of the four centroid tiles (hi | lo per 64-dim half) are never written by TMA: zero them once, so that the
+  // pad columns of the score MMA are exactly 0 (the one-hot tile that aliases the first half only ever sets rows < nwin)
+  for (int i = tid; i < 4 * (npad - nwin) * 8; i += kThreads) {
+    const int k = i / ((npad - nwin) * 8), j = i - k * (npad - nwin) * 8;
+    *reinterpret_cast<uint4*>(smem + k * half_b + nwin * 128 + j * 16) = make_uint4(0, 0, 0, 0);
+  }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   // position of this thread's token inside a tile
   const int li = tid;
@@ -173,7 +179,7 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
   for (int v = tid - 32; v < npad; v += kThreads - 32) {
     if (v < 0) continue;
     int u = 0;
-    float c = 0.f;
+    float c = kInf;     // pad slot: its score column is exactly 0 (pad rows of the centroid tiles are zero), so score = +inf
     if (v < nwin) {
       const int dt = fast_div(v, p.m_whw), r = v - dt * g.wh * g.ww, dh = fast_div(r, p.m_ww), dw = r - dh * g.ww;
       u = ((st + dt) * g.Kh + (sh + dh)) * g.Kw + (sw + dw);
@@ -218,10 +224,14 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
     if (li < ctok && dt0 + ldt < g.kt && t < g.T && h < g.H && w < g.W) { lab = 0; tok = (size_t)(t * g.H + h) * g.W + w; }
   }
   const bool valid = lab == 0;
-  float c_max = 0.f;
-  for (int v = 0; v < npad; v += 4) {
-    const float4 c4 = *reinterpret_cast<const float4*>(s_c + v);
-    c_max = fmaxf(fmaxf(c_max, fmaxf(c4.x, c4.y)), fmaxf(c4.z, c4.w));
+  float c_max = 0.f;      // over the window's slots only: the pad slots hold +inf
+  {
+    int v = 0;
+    for (; v + 4 <= nwin; v += 4) {
+      const float4 c4 = *reinterpret_cast<const float4*>(s_c + v);
+      c_max = fmaxf(fmaxf(c_max, fmaxf(c4.x, c4.y)), fmaxf(c4.z, c4.w));
+    }
+    for (; v < nwin; ++v) c_max = fmaxf(c_max, s_c[v]);
   }
   mbar_wait(&B->full, ph);
   CMARK(1);
@@ -232,13 +242,22 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
     __nv_bfloat162 acc[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[j] = __floats2bfloat162_rn(0.f, 0.f);
-#pragma unroll 8
-    for (int q = 0; q < 16; ++q) {
-      const uint4 r = *x_chunk(sA, half_a, li, q);
+    // chunk q of row li sits at row + (((q & 7) ^ (li & 7)) << 4): the row is 128-byte aligned, so the swizzle is one XOR on
+    // (row | (li & 7) << 4); 32-bit shared-space addresses keep the address arithmetic at one instruction per load
+    const uint32_t xa0 = smem_u32(sA) + (uint32_t)li * 128u + ((uint32_t)(li & 7) << 4), xa1 = xa0 + (uint32_t)half_a;
+#pragma unroll 1
+    for (int hh = 0; hh < 2; ++hh) {
+    const uint32_t xa = hh ? xa1 : xa0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      uint4 r;
+      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                   : "r"(xa ^ ((uint32_t)q << 4)));
       const __nv_bfloat162 x0 = *reinterpret_cast<const __nv_bfloat162*>(&r.x), x1 = *reinterpret_cast<const __nv_bfloat162*>(&r.y),
                            x2 = *reinterpret_cast<const __nv_bfloat162*>(&r.z), x3 = *reinterpret_cast<const __nv_bfloat162*>(&r.w);
       acc[0] = __hfma2(x0, x0, acc[0]); acc[1] = __hfma2(x1, x1, acc[1]);
       acc[2] = __hfma2(x2, x2, acc[2]); acc[3] = __hfma2(x3, x3, acc[3]);
+    }
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j) xsq += __low2float(acc[j]) + __high2float(acc[j]);
@@ -273,13 +292,18 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
       } else {
         tmem_ld16(trow + v0 + h, raw);
       }
+      if (v0 + h >= npad) {      // a whole 16-column granule past the padded window (npad is a multiple of 16): warp-uniform
 #pragma unroll
-      for (int j = 0; j < 16; j += 4) {
-        const float4 c4 = *reinterpret_cast<const float4*>(s_c + v0 + h + j);   // npad is a multiple of 16
-        sv[h + j] = v0 + h + j < nwin ? fmaf(-2.f, __uint_as_float(raw[j]), c4.x) : kInf;
-        sv[h + j + 1] = v0 + h + j + 1 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 1]), c4.y) : kInf;
-        sv[h + j + 2] = v0 + h + j + 2 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 2]), c4.z) : kInf;
-        sv[h + j + 3] = v0 + h + j + 3 < nwin ? fmaf(-2.f, __uint_as_float(raw[j + 3]), c4.w) : kInf;
+        for (int j = 0; j < 16; ++j) sv[h + j] = kInf;
+        continue;
+      }
+#pragma unroll
+      for (int j = 0; j < 16; j += 4) {      // pad slots nwin .. npad-1: column 0, |mu|^2 = +inf  =>  +inf without a compare
+        const float4 c4 = *reinterpret_cast<const float4*>(s_c + v0 + h + j);
+        sv[h + j] = fmaf(-2.f, __uint_as_float(raw[j]), c4.x);
+        sv[h + j + 1] = fmaf(-2.f, __uint_as_float(raw[j + 1]), c4.y);
+        sv[h + j + 2] = fmaf(-2.f, __uint_as_float(raw[j + 2]), c4.z);
+        sv[h + j + 3] = fmaf(-2.f, __uint_as_float(raw[j + 3]), c4.w);
       }
     }
   };
