@@ -55,6 +55,7 @@ struct __align__(8) AssignTcBars {
   uint64_t full, mma_done, sum_done;
   uint32_t tmem_base;
   int next;
+  uint32_t cmax[4];     // per warp: max |mu_v|^2 over the window slots it set up (bits of a non-negative float)
 };
 
 __device__ __noinline__ float direct_dist_probe(const unsigned char* sA, int half_bytes, int r, const float* mu) {
@@ -170,12 +171,17 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
 
   for (int item = blockIdx.x, next_item = 0; item < p.n_items; item = next_item, ph ^= 1u) {
   const Tile T = decode(item);
-  if (tid == 96) B->next = (int)gridDim.x + atomicAdd(p.counter, 1);   // the tile after this one; published by the barrier below
+  if (tid == 96) {   // the tile after this one; published by the barrier below (a plain atomicAdd is wrapped in the compiler's
+    int got;         // warp-aggregation sequence in all four warps: 28 instructions per warp and tile)
+    asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(got) : "l"(p.counter) : "memory");
+    B->next = (int)gridDim.x + got;
+  }
   const int uw = T.uw, uh = T.uh, ut = T.ut, bh = T.bh, chunk = T.chunk;
   const int dt0 = chunk * p.ct;                        // first time slice of this tile inside the cell
   const int cell = (ut * g.Kh + uh) * g.Kw + uw;
   const int st = hva_win_start(ut, g.wt, g.Kt), sh = hva_win_start(uh, g.wh, g.Kh), sw = hva_win_start(uw, g.ww, g.Kw);
   // window slot -> centroid id (ascending == delta_t-major, Alg. 2 line 18), |mu|^2   (warps 1..3)
+  float cm = 0.f;
   for (int v = tid - 32; v < npad; v += kThreads - 32) {
     if (v < 0) continue;
     int u = 0;
@@ -185,7 +191,12 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
       u = ((st + dt) * g.Kh + (sh + dh)) * g.Kw + (sw + dw);
       c = __ldg(p.musq + (size_t)bh * g.Nc + u);
     }
+    if (v < nwin) cm = fmaxf(cm, c);
     s_u[v] = u; s_c[v] = c; s_cnt[v] = 0;
+  }
+  {   // max |mu_v|^2 of the window: one redux per warp instead of every thread scanning s_c (|mu|^2 >= 0: uint order == float order)
+    const uint32_t m = __reduce_max_sync(0xffffffffu, __float_as_uint(cm));
+    if (lane == 0) B->cmax[warp] = m;
   }
   tc_fence_before();
   __syncthreads();
@@ -224,15 +235,9 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
     if (li < ctok && dt0 + ldt < g.kt && t < g.T && h < g.H && w < g.W) { lab = 0; tok = (size_t)(t * g.H + h) * g.W + w; }
   }
   const bool valid = lab == 0;
-  float c_max = 0.f;      // over the window's slots only: the pad slots hold +inf
-  {
-    int v = 0;
-    for (; v + 4 <= nwin; v += 4) {
-      const float4 c4 = *reinterpret_cast<const float4*>(s_c + v);
-      c_max = fmaxf(fmaxf(c_max, fmaxf(c4.x, c4.y)), fmaxf(c4.z, c4.w));
-    }
-    for (; v < nwin; ++v) c_max = fmaxf(c_max, s_c[v]);
-  }
+  // over the window's slots only (the pad slots hold +inf); written before the first barrier of the tile
+  const float c_max = fmaxf(fmaxf(__uint_as_float(B->cmax[0]), __uint_as_float(B->cmax[1])),
+                            fmaxf(__uint_as_float(B->cmax[2]), __uint_as_float(B->cmax[3])));
   mbar_wait(&B->full, ph);
   CMARK(1);
   // |x|^2 only scales the margin: packed bf16 FMAs (4 x 2 accumulators of 16 non-negative terms each: relative
