@@ -25,8 +25,8 @@ sys.path.insert(0, ROOT)
 from paper_2607_03012_b200 import inputs, sharding  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one hva_attn_tc_kernel launch at C4 (top-p 0.9, merging on), from the `ncu --set full`
-# capture summarised in profiles/r1d_ncu_full.md (11.60 GB + 0.78 GB); algorithmic minimum 2.9 GB (Q', K', V' once + O)
-ATTN_DRAM_BYTES_C4 = 12.38e9
+# capture summarised in profiles/r1f_ncu_full.md (11.72 GB + 0.78 GB); algorithmic minimum 2.9 GB (Q', K', V' once + O)
+ATTN_DRAM_BYTES_C4 = 12.49e9
 
 METRIC = "sparse-attn ms/call + clustering ms/step at 118,800-token HunyuanVideo shape"
 
