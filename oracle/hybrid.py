@@ -13,10 +13,15 @@ CURRENT features; mu_u <- z_u / n_u for touched u with n_u > 0; no non-subset to
 R-H3' (`refresh_all`): after the reassignment every centroid is recomputed as the mean of the
 CURRENT features of its members.
 
-PARITY UNPINNED for `subset_update` (the paper gives no formula for the centroid
-adjustment).  Pins that do exist (tests/test_oracle_hybrid.py): f = 1 with refresh_all ==
-one textbook global k-means step (brute force); unchanged X + already optimal labels ->
-no-op; counts stay consistent; non-subset labels untouched; subset size and ordering.
+Pins (tests/test_oracle_plan_attn_hybrid.py): `select_subset` -- hand ties, order statistics.
+`subset_update(refresh_all=True)` -- f = 1 is one textbook global k-means step (brute force).
+`subset_update(refresh_all=False)` -- with UNCHANGED X (cached sums are then exact member sums) the
+incrementally adjusted sums / sizes / mu of every touched centroid equal a from-scratch
+recomputation over the new labels, on a lattice whose window does not cover the grid so that
+subset tokens do move; unchanged X + already optimal labels -> no-op; counts stay consistent;
+non-subset labels untouched.  What the paper does NOT pin is the READING itself (R-H3: which
+centroids "the corresponding centroids" are and with which features they are adjusted); the
+arithmetic of the reading is pinned by the identities above.
 """
 from __future__ import annotations
 

@@ -140,3 +140,51 @@ def test_subset_update_noop_and_consistency():
             assert np.allclose(mu[u], z[u] / n[u])
         else:
             assert np.array_equal(mu[u], c["mu"][u])
+
+
+def test_subset_update_incremental_equals_recomputation_when_x_is_unchanged():
+    """Pin of the R-H3 branch (refresh_all=False; P:101 'updating the corresponding centroids'): with UNCHANGED features the
+    cached sums are exactly the member sums of the cached labels, so after the subset has been re-assigned against the
+    full centroid set the incrementally adjusted sums / sizes / mu of every touched centroid must equal a from-scratch
+    recomputation over the NEW labels (and every untouched centroid keeps its members, hence its mean).  The lattice is
+    chosen so that the (2,3,3) window does not cover the (2,4,8) grid: local-window labels are not globally optimal and
+    subset tokens do move.  A forgotten subtraction, a wrong sign, the wrong feature row or a wrong 'moved' test fails it."""
+    import dataclasses
+    wl = dataclasses.replace(inputs.C1, name="pin-h3", heads=1, D=64, T=4, H=8, W=16, cell=(2, 2, 2), win=(3, 3, 3), seed=17,
+                             noise=0.8)
+    X = inputs.to_f64(inputs.make_head(wl, 0)[1])
+    lat = (wl.T, wl.H, wl.W)
+    c = oracle.local_window_kmeans(X, lat, wl.cell, wl.win, 2)
+    Nc = len(c["sizes"])
+    assert Nc == 64
+    # the cached state is self-consistent: sums = member sums, mu = member means (Alg. 2 l.21-23)
+    z0 = np.zeros_like(c["sums"]); np.add.at(z0, c["assign"], X)
+    assert np.allclose(z0, c["sums"], rtol=1e-13, atol=1e-13)
+    for frac in (0.15, 0.5, 1.0):
+        sub = oracle.select_subset(oracle.lowe_ratio(c["d1sq"], c["d2sq"]), frac)
+        a, mu, z, n, d1, d2 = oracle.subset_update(X, c["assign"], c["mu"], c["sums"], c["sizes"], sub, refresh_all=False)
+        moved = sub[a[sub] != c["assign"][sub]]
+        assert len(moved) > 0, "the pin needs tokens that move (window must not cover the grid)"
+        # the re-assignment itself: global first minimum for subset tokens, everything else untouched
+        dall = ((X[sub][:, None, :] - c["mu"][None]) ** 2).sum(-1)
+        assert np.array_equal(a[sub], dall.argmin(1))
+        rest = np.setdiff1d(np.arange(wl.n), sub)
+        assert np.array_equal(a[rest], c["assign"][rest])
+        # from-scratch recomputation over the new labels
+        n_ref = np.bincount(a, minlength=Nc)
+        z_ref = np.zeros((Nc, wl.D)); np.add.at(z_ref, a, X)
+        assert np.array_equal(n, n_ref)
+        assert np.allclose(z, z_ref, rtol=1e-12, atol=1e-11)
+        touched = np.unique(np.concatenate([a[moved], c["assign"][moved]]))
+        for u in range(Nc):
+            if n_ref[u] > 0:
+                assert np.allclose(mu[u], X[a == u].mean(0), rtol=1e-11, atol=1e-12), u
+            if u not in touched:
+                assert np.array_equal(mu[u], c["mu"][u])           # untouched centroids are not rewritten
+            elif n_ref[u] == 0:
+                assert np.array_equal(mu[u], c["mu"][u])           # emptied cluster keeps mu (Alg. 2 l.23)
+        # and it agrees with the R-H3' branch on unchanged X (both are then exact member statistics)
+        a2, mu2, z2, n2, _, _ = oracle.subset_update(X, c["assign"], c["mu"], c["sums"], c["sizes"], sub, refresh_all=True)
+        assert np.array_equal(a2, a) and np.array_equal(n2, n)
+        nz = n > 0
+        assert np.allclose(mu2[nz], mu[nz], rtol=1e-11, atol=1e-12)
