@@ -343,7 +343,7 @@ def report_selfbase(b, wl, args):
 def report_assign_phases(b, wl, args):
     """Per-phase clock64 breakdown of hva_assign_tc_kernel.  Diagnostic, not a bench number: needs the library built with
     `HVA_NVCC_FLAGS=-DHVA_ASSIGN_TIMING python paper_2607_03012_b200/build.py --force` (thread 0 of every CTA adds its clocks per
-    phase to the HVA_CLUSTER_PROBE buffer); the product build leaves the buffer at zero and this report says so."""
+    phase to the probe buffer of hva_cluster_ex); the product build leaves those entries at zero and this report says so."""
     heads = list(range(min(8, wl.heads)))
     _, K, _ = inputs.make_qkv(wl, heads=heads)
     X = K.cuda().contiguous()
@@ -355,12 +355,8 @@ def report_assign_phases(b, wl, args):
     for lowe, iters in ((False, 1), (True, 1), (False, wl.iters)):
         b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe, want_sums=False)
         probe = torch.zeros(32, dtype=torch.float32, device="cuda")
-        os.environ["HVA_CLUSTER_PROBE"] = str(probe.data_ptr())
-        try:
-            b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe, want_sums=False)
-            torch.cuda.synchronize()
-        finally:
-            del os.environ["HVA_CLUSTER_PROBE"]
+        b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe, want_sums=False, probe=probe)
+        torch.cuda.synchronize()
         pr = probe.cpu().numpy()
         ntiles = cells * len(heads) * iters
         clk = {n: int(round(float(pr[16 + k]) / ntiles)) for k, n in enumerate(names)}

@@ -40,6 +40,16 @@ extern "C" {
 #define HVA_INTERMEDIATE 1    /* hybrid: re-assign only the cached subset (l.101)                  */
 #define HVA_DENSE 2           /* full attention (warm-up steps/layers, l.324); no clustering       */
 
+/* Kernel-selection flags (hva_config.flags and the hva_*_ex entry points).  0 = the product path.  The flagged kernels
+ * compute the same stage with plain CUDA-core code (no tcgen05): they exist so that the tensor-pipe kernels can be
+ * cross-checked against an independent implementation ON THE DEVICE (tests/), not as a dispatch for users.  The
+ * library reads no environment variable and keeps no mutable global state besides per-device caches of CUDA function
+ * attributes and of the copy streams of hva_forward_host. */
+#define HVA_FLAG_CLUSTER_SIMT 1u    /* S1/S4: fp32 direct-form assignment on CUDA cores instead of the tcgen05 filter + refine */
+#define HVA_FLAG_ATTN_SIMT 2u       /* S9: CUDA-core attention kernel instead of the tcgen05 kernel                            */
+#define HVA_FLAG_MASK_BLOCKSORT 4u  /* S5: block-level shared-memory sort instead of the warp-per-row register sort           */
+#define HVA_FLAG_MERGE_SIMT 8u      /* S6: per-pair bit-loop union sizes instead of the tcgen05 overlap contraction           */
+
 /* Bipartition hash of Alg. 1 line 6 ("randomly bipartition", l.141; DESIGN.md R-M1):
  *   h  = seed*0x9E3779B1 ^ bh*0x85EBCA77 ^ round*0xC2B2AE3D ^ gid*0x27D4EB2F   (mod 2^32)
  *   h ^= h>>16; h *= 0x7FEB352D; h ^= h>>15; h *= 0x846CA68B; h ^= h>>16;
@@ -63,6 +73,7 @@ typedef struct {
   float subset_frac;              /* hybrid: 0 = off; the paper uses 0.15            l.322 */
   int32_t hybrid_refresh_all;     /* 0 = reading R-H3, 1 = R-H3'               */
   float softmax_scale;            /* 0 => 1/sqrt(D)                                  l.47  */
+  uint32_t flags;                 /* HVA_FLAG_* (0 = product kernels)                      */
 } hva_config;
 
 typedef struct {              /* per (batch, head); written on device by hva_build_plan */
@@ -94,6 +105,31 @@ typedef struct {              /* byte offsets of the arrays inside the opaque pl
   size_t total;               /* plan size in bytes                                            */
 } hva_plan_layout;
 
+typedef struct {              /* byte offsets of the arrays inside the hybrid `state` buffer of hva_forward; index 0 = Q, 1 = K */
+  size_t assign[2];           /* [BH,n] int32 labels                                            */
+  size_t mu[2];               /* [BH,Nc,D] fp32 centroids                                       */
+  size_t sums[2];             /* [BH,Nc,D] fp32 z                                               */
+  size_t sizes[2];            /* [BH,Nc] int32                                                  */
+  size_t subset[2];           /* [BH,max(m,1)] int32 cached subset (ascending token ids)        */
+  int32_t n_clusters[2];      /* N_q, N_k                                                       */
+  int32_t m;                  /* floor(subset_frac * n + 1/2)                                   */
+  size_t total;               /* = hva_state_bytes()                                            */
+} hva_state_layout;
+
+typedef struct {              /* byte offsets inside the workspace of hva_forward: where a caller (or a test) finds the
+                                 intermediate results of the last ANCHOR / INTERMEDIATE call; valid until the next call */
+  size_t lowe;                /* [BH,n] fp32 rho of the last clustered tensor (hybrid anchors only)            */
+  size_t mask;                /* [BH,Nq,Nk] uint8 M (Eq. 3)                                                    */
+  size_t group_of;            /* [BH,Nq] int32 gid of each query cluster (Alg. 1)                              */
+  size_t n_groups;            /* [BH] int32                                                                    */
+  size_t group_mask;          /* [BH,Nq,Nk] uint8 chi of the active groups in gid order                        */
+  size_t plan, plan_bytes;    /* the plan buffer (hva_plan_describe(BH, n, max(Nq,1), max(Nk,1), tile_q))      */
+  size_t qp, kp, vp;          /* permuted tensors Q', K', V' [B,heads,n,D] (Eq. 1)                             */
+  size_t scratch;             /* stage scratch                                                                 */
+  size_t state;               /* where the per-tensor state lives when hva_forward is called with state == NULL */
+  size_t total;               /* = hva_workspace_bytes()                                                       */
+} hva_workspace_layout;
+
 const char* hva_strerror(int code);
 int hva_version(void);
 
@@ -104,6 +140,11 @@ size_t hva_state_bytes(const hva_shape* s, const hva_config* c);   /* hybrid cac
 /* Scratch needed by one hva_cluster call (per-cell partial sums, split centroids); 0 on invalid arguments. */
 size_t hva_cluster_workspace_bytes(const hva_shape* s, const int32_t cell[3], const int32_t win[3]);
 int hva_plan_describe(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, int32_t tile_q, hva_plan_layout* out);
+/* Scratch needed by one hva_build_plan call; 0 on invalid arguments. */
+size_t hva_plan_workspace_bytes(int32_t BH, int32_t n, int32_t Nq, int32_t Nk);
+int hva_workspace_describe(const hva_shape* s, const hva_config* c, hva_workspace_layout* out);
+/* Layout of the `state` buffer (what hva_forward keeps between calls, and where a caller finds the clustering result). */
+int hva_state_describe(const hva_shape* s, const hva_config* c, hva_state_layout* out);
 
 /* S0-S2 (+A4): 3D local-window k-means on one tensor X[B,heads,n,D] (Alg. 2, l.346-388; Eq. 5
  * l.81; Eq. 6 l.97).  Centre-token init (lines 7-11) unless mu_init != NULL ([BH,Nc,D] fp32,
@@ -116,6 +157,13 @@ int hva_plan_describe(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, int32_t til
 int hva_cluster(const hva_shape* s, const int32_t cell[3], const int32_t win[3], int32_t iters,
                 const void* X, const float* mu_init, int32_t* assign, float* mu, int32_t* sizes,
                 float* sums, float* lowe, void* ws, size_t ws_bytes, void* stream);
+
+/* hva_cluster with kernel-selection flags (HVA_FLAG_CLUSTER_SIMT) and, if probe != NULL (device float[32], zeroed by the
+ * caller; tensor-pipe path only), the instrumented kernel instantiation: probe[0] receives the largest observed
+ * |filter score - exact score| / (|x| max|mu|) (1.0 if the |x|^2 bound was violated).  Labels are unaffected. */
+int hva_cluster_ex(const hva_shape* s, const int32_t cell[3], const int32_t win[3], int32_t iters,
+                   const void* X, const float* mu_init, int32_t* assign, float* mu, int32_t* sizes,
+                   float* sums, float* lowe, uint32_t flags, float* probe, void* ws, size_t ws_bytes, void* stream);
 
 /* S3: indices (ascending) of the m tokens with the largest rho per (b,head), ties -> lower
  * token index (l.101, l.322; R-H2).  lowe[BH,n] fp32 >= 0; subset[BH,m] int32. */
@@ -131,6 +179,10 @@ int hva_cluster_update(const hva_shape* s, int32_t Nc, const void* X, const int3
                        int32_t refresh_all, int32_t* assign, float* mu, float* sums, int32_t* sizes,
                        void* ws, size_t ws_bytes, void* stream);
 
+int hva_cluster_update_ex(const hva_shape* s, int32_t Nc, const void* X, const int32_t* subset, int32_t m,
+                          int32_t refresh_all, int32_t* assign, float* mu, float* sums, int32_t* sizes, uint32_t flags,
+                          void* ws, size_t ws_bytes, void* stream);   /* flags: HVA_FLAG_CLUSTER_SIMT */
+
 /* Scratch needed by one hva_cluster_update call; 0 on invalid arguments. */
 size_t hva_cluster_update_workspace_bytes(const hva_shape* s, int32_t Nc, int32_t m);
 
@@ -141,6 +193,10 @@ int hva_build_mask(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, const float* m
                    const int32_t* sizes_k, float scale, float top_p, float min_kc, uint8_t* mask,
                    void* ws, size_t ws_bytes, void* stream);
 
+int hva_build_mask_ex(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, const float* mu_q, const float* mu_k,
+                      const int32_t* sizes_k, float scale, float top_p, float min_kc, uint8_t* mask, uint32_t flags,
+                      void* ws, size_t ws_bytes, void* stream);       /* flags: HVA_FLAG_MASK_BLOCKSORT */
+
 /* S6: parallel agglomerative merging (Eq. 7-10 l.111-125; Alg. 1 l.131-168), R = rounds.
  * group_of_cluster[BH,Nq] = gid (smallest member) of each query cluster's group (clusters with
  * s^q = 0 keep their own id); n_groups[BH]; group_mask[BH,Nq,Nk] uint8: row g = chi(S_g) for the
@@ -150,6 +206,11 @@ int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const 
               const uint8_t* mask, int32_t tile_q, int32_t tile_k, int32_t rounds, int32_t max_q_tiles,
               uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask,
               void* ws, size_t ws_bytes, void* stream);
+
+int hva_merge_ex(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k,
+                 const uint8_t* mask, int32_t tile_q, int32_t tile_k, int32_t rounds, int32_t max_q_tiles,
+                 uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask, uint32_t flags,
+                 void* ws, size_t ws_bytes, void* stream);            /* flags: HVA_FLAG_MERGE_SIMT */
 
 /* Scratch needed by one hva_merge call; 0 on invalid arguments. */
 size_t hva_merge_workspace_bytes(int32_t BH, int32_t Nq, int32_t Nk);
@@ -171,7 +232,10 @@ int hva_unpermute(const hva_shape* s, const void* Xp, const int32_t* perm, void*
 /* S9 (+S10): block-sparse attention over the permuted tensors (Eq. 4 l.56; packed key blocks
  * l.109; union masks Eq. 8 l.115).  Qp/Kp/Vp[B,heads,n,D] permuted by the plan.  If
  * unpermute != 0, row i of group order is written to O[perm_q[i]] (S10 fused), else to O'[i].
- * bf16, D=128: tcgen05 kernel with 128x128 tiles; f32: CUDA-core reference-precision kernel. */
+ * bf16, D = 128, tile 128 x 128: the tcgen05 kernel (the product path).  Every other combination (f32; bf16 with D = 64;
+ * tiles other than 128 x 128) and c->flags & HVA_FLAG_ATTN_SIMT run the CUDA-core kernel: same result at reference
+ * precision, one warp per query row, NOT tuned -- orders of magnitude slower at the large shapes.  It exists for the
+ * fp32 C1 config and as the on-device cross-check of the tcgen05 kernel. */
 int hva_sparse_attention(const hva_shape* s, const hva_config* c, const void* Qp, const void* Kp,
                          const void* Vp, const void* plan, size_t plan_bytes, int32_t Nq, int32_t Nk,
                          void* O, int32_t unpermute, void* ws, size_t ws_bytes, void* stream);
@@ -189,6 +253,8 @@ int hva_forward(const hva_shape* s, const hva_config* c, const void* Q, const vo
  * only the first chunk's H2D copy and the last chunk's D2H copy are not covered by kernels): the copies of the neighbouring
  * chunks (two library-owned copy streams, both PCIe directions; pinned host buffers needed for the overlap) run under the
  * kernels of the current one.  Chunked and unchunked calls give the same bits (the merge hash is keyed by the global head).
+ * Arguments are validated before anything is enqueued; on any error the stream and the copy streams are drained before
+ * returning.  The copy streams are per device; concurrent host calls on the same device are serialised by the library.
  * Synchronises the stream. */
 int hva_forward_host(const hva_shape* s, const hva_config* c, const void* hQ, const void* hK,
                      const void* hV, void* hO, int32_t step_kind, void* state, void* dev_qkvo,

@@ -17,10 +17,13 @@ LIB_PATH = os.path.join(_HERE, "libhva.so")
 
 HVA_F32, HVA_BF16 = 0, 1
 HVA_ANCHOR, HVA_INTERMEDIATE, HVA_DENSE = 0, 1, 2
+HVA_FLAG_CLUSTER_SIMT, HVA_FLAG_ATTN_SIMT, HVA_FLAG_MASK_BLOCKSORT, HVA_FLAG_MERGE_SIMT = 1, 2, 4, 8
 
-EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes", "hva_merge_workspace_bytes",
-           "hva_plan_describe", "hva_cluster", "hva_select_subset", "hva_cluster_update", "hva_build_mask", "hva_merge",
-           "hva_build_plan", "hva_permute", "hva_unpermute", "hva_sparse_attention", "hva_forward", "hva_forward_host"]
+EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_state_describe", "hva_workspace_describe",
+           "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes", "hva_merge_workspace_bytes", "hva_plan_workspace_bytes",
+           "hva_plan_describe", "hva_cluster", "hva_cluster_ex", "hva_select_subset", "hva_cluster_update", "hva_cluster_update_ex",
+           "hva_build_mask", "hva_build_mask_ex", "hva_merge", "hva_merge_ex", "hva_build_plan", "hva_permute", "hva_unpermute",
+           "hva_sparse_attention", "hva_forward", "hva_forward_host"]
 
 
 class hva_shape(C.Structure):
@@ -31,7 +34,8 @@ class hva_config(C.Structure):
     _fields_ = [("cell_q", C.c_int32 * 3), ("cell_k", C.c_int32 * 3), ("win_q", C.c_int32 * 3), ("win_k", C.c_int32 * 3),
                 ("iters", C.c_int32), ("tile_q", C.c_int32), ("tile_k", C.c_int32), ("top_p", C.c_float),
                 ("min_kc", C.c_float), ("merge_rounds", C.c_int32), ("max_q_tiles", C.c_int32), ("seed", C.c_uint32),
-                ("subset_frac", C.c_float), ("hybrid_refresh_all", C.c_int32), ("softmax_scale", C.c_float)]
+                ("subset_frac", C.c_float), ("hybrid_refresh_all", C.c_int32), ("softmax_scale", C.c_float),
+                ("flags", C.c_uint32)]
 
 
 class hva_stats(C.Structure):
@@ -43,6 +47,16 @@ class hva_stats(C.Structure):
 class hva_plan_layout(C.Structure):
     _fields_ = [(k, C.c_size_t) for k in ("perm_q", "inv_perm_q", "perm_k", "koff", "n_groups", "gid", "goff", "kappa",
                                           "run_cnt", "runs", "run_stride", "work_cnt", "work", "work_cap", "stats", "total")]
+
+
+class hva_state_layout(C.Structure):
+    _fields_ = [(k, C.c_size_t * 2) for k in ("assign", "mu", "sums", "sizes", "subset")] + \
+               [("n_clusters", C.c_int32 * 2), ("m", C.c_int32), ("total", C.c_size_t)]
+
+
+class hva_workspace_layout(C.Structure):
+    _fields_ = [(k, C.c_size_t) for k in ("lowe", "mask", "group_of", "n_groups", "group_mask", "plan", "plan_bytes", "qp", "kp",
+                                          "vp", "scratch", "state", "total")]
 
 
 _lib = None
@@ -61,6 +75,7 @@ def lib():
         L.hva_cluster_workspace_bytes.restype = C.c_size_t
         L.hva_cluster_update_workspace_bytes.restype = C.c_size_t
         L.hva_merge_workspace_bytes.restype = C.c_size_t
+        L.hva_plan_workspace_bytes.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -101,7 +116,7 @@ def make_shape(wl_or_dims, heads=None, dtype=None) -> hva_shape:
 
 
 def make_config(wl: Workload, top_p=None, merge_rounds=None, subset_frac=0.0, refresh_all=0, min_kc=0.0,
-                max_q_tiles=0) -> hva_config:
+                max_q_tiles=0, flags=0) -> hva_config:
     c = hva_config()
     c.cell_q = _i3(wl.cell); c.cell_k = _i3(wl.cell); c.win_q = _i3(wl.win); c.win_k = _i3(wl.win)
     c.iters = wl.iters; c.tile_q, c.tile_k = wl.tile
@@ -109,7 +124,7 @@ def make_config(wl: Workload, top_p=None, merge_rounds=None, subset_frac=0.0, re
     c.min_kc = min_kc
     c.merge_rounds = wl.merge_rounds if merge_rounds is None else merge_rounds
     c.max_q_tiles = max_q_tiles; c.seed = wl.seed; c.subset_frac = subset_frac
-    c.hybrid_refresh_all = refresh_all; c.softmax_scale = 0.0
+    c.hybrid_refresh_all = refresh_all; c.softmax_scale = 0.0; c.flags = flags
     return c
 
 
@@ -135,8 +150,8 @@ def hva_plan_describe(BH, n, Nq, Nk, tile_q) -> hva_plan_layout:
     return L
 
 
-def hva_cluster(shape, cell, win, iters, X, mu_init=None, want_sums=True, want_lowe=True):
-    """-> dict(assign [BH,n] i32, mu [BH,Nc,D] f32, sizes [BH,Nc] i32, sums, lowe)."""
+def hva_cluster(shape, cell, win, iters, X, mu_init=None, want_sums=True, want_lowe=True, flags=0, probe=None):
+    """-> dict(assign [BH,n] i32, mu [BH,Nc,D] f32, sizes [BH,Nc] i32, sums, lowe).  flags / probe: hva_cluster_ex."""
     BH, n, D = shape.B * shape.heads, shape.T * shape.H * shape.W, shape.D
     Nc = hva_num_clusters(shape, cell)
     K = [-(-d // k) for d, k in zip((shape.T, shape.H, shape.W), cell)]
@@ -148,9 +163,14 @@ def hva_cluster(shape, cell, win, iters, X, mu_init=None, want_sums=True, want_l
                sums=torch.empty((BH, Nc, D), dtype=torch.float32, device=dev) if want_sums else None,
                lowe=torch.empty((BH, n), dtype=torch.float32, device=dev) if want_lowe else None)
     ws = _ws(lib().hva_cluster_workspace_bytes(C.byref(shape), _i3(cell), _i3(win)), dev)
-    _check(lib().hva_cluster(C.byref(shape), _i3(cell), _i3(win), int(iters), _p(X), _p(mu_init), _p(out["assign"]),
-                             _p(out["mu"]), _p(out["sizes"]), _p(out["sums"]), _p(out["lowe"]), _p(ws),
-                             C.c_size_t(ws.numel()), _stream()))
+    if flags or probe is not None:
+        _check(lib().hva_cluster_ex(C.byref(shape), _i3(cell), _i3(win), int(iters), _p(X), _p(mu_init), _p(out["assign"]),
+                                    _p(out["mu"]), _p(out["sizes"]), _p(out["sums"]), _p(out["lowe"]), C.c_uint32(flags),
+                                    _p(probe), _p(ws), C.c_size_t(ws.numel()), _stream()))
+    else:
+        _check(lib().hva_cluster(C.byref(shape), _i3(cell), _i3(win), int(iters), _p(X), _p(mu_init), _p(out["assign"]),
+                                 _p(out["mu"]), _p(out["sizes"]), _p(out["sums"]), _p(out["lowe"]), _p(ws),
+                                 C.c_size_t(ws.numel()), _stream()))
     return out
 
 
@@ -161,33 +181,33 @@ def hva_select_subset(lowe, m):
     return subset
 
 
-def hva_cluster_update(shape, X, subset, assign, mu, sums, sizes, refresh_all=0):
+def hva_cluster_update(shape, X, subset, assign, mu, sums, sizes, refresh_all=0, flags=0):
     """In place on assign / mu / sums / sizes."""
     BH, m = subset.shape
     ws = _ws(lib().hva_cluster_update_workspace_bytes(C.byref(shape), int(mu.shape[1]), int(m)), X.device)
-    _check(lib().hva_cluster_update(C.byref(shape), mu.shape[1], _p(X), _p(subset), int(m), int(refresh_all), _p(assign),
-                                    _p(mu), _p(sums), _p(sizes), _p(ws), C.c_size_t(ws.numel()), _stream()))
+    _check(lib().hva_cluster_update_ex(C.byref(shape), mu.shape[1], _p(X), _p(subset), int(m), int(refresh_all), _p(assign),
+                                       _p(mu), _p(sums), _p(sizes), C.c_uint32(flags), _p(ws), C.c_size_t(ws.numel()), _stream()))
 
 
-def hva_build_mask(mu_q, mu_k, sizes_k, scale, top_p, min_kc=0.0):
+def hva_build_mask(mu_q, mu_k, sizes_k, scale, top_p, min_kc=0.0, flags=0):
     BH, Nq, D = mu_q.shape
     Nk = mu_k.shape[1]
     mask = torch.empty((BH, Nq, Nk), dtype=torch.uint8, device=mu_q.device)
-    _check(lib().hva_build_mask(BH, Nq, Nk, D, _p(mu_q), _p(mu_k), _p(sizes_k), C.c_float(scale), C.c_float(top_p),
-                                C.c_float(min_kc), _p(mask), C.c_void_p(0), C.c_size_t(0), _stream()))
+    _check(lib().hva_build_mask_ex(BH, Nq, Nk, D, _p(mu_q), _p(mu_k), _p(sizes_k), C.c_float(scale), C.c_float(top_p),
+                                   C.c_float(min_kc), _p(mask), C.c_uint32(flags), C.c_void_p(0), C.c_size_t(0), _stream()))
     return mask
 
 
-def hva_merge(sizes_q, sizes_k, mask, tile_q, tile_k, rounds, seed=0, max_q_tiles=0):
+def hva_merge(sizes_q, sizes_k, mask, tile_q, tile_k, rounds, seed=0, max_q_tiles=0, flags=0):
     BH, Nq, Nk = mask.shape
     dev = mask.device
     group_of = torch.empty((BH, Nq), dtype=torch.int32, device=dev)
     n_groups = torch.empty((BH,), dtype=torch.int32, device=dev)
     gmask = torch.empty((BH, Nq, Nk), dtype=torch.uint8, device=dev)
     ws = _ws(lib().hva_merge_workspace_bytes(BH, Nq, Nk), dev)
-    _check(lib().hva_merge(BH, Nq, Nk, _p(sizes_q), _p(sizes_k), _p(mask), int(tile_q), int(tile_k), int(rounds),
-                           int(max_q_tiles), C.c_uint32(seed), _p(group_of), _p(n_groups), _p(gmask), _p(ws),
-                           C.c_size_t(ws.numel()), _stream()))
+    _check(lib().hva_merge_ex(BH, Nq, Nk, _p(sizes_q), _p(sizes_k), _p(mask), int(tile_q), int(tile_k), int(rounds),
+                              int(max_q_tiles), C.c_uint32(seed), _p(group_of), _p(n_groups), _p(gmask), C.c_uint32(flags), _p(ws),
+                              C.c_size_t(ws.numel()), _stream()))
     return group_of, n_groups, gmask
 
 
@@ -227,7 +247,7 @@ def hva_build_plan(n, assign_q, assign_k, sizes_q, sizes_k, group_of, n_groups, 
     dev = gmask.device
     L = hva_plan_describe(BH, n, Nq, Nk, tile_q)
     buf = torch.zeros(L.total, dtype=torch.uint8, device=dev)
-    ws = _ws(BH * ((n + 1023) // 1024) * max(Nq, Nk) * 4 + BH * Nq * 4 + 1024, dev)
+    ws = _ws(lib().hva_plan_workspace_bytes(BH, n, Nq, Nk), dev)
     _check(lib().hva_build_plan(BH, n, Nq, Nk, _p(assign_q), _p(assign_k), _p(sizes_q), _p(sizes_k), _p(group_of),
                                 _p(n_groups), _p(gmask), int(tile_q), int(tile_k), _p(buf), C.c_size_t(L.total), _p(ws),
                                 C.c_size_t(ws.numel()), _stream()))
@@ -281,23 +301,37 @@ class Forward:
         return hO
 
     def state_views(self):
-        """Typed views of the hybrid cache (layout of api.cu make_layout: per tensor Q then K, 256-byte aligned
-        assign[BH,n] i32, mu[BH,Nc,D] f32, sums[BH,Nc,D] f32, sizes[BH,Nc] i32, subset[BH,m] i32)."""
+        """Typed views of the hybrid cache, located by hva_state_describe()."""
         assert self.state is not None
-        s, c = self.shape, self.cfg
+        s = self.shape
         BH, n, D = self.BH, s.T * s.H * s.W, s.D
-        m = int(math.floor(float(c.subset_frac) * n + 0.5))
-        al = lambda x: (x + 255) // 256 * 256
-        out, o = {}, 0
-        for t, cell in (("q", c.cell_q), ("k", c.cell_k)):
-            Nc = hva_num_clusters(s, list(cell))
+        L = hva_state_layout()
+        _check(lib().hva_state_describe(C.byref(s), C.byref(self.cfg), C.byref(L)))
+        out = {}
+        for i, t in enumerate("qk"):
+            Nc = L.n_clusters[i]
             for name, shp, dt in (("assign", (BH, n), torch.int32), ("mu", (BH, Nc, D), torch.float32),
                                   ("sums", (BH, Nc, D), torch.float32), ("sizes", (BH, Nc), torch.int32),
-                                  ("subset", (BH, max(m, 1)), torch.int32)):
+                                  ("subset", (BH, max(L.m, 1)), torch.int32)):
+                o = getattr(L, name)[i]
                 nb = int(math.prod(shp)) * 4
                 out[f"{name}_{t}"] = self.state[o:o + nb].view(dt).view(*shp)
-                o += al(nb)
         return out
+
+    def ws_views(self):
+        """Typed views of the intermediate results the last sparse call left in the workspace (hva_workspace_describe):
+        mask, group_of, n_groups, group_mask and the plan."""
+        s = self.shape
+        BH, n = self.BH, s.T * s.H * s.W
+        W = hva_workspace_layout()
+        _check(lib().hva_workspace_describe(C.byref(s), C.byref(self.cfg), C.byref(W)))
+        Nq, Nk = hva_num_clusters(s, list(self.cfg.cell_q)), hva_num_clusters(s, list(self.cfg.cell_k))
+        v = lambda off, shp, dt: self.ws[off:off + int(math.prod(shp)) * torch.empty((), dtype=dt).element_size()].view(dt).view(*shp)
+        L = hva_plan_describe(BH, n, max(Nq, 1), max(Nk, 1), self.cfg.tile_q)
+        assert L.total == W.plan_bytes
+        return dict(mask=v(W.mask, (BH, Nq, Nk), torch.uint8), group_of=v(W.group_of, (BH, Nq), torch.int32),
+                    n_groups=v(W.n_groups, (BH,), torch.int32), group_mask=v(W.group_mask, (BH, Nq, Nk), torch.uint8),
+                    plan=Plan(self.ws[W.plan:W.plan + W.plan_bytes], L, BH, n, Nq, Nk))
 
     def stats_dicts(self):
         out = []

@@ -4,7 +4,7 @@
 // -> attention + inverse permutation (Eq. 4).  Everything is enqueued on one stream, no host sync.
 #include "common.cuh"
 #include <cmath>
-#include <cstdlib>
+#include <mutex>
 
 namespace {
 
@@ -92,6 +92,30 @@ extern "C" size_t hva_state_bytes(const hva_shape* s, const hva_config* c) {
   if (make_layout(s, c, &F) != HVA_OK) return 0;
   return F.state_total;
 }
+extern "C" int hva_state_describe(const hva_shape* s, const hva_config* c, hva_state_layout* out) {
+  if (!valid_shape(s) || !valid_config(c) || !out) return HVA_EINVAL;
+  FwdLayout F;
+  HVA_TRY(make_layout(s, c, &F));
+  for (int t = 0; t < 2; ++t) {
+    out->assign[t] = F.assign[t]; out->mu[t] = F.mu[t]; out->sums[t] = F.sums[t]; out->sizes[t] = F.sizes[t];
+    out->subset[t] = F.subset[t];
+  }
+  out->n_clusters[0] = F.Nq; out->n_clusters[1] = F.Nk; out->m = F.m; out->total = F.state_total;
+  return HVA_OK;
+}
+extern "C" int hva_workspace_describe(const hva_shape* s, const hva_config* c, hva_workspace_layout* out) {
+  if (!valid_shape(s) || !valid_config(c) || !out) return HVA_EINVAL;
+  FwdLayout F;
+  HVA_TRY(make_layout(s, c, &F));
+  out->lowe = F.lowe; out->mask = F.mask; out->group_of = F.group_of; out->n_groups = F.n_groups; out->group_mask = F.group_mask;
+  out->plan = F.plan; out->plan_bytes = F.PL.total; out->qp = F.qp; out->kp = F.kp; out->vp = F.vp; out->scratch = F.scratch;
+  out->state = F.ws_total; out->total = F.ws_total + F.state_total;
+  return HVA_OK;
+}
+extern "C" size_t hva_plan_workspace_bytes(int32_t BH, int32_t n, int32_t Nq, int32_t Nk) {
+  if (BH < 1 || n < 1 || Nq < 1 || Nk < 1) return 0;
+  return hva_plan_ws_bytes(BH, n, Nq, Nk);
+}
 
 extern "C" int hva_sparse_attention(const hva_shape* s, const hva_config* c, const void* Qp, const void* Kp, const void* Vp,
                                     const void* plan, size_t plan_bytes, int32_t Nq, int32_t Nk, void* O,
@@ -104,9 +128,8 @@ extern "C" int hva_sparse_attention(const hva_shape* s, const hva_config* c, con
   if (plan_bytes < L.total) return HVA_EWORKSPACE;
   const float scale = c->softmax_scale > 0.f ? c->softmax_scale : 1.0f / sqrtf((float)s->D);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  const char* force = getenv("HVA_ATTN_SIMT");
   const bool tc_ok = s->dtype == HVA_BF16 && s->D == 128 && c->tile_q == 128 && c->tile_k == 128;
-  if (tc_ok && !(force && force[0] == '1')) return hva_attention_tc_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st);
+  if (tc_ok && !(c->flags & HVA_FLAG_ATTN_SIMT)) return hva_attention_tc_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st);
   return hva_attention_simt_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st, c->tile_q);
 }
 
@@ -128,7 +151,7 @@ int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const v
   if (step_kind == HVA_DENSE) {   // full attention (warm-up steps / layers, l.324): one group, one key run
     hva_plan_layout L;
     HVA_TRY(hva_plan_describe(BH, n, 1, 1, c->tile_q, &L));
-    HVA_TRY(hva_attention_dense_plan(BH, n, c->tile_q, plan, L, st));
+    HVA_TRY(hva_attention_dense_plan(BH, n, c->tile_q, c->tile_k, plan, L, st));
     HVA_TRY(hva_sparse_attention(s, c, Q, K, V, plan, L.total, 1, 1, O, 0, nullptr, 0, stream));
     if (stats_out && cudaMemcpyAsync(stats_out, (char*)plan + L.stats, sizeof(hva_stats) * BH, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
       return HVA_ECUDA;
@@ -148,12 +171,12 @@ int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const v
     int32_t* subset = (int32_t*)(sb + F.subset[t]);
     if (step_kind == HVA_ANCHOR) {
       float* lowe = hybrid ? (float*)(w + F.lowe) : nullptr;
-      HVA_TRY(hva_cluster(s, cell[t], win[t], c->iters, X[t], nullptr, assign, mu, sizes, sums, lowe, w + F.scratch,
-                          F.scratch_bytes, stream));
+      HVA_TRY(hva_cluster_ex(s, cell[t], win[t], c->iters, X[t], nullptr, assign, mu, sizes, sums, lowe, c->flags, nullptr,
+                             w + F.scratch, F.scratch_bytes, stream));
       if (hybrid) HVA_TRY(hva_select_subset(BH, n, lowe, F.m, subset, w + F.scratch, F.scratch_bytes, stream));
     } else {
-      HVA_TRY(hva_cluster_update(s, Nc[t], X[t], subset, F.m, c->hybrid_refresh_all, assign, mu, sums, sizes,
-                                 w + F.scratch, F.scratch_bytes, stream));
+      HVA_TRY(hva_cluster_update_ex(s, Nc[t], X[t], subset, F.m, c->hybrid_refresh_all, assign, mu, sums, sizes, c->flags,
+                                    w + F.scratch, F.scratch_bytes, stream));
     }
   }
   const float scale = c->softmax_scale > 0.f ? c->softmax_scale : 1.0f / sqrtf((float)s->D);
@@ -161,10 +184,10 @@ int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const v
   uint8_t* gmask = (uint8_t*)(w + F.group_mask);
   int32_t* group_of = (int32_t*)(w + F.group_of);
   int32_t* n_groups = (int32_t*)(w + F.n_groups);
-  HVA_TRY(hva_build_mask(BH, F.Nq, F.Nk, s->D, (float*)(sb + F.mu[0]), (float*)(sb + F.mu[1]), (int32_t*)(sb + F.sizes[1]),
-                         scale, c->top_p, c->min_kc, mask, w + F.scratch, F.scratch_bytes, stream));
+  HVA_TRY(hva_build_mask_ex(BH, F.Nq, F.Nk, s->D, (float*)(sb + F.mu[0]), (float*)(sb + F.mu[1]), (int32_t*)(sb + F.sizes[1]),
+                            scale, c->top_p, c->min_kc, mask, c->flags, w + F.scratch, F.scratch_bytes, stream));
   HVA_TRY(hva_merge_offset(bh0, BH, F.Nq, F.Nk, (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), mask, c->tile_q, c->tile_k,
-                    c->merge_rounds, c->max_q_tiles, c->seed, group_of, n_groups, gmask, w + F.scratch, F.scratch_bytes, stream));
+                    c->merge_rounds, c->max_q_tiles, c->seed, group_of, n_groups, gmask, c->flags, w + F.scratch, F.scratch_bytes, stream));
   HVA_TRY(hva_build_plan(BH, n, F.Nq, F.Nk, (int32_t*)(sb + F.assign[0]), (int32_t*)(sb + F.assign[1]),
                          (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), group_of, n_groups, gmask, c->tile_q,
                          c->tile_k, plan, F.PL.total, w + F.scratch, F.scratch_bytes, stream));
@@ -186,12 +209,16 @@ extern "C" int hva_forward(const hva_shape* s, const hva_config* c, const void* 
 }
 
 namespace {
-// copy streams / events of hva_forward_host, created once per process (no device memory is allocated)
+// Copy streams / events of hva_forward_host: one set per device, created on first use on that device (no device memory
+// is allocated).  The table is guarded by a mutex; a call holds its device's set for its whole duration, so concurrent host
+// calls on one device are serialised (documented in hva.h).
 struct HostPipe {
   cudaStream_t h2d = nullptr, d2h = nullptr;
   cudaEvent_t in_done[8] = {}, out_ready[8] = {}, start = nullptr;
-  bool ok = false;
-  HostPipe() {
+  bool tried = false, ok = false;
+  std::mutex busy;
+  void create() {
+    tried = true;
     ok = cudaStreamCreateWithFlags(&h2d, cudaStreamNonBlocking) == cudaSuccess &&
          cudaStreamCreateWithFlags(&d2h, cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&start, cudaEventDisableTiming) == cudaSuccess;
@@ -200,6 +227,16 @@ struct HostPipe {
            cudaEventCreateWithFlags(&out_ready[i], cudaEventDisableTiming) == cudaSuccess;
   }
 };
+constexpr int kMaxDevices = 64;
+HostPipe* host_pipe() {
+  static HostPipe pipes[kMaxDevices];
+  static std::mutex table;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+  std::lock_guard<std::mutex> g(table);
+  if (!pipes[dev].tried) pipes[dev].create();
+  return pipes[dev].ok ? &pipes[dev] : nullptr;
+}
 }  // namespace
 
 // Heads are independent instances of the whole pipeline, so the host variant runs the call in chunks of heads: the
@@ -209,54 +246,68 @@ struct HostPipe {
 extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const void* hQ, const void* hK, const void* hV,
                                 void* hO, int32_t step_kind, void* state, void* dev_qkvo, void* ws, size_t ws_bytes,
                                 void* stream) {
-  if (!valid_shape(s) || !hQ || !hK || !hV || !hO || !dev_qkvo) return HVA_EINVAL;
+  // everything that can fail on the arguments is checked before anything is enqueued (hva.h: nothing is enqueued on
+  // EINVAL / EWORKSPACE): the full-size layout bounds the layout of every chunk
+  if (!valid_shape(s) || !valid_config(c) || !hQ || !hK || !hV || !hO || !dev_qkvo || !ws) return HVA_EINVAL;
+  if (step_kind != HVA_ANCHOR && step_kind != HVA_INTERMEDIATE && step_kind != HVA_DENSE) return HVA_EINVAL;
+  if (step_kind == HVA_INTERMEDIATE && (!state || c->subset_frac <= 0.f)) return HVA_EINVAL;
+  {
+    FwdLayout F;
+    HVA_TRY(make_layout(s, c, &F));
+    if (ws_bytes < F.ws_total + (state ? 0 : F.state_total)) return HVA_EWORKSPACE;
+  }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const size_t es = s->dtype == HVA_F32 ? 4 : 2;
   const size_t head_bytes = (size_t)s->T * s->H * s->W * s->D * es;
   const size_t bytes = (size_t)s->B * s->heads * head_bytes;
   char* d = reinterpret_cast<char*>(dev_qkvo);
-  static HostPipe pipe;
+  HostPipe* pipe = (!state && s->B == 1 && s->heads >= 8) ? host_pipe() : nullptr;
+  if (!pipe) {
+    int rc = HVA_OK;
+    if (cudaMemcpyAsync(d, hQ, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(d + bytes, hK, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(d + 2 * bytes, hV, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+      rc = HVA_ECUDA;
+    if (rc == HVA_OK) rc = hva_forward(s, c, d, d + bytes, d + 2 * bytes, d + 3 * bytes, step_kind, state, nullptr, ws, ws_bytes, stream);
+    if (rc == HVA_OK && cudaMemcpyAsync(hO, d + 3 * bytes, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = HVA_ECUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess && rc == HVA_OK) rc = HVA_ECUDA;   // also on error: nothing of ours stays in flight
+    return rc;
+  }
+  std::lock_guard<std::mutex> hold(pipe->busy);
   // chunk boundaries: the first chunk's H2D copy and the last chunk's D2H copy are the only transfers no kernel covers, so
   // both end chunks are small (heads / 12) and the heads between them go in three equal parts
-  int nchunk = 1, bound[8] = {0, s->heads};
-  if (pipe.ok && !state && s->B == 1 && s->heads >= 8) {
+  const int nchunk = 5;
+  int bound[8];
+  {
     const int edge = s->heads / 12 > 0 ? s->heads / 12 : 1, mid = s->heads - 2 * edge;
-    nchunk = 5;
-    bound[1] = edge;
-    bound[2] = edge + mid / 3;
-    bound[3] = edge + (2 * mid) / 3;
-    bound[4] = edge + mid;
-    bound[5] = s->heads;
+    bound[0] = 0; bound[1] = edge; bound[2] = edge + mid / 3; bound[3] = edge + (2 * mid) / 3; bound[4] = edge + mid; bound[5] = s->heads;
   }
-  if (nchunk == 1) {
-    if (cudaMemcpyAsync(d, hQ, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
-    if (cudaMemcpyAsync(d + bytes, hK, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
-    if (cudaMemcpyAsync(d + 2 * bytes, hV, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return HVA_ECUDA;
-    HVA_TRY(hva_forward(s, c, d, d + bytes, d + 2 * bytes, d + 3 * bytes, step_kind, state, nullptr, ws, ws_bytes, stream));
-    if (cudaMemcpyAsync(hO, d + 3 * bytes, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return HVA_ECUDA;
-    if (cudaStreamSynchronize(st) != cudaSuccess) return HVA_ECUDA;
-    return HVA_OK;
-  }
+  int rc = HVA_OK;
   // the copy streams start after whatever the caller has queued on `st`
-  if (cudaEventRecord(pipe.start, st) != cudaSuccess || cudaStreamWaitEvent(pipe.h2d, pipe.start, 0) != cudaSuccess ||
-      cudaStreamWaitEvent(pipe.d2h, pipe.start, 0) != cudaSuccess)
-    return HVA_ECUDA;
+  if (cudaEventRecord(pipe->start, st) != cudaSuccess || cudaStreamWaitEvent(pipe->h2d, pipe->start, 0) != cudaSuccess ||
+      cudaStreamWaitEvent(pipe->d2h, pipe->start, 0) != cudaSuccess)
+    rc = HVA_ECUDA;
   const char* src[3] = {(const char*)hQ, (const char*)hK, (const char*)hV};
-  for (int i = 0; i < nchunk; ++i) {
+  for (int i = 0; i < nchunk && rc == HVA_OK; ++i) {
     const int h0 = bound[i], h1 = bound[i + 1], nh = h1 - h0;
     const size_t off = (size_t)h0 * head_bytes, cb = (size_t)nh * head_bytes;
-    for (int t = 0; t < 3; ++t)
-      if (cudaMemcpyAsync(d + t * bytes + off, src[t] + off, cb, cudaMemcpyHostToDevice, pipe.h2d) != cudaSuccess) return HVA_ECUDA;
-    if (cudaEventRecord(pipe.in_done[i], pipe.h2d) != cudaSuccess || cudaStreamWaitEvent(st, pipe.in_done[i], 0) != cudaSuccess)
-      return HVA_ECUDA;
+    for (int t = 0; t < 3 && rc == HVA_OK; ++t)
+      if (cudaMemcpyAsync(d + t * bytes + off, src[t] + off, cb, cudaMemcpyHostToDevice, pipe->h2d) != cudaSuccess) rc = HVA_ECUDA;
+    if (rc == HVA_OK && (cudaEventRecord(pipe->in_done[i], pipe->h2d) != cudaSuccess || cudaStreamWaitEvent(st, pipe->in_done[i], 0) != cudaSuccess))
+      rc = HVA_ECUDA;
+    if (rc != HVA_OK) break;
     hva_shape sc = *s;
     sc.heads = nh;
-    HVA_TRY(forward_impl(&sc, c, d + off, d + bytes + off, d + 2 * bytes + off, d + 3 * bytes + off, step_kind, nullptr, nullptr, ws,
-                         ws_bytes, stream, h0));
-    if (cudaEventRecord(pipe.out_ready[i], st) != cudaSuccess || cudaStreamWaitEvent(pipe.d2h, pipe.out_ready[i], 0) != cudaSuccess)
-      return HVA_ECUDA;
-    if (cudaMemcpyAsync((char*)hO + off, d + 3 * bytes + off, cb, cudaMemcpyDeviceToHost, pipe.d2h) != cudaSuccess) return HVA_ECUDA;
+    rc = forward_impl(&sc, c, d + off, d + bytes + off, d + 2 * bytes + off, d + 3 * bytes + off, step_kind, nullptr, nullptr, ws,
+                      ws_bytes, stream, h0);
+    if (rc != HVA_OK) break;
+    if (cudaEventRecord(pipe->out_ready[i], st) != cudaSuccess || cudaStreamWaitEvent(pipe->d2h, pipe->out_ready[i], 0) != cudaSuccess ||
+        cudaMemcpyAsync((char*)hO + off, d + 3 * bytes + off, cb, cudaMemcpyDeviceToHost, pipe->d2h) != cudaSuccess)
+      rc = HVA_ECUDA;
   }
-  if (cudaStreamSynchronize(pipe.d2h) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return HVA_ECUDA;
-  return HVA_OK;
+  // drain all three streams, also on error: no copy into or out of the caller's buffers is left in flight
+  const bool s0 = cudaStreamSynchronize(pipe->h2d) == cudaSuccess, s1 = cudaStreamSynchronize(st) == cudaSuccess,
+             s2 = cudaStreamSynchronize(pipe->d2h) == cudaSuccess;
+  if (rc == HVA_OK && !(s0 && s1 && s2)) rc = HVA_ECUDA;
+  return rc;
 }

@@ -2,21 +2,22 @@
 // block-sparse FlashAttention over the plan's packed key runs (Eq. 4 l.56; packed key
 // blocks l.109; union masks Eq. 8 l.115).
 //
-// One CTA per (group, q-tile) work item.  Warp roles:
-//   warps 0-3  softmax / correction / epilogue: thread i owns query row i == TMEM lane i
-//   warp  4    TMA producer: Q tile once, then per packed key tile the K and V rows of the group's
-//              key runs, as power-of-two-height boxes of a 128B-swizzled 2-D tensor map, packed
-//              back to back in the stage buffer (exact packing across cluster boundaries)
-//   warp  5    TMEM allocator + single-thread tcgen05.mma issuer
-// Two CTAs are resident per SM (96 KB smem, 256 TMEM columns each): one CTA's softmax overlaps the other's MMAs.
-// Per key tile j:  S_j = Q K_j^T (SS MMA, K-major operands, fp32 accumulators in TMEM)
-//                  P_j = exp2(S_j*scale*log2e - m) written back over S_j as bf16 (tcgen05.st)
-//                  O  += P_j V_j (TS MMA: A = P from TMEM, B = V from smem, MN-major)
+// One CTA per (group, q-tile) work item, one CTA per SM, 16 warps in four warpgroups:
+//   warps 0-3 / 4-7  two softmax sets (setmaxnreg 200): set b takes the key tiles j = b (mod 2), i.e. always the buffers S_b / P_b;
+//                    thread = one full query row (TMEM lane) held in 128 registers; correction and epilogue
+//   warps 8, 11      TMA producers of the K ring (64-dim halves 0 / 1; warp 8 also loads the Q tile)
+//   warps 10, 12     TMA producers of the V ring (64-dim halves 0 / 1)
+//   warp  9          TMEM allocator (512 columns) + tcgen05.mma issuer (one elected lane)
+// The producers walk the group's key runs and issue power-of-two-height boxes of a 128B-swizzled 2-D tensor map so that rows
+// of different clusters land back to back in the stage buffer (exact packing across cluster boundaries, l.109).
+// TMEM: S_0, S_1 (fp32 scores, 128 columns each), O (128), P_0, P_1 (bf16 probabilities, 64 each).
+// Per key tile j:  S_b = Q K_j^T (SS MMA, K-major operands, fp32 accumulators in TMEM)
+//                  P_b = exp2(S_b*scale*log2e - m_ref) written as bf16 into its own TMEM buffer (tcgen05.st)
+//                  O  += P_b V_j (TS MMA: A = P from TMEM, B = V from smem, MN-major)
 // with lazy (thresholded) rescaling of O in TMEM, 1/l normalisation and the inverse permutation
 // fused into the epilogue's row stores.
 #include "common.cuh"
 #include "ptx.cuh"
-#include <cstdlib>
 
 namespace {
 using namespace hva_ptx;
@@ -48,8 +49,13 @@ struct TcParams {
   const int *goff, *koff, *kappa, *run_cnt, *work_cnt, *work, *perm_q;
   const uint32_t* runs;
   __nv_bfloat16* O;
-  unsigned long long* probe;   // HVA_ATTN_TIMING builds only: per-phase cycle totals
+#ifdef HVA_ATTN_TIMING
+  unsigned long long* probe;   // per-phase cycle totals (diagnostic build only)
+#endif
 };
+#ifdef HVA_ATTN_TIMING
+unsigned long long* g_attn_timing = nullptr;   // diagnostic build only: set through hva_debug_attn_timing()
+#endif
 
 // instruction descriptor: D = F32, A = B = BF16, M = 128, N = 128; b_major selects MN-major B
 __device__ __forceinline__ uint32_t umma_idesc(uint32_t b_mn_major) {
@@ -454,6 +460,10 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint32_t box_rows
 
 }  // namespace
 
+#ifdef HVA_ATTN_TIMING
+extern "C" void hva_debug_attn_timing(unsigned long long* dev16) { g_attn_timing = dev16; }
+#endif
+
 int hva_attention_tc_launch(const hva_shape* s, float scale, const void* Qp, const void* Kp, const void* Vp,
                             const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute,
                             cudaStream_t st) {
@@ -475,16 +485,12 @@ int hva_attention_tc_launch(const hva_shape* s, float scale, const void* Qp, con
   p.run_cnt = (const int*)(b + L.run_cnt); p.work_cnt = (const int*)(b + L.work_cnt); p.work = (const int*)(b + L.work);
   p.perm_q = (const int*)(b + L.perm_q); p.runs = (const uint32_t*)(b + L.runs);
   p.O = reinterpret_cast<__nv_bfloat16*>(O);
-  {
-    const char* pe = getenv("HVA_ATTN_PROBE");
-    p.probe = pe ? reinterpret_cast<unsigned long long*>(strtoull(pe, nullptr, 0)) : nullptr;
-  }
-  static bool attr_set = false;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(hva_attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemTC) != cudaSuccess)
-      return HVA_ECUDA;
-    attr_set = true;
-  }
+#ifdef HVA_ATTN_TIMING
+  p.probe = g_attn_timing;
+#endif
+  // the attribute is per device: set on every call (cheap) rather than behind a process-wide flag
+  if (cudaFuncSetAttribute(hva_attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemTC) != cudaSuccess)
+    return HVA_ECUDA;
   dim3 grid((unsigned)L.work_cap, BH);
   hva_attn_tc_kernel<<<grid, kThreadsTC, kSmemTC, st>>>(maps, p);
   HVA_CHECK_LAUNCH();

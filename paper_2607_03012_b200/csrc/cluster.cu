@@ -9,7 +9,6 @@
 // fixed cell order, by hva_finalize_kernel (Alg. 2 line 23: mu <- z/n, empty keeps mu).
 #include "common.cuh"
 #include "cluster_tc.cuh"
-#include <cstdlib>
 
 namespace {
 
@@ -346,14 +345,14 @@ struct ClusterWs {
 
 template <typename T, int D>
 int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float* mu_init, int* assign, float* mu,
-                int* sizes, float* sums, float* lowe, const ClusterWs& ws, int dtype, cudaStream_t st) {
+                int* sizes, float* sums, float* lowe, const ClusterWs& ws, int dtype, uint32_t flags, float* probe, cudaStream_t st) {
   dim3 grid(g.Nc, BH);
-  const char* force = getenv("HVA_CLUSTER_SIMT");
-  const bool tc = hva_assign_tc_supported(g, D, dtype) && !(force && force[0] == '1');
+  const bool tc = hva_assign_tc_supported(g, D, dtype) && !(flags & HVA_FLAG_CLUSTER_SIMT);
+  if (!tc) probe = nullptr;
   HvaAssignTc atc;
   size_t smem = 0;
   if (tc) {
-    HVA_TRY(hva_assign_tc_prepare(g, BH, X, ws.hi, ws.lo, &atc));
+    HVA_TRY(hva_assign_tc_prepare(g, BH, X, ws.hi, ws.lo, probe != nullptr, &atc));
   } else {
     smem = assign_smem_bytes(g, D, sizeof(T));
     if (smem > 227 * 1024) return HVA_EUNSUPPORTED;
@@ -373,8 +372,6 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
     hva_mu_split_kernel<D><<<grid, D, 0, st>>>(g.Nc, mu, sp);
     HVA_CHECK_LAUNCH();
   }
-  const char* probe_env = getenv("HVA_CLUSTER_PROBE");   // debug: device float receiving the observed filter error
-  float* probe = (tc && probe_env) ? reinterpret_cast<float*>(strtoull(probe_env, nullptr, 0)) : nullptr;
   for (int it = 0; it < iters; ++it) {
     bool last = (it == iters - 1);
     if (tc) {
@@ -418,6 +415,12 @@ extern "C" size_t hva_cluster_workspace_bytes(const hva_shape* s, const int32_t 
 extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int32_t win[3], int32_t iters, const void* X,
                            const float* mu_init, int32_t* assign, float* mu, int32_t* sizes, float* sums, float* lowe,
                            void* ws, size_t ws_bytes, void* stream) {
+  return hva_cluster_ex(s, cell, win, iters, X, mu_init, assign, mu, sizes, sums, lowe, 0u, nullptr, ws, ws_bytes, stream);
+}
+
+extern "C" int hva_cluster_ex(const hva_shape* s, const int32_t cell[3], const int32_t win[3], int32_t iters, const void* X,
+                              const float* mu_init, int32_t* assign, float* mu, int32_t* sizes, float* sums, float* lowe,
+                              uint32_t flags, float* probe, void* ws, size_t ws_bytes, void* stream) {
   if (!s || !cell || !win || !X || !assign || !mu || !sizes || !ws) return HVA_EINVAL;
   if (s->B < 1 || s->heads < 1 || s->T < 1 || s->H < 1 || s->W < 1 || iters < 1) return HVA_EINVAL;
   if (s->D != 64 && s->D != 128) return HVA_EINVAL;
@@ -440,7 +443,7 @@ extern "C" int hva_cluster(const hva_shape* s, const int32_t cell[3], const int3
     cw.counter = reinterpret_cast<int*>(w);
   }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-#define HVA_DISPATCH(T, DD) return run_cluster<T, DD>(g, BH, iters, X, mu_init, assign, mu, sizes, sums, lowe, cw, s->dtype, st)
+#define HVA_DISPATCH(T, DD) return run_cluster<T, DD>(g, BH, iters, X, mu_init, assign, mu, sizes, sums, lowe, cw, s->dtype, flags, probe, st)
   if (s->dtype == HVA_F32) {
     if (s->D == 64) HVA_DISPATCH(float, 64);
     HVA_DISPATCH(float, 128);

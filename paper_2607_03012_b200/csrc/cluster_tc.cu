@@ -22,8 +22,6 @@
 #include "ptx.cuh"
 #include "cluster_tc.cuh"
 #include <algorithm>
-#include <cstdio>
-#include <cstdlib>
 
 namespace {
 using namespace hva_ptx;
@@ -78,6 +76,9 @@ __device__ __forceinline__ int fast_div64(int x, unsigned long long m) { return 
 // order from a device counter; 128 threads, thread = token row of the tile = TMEM lane.  Per-CTA set-up (TMEM allocation,
 // barriers, the CTA launch itself: ~2.5K clk, during which a kernel that allocates TMEM starts no other CTA on the SM)
 // is paid once, and the loads of the next tile are issued as soon as the sums MMA has released the tiles, under the epilogue.
+// kProbe = true is the instrumented instantiation behind hva_cluster_ex(probe != NULL) (tests: observed filter error; timing builds:
+// per-phase clocks); the product instantiation carries none of that code.
+template <bool kProbe>
 __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_hi,
                                                                  const __grid_constant__ CUtensorMap map_lo, AssignTcParams p) {
@@ -353,6 +354,8 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
       if (sv[j + 1] <= thr) cand_b |= 2u << j;
     }
     cand |= cand_b;
+    // thr = +inf (single-candidate window with the Lowe ratio: s2 = +inf) would also admit the pad slots, whose score is +inf
+    cand &= nwin - v0 >= 32 ? 0xffffffffu : (1u << (nwin - v0)) - 1u;
     if (n_cont == 0 && cand) first = v0 + __ffs(cand) - 1;
     n_cont += __popc(cand);
     if (v0 == 0) cand0 = cand;
@@ -368,6 +371,7 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
 #pragma unroll
         for (int j = 0; j < 32; ++j)
           if (sv[j] <= thr) cand |= 1u << j;
+        cand &= nwin - v0 >= 32 ? 0xffffffffu : (1u << (nwin - v0)) - 1u;
       }
       if (!refine) cand = 0;
       while (cand) {
@@ -388,7 +392,7 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
   }
   CMARK(5);
 #ifndef HVA_ASSIGN_TIMING
-  if (p.probe) {   // debug: observed filter error against the exact direct form
+  if constexpr (kProbe) {   // observed filter error against the exact direct form
     float worst = 0.f, xx = 0.f;
     if (valid) {
       for (int q = 0; q < 16; ++q) {
@@ -474,7 +478,7 @@ __global__ void __launch_bounds__(kThreads, 4) hva_assign_tc_kernel(const __grid
   CMARK(9);
   }   // tiles
 #ifdef HVA_ASSIGN_TIMING
-  if (threadIdx.x == 0 && p.probe) for (int k = 0; k < 10; ++k) atomicAdd(p.probe + 16 + k, (float)tacc[k]);
+  if (kProbe && threadIdx.x == 0) for (int k = 0; k < 10; ++k) atomicAdd(p.probe + 16 + k, (float)tacc[k]);
 #endif
   __syncthreads();
   if (warp == 1) { tc_fence_after(); tmem_dealloc(B->tmem_base, p.tmem_cols); }
@@ -503,7 +507,9 @@ bool make_map5(CUtensorMap* m, const void* base, int BH, int d3, int d2, int d1,
 }
 }  // namespace
 
-int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, HvaAssignTc* a) {
+int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, bool probe, HvaAssignTc* a) {
+  const void* kern = probe ? (const void*)hva_assign_tc_kernel<true> : (const void*)hva_assign_tc_kernel<false>;
+  a->probe = probe;
   a->ct = hva_assign_tc_slices(g);
   a->csplit = (g.kt + a->ct - 1) / a->ct;
   const int ctok = a->ct * g.kh * g.kw;
@@ -522,7 +528,7 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
   if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, a->ct, g.kh, g.kw)) return HVA_ECUDA;
   if (!make_map5(&a->map_hi, mu_hi, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
   if (!make_map5(&a->map_lo, mu_lo, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
-  if (cudaFuncSetAttribute(hva_assign_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
     return HVA_ECUDA;
   // resident CTAs per SM from the shared-memory, register and TMEM budgets (the runtime's occupancy query answers 1 for a
   // kernel that allocates TMEM, whatever it allocates)
@@ -532,13 +538,12 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
       cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev) != cudaSuccess ||
       cudaDeviceGetAttribute(&smem_res, cudaDevAttrReservedSharedMemoryPerBlock, dev) != cudaSuccess ||
       cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev) != cudaSuccess ||
-      cudaFuncGetAttributes(&fa, hva_assign_tc_kernel) != cudaSuccess)
+      cudaFuncGetAttributes(&fa, kern) != cudaSuccess)
     return HVA_ECUDA;
   const int regs_cta = ((fa.numRegs + 7) & ~7) * kThreads;
   int per_sm = std::min({(int)((size_t)smem_sm / (bytes + (size_t)smem_res)), regs_sm / std::max(regs_cta, 1), 512 / (int)a->tmem_cols});
   if (per_sm < 1) return HVA_EUNSUPPORTED;
   a->grid = sms * per_sm;
-  if (getenv("HVA_DEBUG")) fprintf(stderr, "assign_tc: %d SMs x %d CTAs, smem %zu, tmem %u\n", sms, per_sm, bytes, a->tmem_cols);
   return HVA_OK;
 }
 
@@ -550,7 +555,9 @@ int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const f
                    magic(g.ww), a.tmem_cols, a.one_pass, magic64(g.Kw * g.Kh), magic64(g.Kw), magic64(a.csplit), magic64(g.Kt),
                    g.Kw * g.Kh * g.Kt * BH * a.csplit, counter, probe};
   if (cudaMemsetAsync(counter, 0, sizeof(int), st) != cudaSuccess) return HVA_ECUDA;
-  hva_assign_tc_kernel<<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  if (a.probe != (probe != nullptr)) return HVA_EINVAL;
+  if (probe) hva_assign_tc_kernel<true><<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  else hva_assign_tc_kernel<false><<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }

@@ -10,6 +10,7 @@ struct HvaAssignTc {
   size_t smem;
   int one_pass;        // one MMA pass over the stacked [hi; lo] centroid tile
   int grid;            // resident CTAs (SMs x CTAs per SM): the kernel is persistent
+  bool probe;          // prepared for the instrumented instantiation (hva_cluster_ex with a probe buffer)
 };
 
 // time slices of a cell per CTA tile (<= 128 token rows): a cell of more than 128 tokens is split along t
@@ -28,7 +29,7 @@ static inline int hva_assign_tc_csplit(const HvaGrid& g) {
 // bf16, D = 128, k_h k_w <= 128 (a tile of whole time slices fits 128 rows), window of at most 256 centroids
 bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype);
 // X[BH,T,H,W,128] bf16; mu_hi / mu_lo [BH,Kt,Kh,Kw,128] bf16 (two-term split of the fp32 centroids)
-int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, HvaAssignTc* out);
+int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, bool probe, HvaAssignTc* out);
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
                          int* part_cnt, int* assign, float* lowe, int* counter, float* probe, cudaStream_t st);
 
@@ -42,7 +43,7 @@ int hva_mu_split_launch(int BH, int Nc, int D, const float* mu, void* mu_hi, voi
 #ifdef __CUDACC__
 namespace hva_tc_dev {
 // |tensor-pipe dot - exact dot| <= kEpsDot |x| |mu|: split error 2^-18 plus fp32 accumulation of 256 exact
-// products.  Observed on B200 (HVA_CLUSTER_PROBE, tests/test_gpu_parity.py): score error 4.6e-6 |x||mu| including the
+// products.  Observed on B200 (hva_cluster_ex probe, tests/test_gpu_parity.py): score error 4.6e-6 |x||mu| including the
 // rounding of the fp32 direct form it is compared with, against the 2 kEpsDot = 6.1e-5 assumed: 13x head room.
 constexpr float kEpsDot = 1.0f / 32768.0f;
 

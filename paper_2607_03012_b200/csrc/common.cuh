@@ -63,12 +63,12 @@ int hva_attention_tc_launch(const hva_shape* s, float scale, const void* Qp, con
 int hva_attention_simt_launch(const hva_shape* s, float scale, const void* Qp, const void* Kp, const void* Vp,
                               const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute,
                               cudaStream_t st, int tile_q);
-int hva_attention_dense_plan(int BH, int n, int tile_q, void* plan, const hva_plan_layout& L, cudaStream_t st);
+int hva_attention_dense_plan(int BH, int n, int tile_q, int tile_k, void* plan, const hva_plan_layout& L, cudaStream_t st);
 
 // hva_merge for the (batch, head) pairs bh0 .. bh0 + BH - 1 of a larger problem (chunked host path)
 int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k, const uint8_t* mask,
                      int32_t tile_q, int32_t tile_k, int32_t rounds, int32_t max_q_tiles, uint32_t seed, int32_t* group_of_cluster,
-                     int32_t* n_groups, uint8_t* group_mask, void* ws, size_t ws_bytes, void* stream);
+                     int32_t* n_groups, uint8_t* group_mask, uint32_t flags, void* ws, size_t ws_bytes, void* stream);
 
 struct HvaGrid;
 size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D);

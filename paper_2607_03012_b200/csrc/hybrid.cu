@@ -5,7 +5,6 @@
 //                       (DESIGN.md R-H3), or a full refresh of every centroid (R-H3').
 #include "common.cuh"
 #include "cluster_tc.cuh"
-#include <cstdlib>
 
 namespace {
 
@@ -291,11 +290,10 @@ __global__ void __launch_bounds__(D) hva_refresh_kernel(int n, int Nc, const T* 
 
 template <typename T, int D>
 int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, int refresh_all, int* assign, float* mu,
-               float* sums, int* sizes, int* newlab, char* split, int dtype, cudaStream_t st) {
+               float* sums, int* sizes, int* newlab, char* split, int dtype, uint32_t flags, cudaStream_t st) {
   int* oldlab = newlab + (size_t)BH * (m > 0 ? m : 1);
   const T* x = reinterpret_cast<const T*>(X);
-  const char* force = getenv("HVA_CLUSTER_SIMT");
-  if (m > 0 && hva_subset_tc_supported(D, dtype, Nc) && !(force && force[0] == '1')) {
+  if (m > 0 && hva_subset_tc_supported(D, dtype, Nc) && !(flags & HVA_FLAG_CLUSTER_SIMT)) {
     // tensor-pipe path: split the cached centroids, then the dense m x N_c x D filter with exact refine (hybrid_tc.cu)
     char* hi = split;
     char* lo = hi + hva_align((size_t)BH * Nc * D * 2);
@@ -360,6 +358,12 @@ extern "C" int hva_select_subset(int32_t BH, int32_t n, const float* lowe, int32
 extern "C" int hva_cluster_update(const hva_shape* s, int32_t Nc, const void* X, const int32_t* subset, int32_t m,
                                   int32_t refresh_all, int32_t* assign, float* mu, float* sums, int32_t* sizes, void* ws,
                                   size_t ws_bytes, void* stream) {
+  return hva_cluster_update_ex(s, Nc, X, subset, m, refresh_all, assign, mu, sums, sizes, 0u, ws, ws_bytes, stream);
+}
+
+extern "C" int hva_cluster_update_ex(const hva_shape* s, int32_t Nc, const void* X, const int32_t* subset, int32_t m,
+                                     int32_t refresh_all, int32_t* assign, float* mu, float* sums, int32_t* sizes, uint32_t flags,
+                                     void* ws, size_t ws_bytes, void* stream) {
   if (!s || !X || !subset || !assign || !mu || !sums || !sizes || !ws) return HVA_EINVAL;
   if (Nc < 1 || m < 0 || (s->D != 64 && s->D != 128)) return HVA_EINVAL;
   if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
@@ -370,7 +374,7 @@ extern "C" int hva_cluster_update(const hva_shape* s, int32_t Nc, const void* X,
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   int* newlab = reinterpret_cast<int*>(ws);
   char* split = reinterpret_cast<char*>(ws) + hva_align((size_t)BH * (m > 0 ? m : 1) * 8);
-#define HVA_DISPATCH(T, DD) return run_update<T, DD>(BH, n, Nc, m, X, subset, refresh_all, assign, mu, sums, sizes, newlab, split, s->dtype, st)
+#define HVA_DISPATCH(T, DD) return run_update<T, DD>(BH, n, Nc, m, X, subset, refresh_all, assign, mu, sums, sizes, newlab, split, s->dtype, flags, st)
   if (s->dtype == HVA_F32) { if (s->D == 64) HVA_DISPATCH(float, 64); HVA_DISPATCH(float, 128); }
   if (s->D == 64) HVA_DISPATCH(__nv_bfloat16, 64);
   HVA_DISPATCH(__nv_bfloat16, 128);

@@ -4,7 +4,6 @@
 // (DESIGN.md R-K3); each CTA scores kRowsPerCta query clusters per pass over mu^k: w_j = s^k_j exp(S_j - max_j S_j); sort by (w desc, j asc) with an in-smem
 // bitonic network; inclusive scan; k = first position with cum >= top_p * Z; keep at least kmin.
 #include "common.cuh"
-#include <cstdlib>
 
 namespace {
 
@@ -266,6 +265,12 @@ int launch_mask_warp(int BH, int Nq, int Nk, const float* mu_q, const float* mu_
 extern "C" int hva_build_mask(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, const float* mu_q, const float* mu_k,
                               const int32_t* sizes_k, float scale, float top_p, float min_kc, uint8_t* mask, void* ws,
                               size_t ws_bytes, void* stream) {
+  return hva_build_mask_ex(BH, Nq, Nk, D, mu_q, mu_k, sizes_k, scale, top_p, min_kc, mask, 0u, ws, ws_bytes, stream);
+}
+
+extern "C" int hva_build_mask_ex(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, const float* mu_q, const float* mu_k,
+                                 const int32_t* sizes_k, float scale, float top_p, float min_kc, uint8_t* mask, uint32_t flags,
+                                 void* ws, size_t ws_bytes, void* stream) {
   (void)ws; (void)ws_bytes;
   if (!mu_q || !mu_k || !sizes_k || !mask) return HVA_EINVAL;
   if (BH < 1 || Nq < 1 || Nk < 1 || (D != 64 && D != 128)) return HVA_EINVAL;
@@ -276,8 +281,7 @@ extern "C" int hva_build_mask(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, con
   int kmin = (int)ceil((double)min_kc * (double)Nk);
   size_t smem = (size_t)P * 12 + (size_t)kRowsPerCta * Nk * 8 + (size_t)kRowsPerCta * D * 8 + kMaskThreads * 8 + 16;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  const char* force = getenv("HVA_MASK_BLOCKSORT");
-  if (top_p < 1.f && Nk <= 1024 && !(force && force[0] == '1')) {   // warp-per-row register sort
+  if (top_p < 1.f && Nk <= 1024 && !(flags & HVA_FLAG_MASK_BLOCKSORT)) {   // warp-per-row register sort
 #define HVA_MASK_WARP(DD)                                                                                                             \
     do {                                                                                                                              \
       if (Nk <= 256) return launch_mask_warp<DD, 8>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st);  \

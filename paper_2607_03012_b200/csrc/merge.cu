@@ -203,10 +203,6 @@ size_t hva_merge_inter_bytes(int BH, int Nq);
 int hva_merge_nterms_launch(int BH, int Nk, const int* sizes_k, int* nterms, cudaStream_t st);
 int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, cudaStream_t st);
 
-static bool merge_use_inter(int Nq) {
-  const char* force = getenv("HVA_MERGE_SIMT");
-  return Nq <= 2048 && !(force && force[0] == '1');
-}
 
 size_t hva_merge_ws_bytes(int BH, int Nq, int Nk) {
   size_t Wd = (Nk + 31) / 32;
@@ -221,7 +217,7 @@ extern "C" size_t hva_merge_workspace_bytes(int32_t BH, int32_t Nq, int32_t Nk) 
 
 int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k,
                          const uint8_t* mask, int32_t tile_q, int32_t tile_k, int32_t rounds, int32_t max_q_tiles,
-                         uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask, void* ws,
+                         uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask, uint32_t flags, void* ws,
                          size_t ws_bytes, void* stream) {
   if (!sizes_q || !sizes_k || !mask || !group_of_cluster || !n_groups || !group_mask || !ws) return HVA_EINVAL;
   if (BH < 1 || Nq < 1 || Nk < 1 || tile_q < 1 || tile_k < 1 || rounds < 0 || max_q_tiles < 0) return HVA_EINVAL;
@@ -241,7 +237,7 @@ int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int3
   p.side = reinterpret_cast<int*>(w); w += a4;
   p.remap = reinterpret_cast<int*>(w); w += a4;
   p.best = reinterpret_cast<unsigned long long*>(w); w += hva_align((size_t)BH * Nq * 8);
-  const bool use_inter = rounds > 0 && merge_use_inter(Nq);
+  const bool use_inter = rounds > 0 && Nq <= 2048 && !(flags & HVA_FLAG_MERGE_SIMT);
   const int Nqp = (Nq + 127) / 128 * 128;
   int* inter = reinterpret_cast<int*>(w);
   int* nterms = reinterpret_cast<int*>(w + hva_align((size_t)BH * Nqp * Nqp * 4));
@@ -274,5 +270,13 @@ extern "C" int hva_merge(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* size
                          uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask, void* ws,
                          size_t ws_bytes, void* stream) {
   return hva_merge_offset(0, BH, Nq, Nk, sizes_q, sizes_k, mask, tile_q, tile_k, rounds, max_q_tiles, seed, group_of_cluster, n_groups,
-                          group_mask, ws, ws_bytes, stream);
+                          group_mask, 0u, ws, ws_bytes, stream);
+}
+
+extern "C" int hva_merge_ex(int32_t BH, int32_t Nq, int32_t Nk, const int32_t* sizes_q, const int32_t* sizes_k,
+                            const uint8_t* mask, int32_t tile_q, int32_t tile_k, int32_t rounds, int32_t max_q_tiles,
+                            uint32_t seed, int32_t* group_of_cluster, int32_t* n_groups, uint8_t* group_mask, uint32_t flags,
+                            void* ws, size_t ws_bytes, void* stream) {
+  return hva_merge_offset(0, BH, Nq, Nk, sizes_q, sizes_k, mask, tile_q, tile_k, rounds, max_q_tiles, seed, group_of_cluster, n_groups,
+                          group_mask, flags, ws, ws_bytes, stream);
 }

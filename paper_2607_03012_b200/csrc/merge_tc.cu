@@ -185,11 +185,8 @@ int hva_merge_nterms_launch(int BH, int Nk, const int* sizes_k, int* nterms, cud
 int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, cudaStream_t st) {
   InterParams p{Nq, Nk, (Nk + 31) / 32, (Nq + 127) / 128 * 128, chi, sizes_k, nterms, inter};
   const size_t smem = 1024 + 5 * (size_t)kTileB + 8 * 16 + 64;
-  static bool attr = false;
-  if (!attr) {
-    if (cudaFuncSetAttribute(hva_merge_inter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return HVA_ECUDA;
-    attr = true;
-  }
+  // (per device and cheap: set on every call rather than behind a process-wide flag)
+  if (cudaFuncSetAttribute(hva_merge_inter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return HVA_ECUDA;
   const int nrb = p.Nqp / 128;
   hva_merge_inter_kernel<<<dim3(nrb, (nrb + 3) / 4, BH), kThreadsG, smem, st>>>(p);
   HVA_CHECK_LAUNCH();

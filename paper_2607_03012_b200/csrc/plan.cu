@@ -226,12 +226,12 @@ __global__ void hva_permute_kernel(size_t rows_total, int n, int row_chunks, con
   else Y[other * row_chunks + q] = __ldg(X + row * row_chunks + q);            // X[perm[i]] = Xp[i]
 }
 
-__global__ void hva_dense_plan_kernel(int n, int tile_q, PlanPtrs P) {
+__global__ void hva_dense_plan_kernel(int n, int tile_q, int tile_k, PlanPtrs P) {
   const int bh = blockIdx.x, tid = threadIdx.x;
   for (int i = tid; i < n; i += blockDim.x) {
     P.perm_q[(size_t)bh * n + i] = i; P.inv_perm_q[(size_t)bh * n + i] = i; P.perm_k[(size_t)bh * n + i] = i;
   }
-  int rt = (n + tile_q - 1) / tile_q;
+  int rt = (n + tile_q - 1) / tile_q, kt = (n + tile_k - 1) / tile_k;
   int* work = P.work + (size_t)bh * P.work_cap;
   for (int t = tid; t < rt; t += blockDim.x) work[t] = 0 | (t << 16);
   if (tid == 0) {
@@ -241,7 +241,7 @@ __global__ void hva_dense_plan_kernel(int n, int tile_q, PlanPtrs P) {
     P.work_cnt[bh] = rt;
     hva_stats s = {};
     s.n_groups = 1; s.q_tiles = rt; s.q_rows_valid = n; s.q_rows_padded = (int64_t)rt * tile_q;
-    s.k_cols_valid = n; s.k_cols_padded = (int64_t)rt * tile_q; s.tiles_executed = (int64_t)rt * rt;
+    s.k_cols_valid = n; s.k_cols_padded = (int64_t)kt * tile_k; s.tiles_executed = (int64_t)rt * kt;
     s.pairs_valid = (int64_t)n * n;
     P.stats[bh] = s;
   }
@@ -330,9 +330,9 @@ extern "C" int hva_unpermute(const hva_shape* s, const void* Xp, const int32_t* 
   return permute_common(s, Xp, perm, X, stream, 1);
 }
 
-int hva_attention_dense_plan(int BH, int n, int tile_q, void* plan, const hva_plan_layout& L, cudaStream_t st) {
+int hva_attention_dense_plan(int BH, int n, int tile_q, int tile_k, void* plan, const hva_plan_layout& L, cudaStream_t st) {
   PlanPtrs P = plan_ptrs(plan, L);
-  hva_dense_plan_kernel<<<BH, 256, 0, st>>>(n, tile_q, P);
+  hva_dense_plan_kernel<<<BH, 256, 0, st>>>(n, tile_q, tile_k, P);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }

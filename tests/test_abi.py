@@ -59,3 +59,40 @@ def test_argument_checks_return_error_codes_without_cuda(lib):
     bad.D = 96
     assert lib.hva_workspace_bytes(C.byref(bad), C.byref(cfg)) == 0
     assert lib.hva_merge_workspace_bytes(0, 8, 8) == 0
+
+
+def test_state_and_plan_layout_queries(lib):
+    """hva_state_describe / hva_plan_workspace_bytes: the binding no longer mirrors private layouts of api.cu / plan.cu."""
+    wl = inputs.C4
+    shape, cfg = b.make_shape(wl), b.make_config(wl, subset_frac=0.15)
+    L = b.hva_state_layout()
+    assert lib.hva_state_describe(C.byref(shape), C.byref(cfg), C.byref(L)) == 0
+    assert L.total == lib.hva_state_bytes(C.byref(shape), C.byref(cfg))
+    assert list(L.n_clusters) == [990, 990] and L.m == 17820            # floor(0.15 * 118800 + 1/2)  (P:322, R-H2)
+    offs = sorted([L.assign[0], L.mu[0], L.sums[0], L.sizes[0], L.subset[0], L.assign[1], L.mu[1], L.sums[1], L.sizes[1], L.subset[1]])
+    assert offs[0] == 0 and all(o % 256 == 0 for o in offs) and len(set(offs)) == 10 and offs[-1] < L.total
+    assert L.mu[0] - L.assign[0] >= 24 * wl.n * 4 and L.sums[0] - L.mu[0] >= 24 * 990 * 128 * 4
+    assert lib.hva_state_describe(C.byref(shape), C.byref(cfg), C.c_void_p(0)) == -1
+    assert lib.hva_plan_workspace_bytes(24, wl.n, 990, 990) >= 24 * 117 * 990 * 4
+    assert lib.hva_plan_workspace_bytes(0, wl.n, 990, 990) == 0
+
+
+def test_host_call_validates_before_enqueueing(lib):
+    """hva_forward_host: bad arguments / a short workspace are reported before any copy is enqueued (no CUDA needed)."""
+    wl = inputs.C2
+    shape, cfg = b.make_shape(wl), b.make_config(wl)
+    null, one = C.c_void_p(0), C.c_void_p(16)
+    assert lib.hva_forward_host(C.byref(shape), C.byref(cfg), null, one, one, one, 0, null, one, one, C.c_size_t(1 << 40), null) == -1
+    assert lib.hva_forward_host(C.byref(shape), C.byref(cfg), one, one, one, one, 7, null, one, one, C.c_size_t(1 << 40), null) == -1
+    assert lib.hva_forward_host(C.byref(shape), C.byref(cfg), one, one, one, one, 1, null, one, one, C.c_size_t(1 << 40), null) == -1  # intermediate without state
+    assert lib.hva_forward_host(C.byref(shape), C.byref(cfg), one, one, one, one, 0, null, one, one, C.c_size_t(1024), null) == -2
+
+
+def test_library_reads_no_environment_and_keeps_no_probe_pointers():
+    """SURVEY section 5 'no env vars, no global state': kernel selection is an explicit `flags` argument."""
+    csrc = os.path.join(ROOT, "paper_2607_03012_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        src = open(os.path.join(csrc, f)).read()
+        assert "getenv" not in src and "strtoull" not in src, f
+    cfg = b.make_config(inputs.C2, flags=b.HVA_FLAG_ATTN_SIMT | b.HVA_FLAG_MERGE_SIMT)
+    assert cfg.flags == 10 and C.sizeof(b.hva_config) == 4 * (12 + 12)
