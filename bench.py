@@ -348,20 +348,27 @@ def report_assign_phases(b, wl, args):
     _, K, _ = inputs.make_qkv(wl, heads=heads)
     X = K.cuda().contiguous()
     shape = b.make_shape(wl, heads=len(heads))
-    names = ["setup", "tile_wait", "xsq", "mma1_wait", "epilogue", "scan_refine_store", "sync", "onehot_fence", "sums_mma", "end_sync"]
+    roles = {"scan_group0": ["loop", "table_wait", "tile_wait_xsq", "mma1_wait", "scan_refine_store", "onehot_tile_wait", "onehot_fence_arrive"],
+             "epilogue": ["loop", "table_wait", "sums_wait", "stores"],
+             "loader": ["draw_issue", "slot_wait", "header", "centroid_buf_wait", "boxes", "draw_wait"],
+             "mma1": ["loop", "header_wait", "tables", "tile_wait", "issue"],
+             "mma2": ["loop", "table_wait", "onehot_wait", "issue"]}
     cells = 1
     for d, k in zip((wl.T, wl.H, wl.W), wl.cell):
         cells *= -(-d // k)
     for lowe, iters in ((False, 1), (True, 1), (False, wl.iters)):
         b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe, want_sums=False)
-        probe = torch.zeros(32, dtype=torch.float32, device="cuda")
+        probe = torch.zeros(64, dtype=torch.float32, device="cuda")
         b.hva_cluster(shape, wl.cell, wl.win, iters, X, want_lowe=lowe, want_sums=False, probe=probe)
         torch.cuda.synchronize()
         pr = probe.cpu().numpy()
         ntiles = cells * len(heads) * iters
-        clk = {n: int(round(float(pr[16 + k]) / ntiles)) for k, n in enumerate(names)}
-        print(json.dumps({"report": "assign-phases", "workload": wl.name, "heads": len(heads), "iters": iters, "lowe_ratio": lowe,
-                          "timing_build": bool(pr[16:26].sum() > 0), "clk_per_tile": clk, "clk_per_tile_sum": int(sum(clk.values()))}))
+        out = {"report": "assign-phases", "workload": wl.name, "heads": len(heads), "iters": iters, "lowe_ratio": lowe,
+               "timing_build": bool(pr[16:56].sum() > 0), "unit": "clk per tile of the CTA (scan_group0 handles every third tile)"}
+        for r, (role, names) in enumerate(roles.items()):
+            out[role] = {n: int(round(float(pr[16 + 8 * r + k]) / ntiles)) for k, n in enumerate(names)}
+            out[role]["sum"] = int(sum(out[role].values()))
+        print(json.dumps(out))
 
 
 def report_hybrid(b, wl, args):

@@ -9,11 +9,11 @@
 // fixed cell order, by hva_finalize_kernel (Alg. 2 line 23: mu <- z/n, empty keeps mu).
 #include "common.cuh"
 #include "cluster_tc.cuh"
+#include <algorithm>
 
 namespace {
 
 constexpr int kThreads = 128;
-constexpr int kCB = 9;  // candidates evaluated per register block
 
 __device__ __forceinline__ void load8(const float* p, float x[8]) {
   float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
@@ -133,37 +133,22 @@ __global__ void __launch_bounds__(kThreads) hva_assign_kernel(ClusterParams p) {
     if (valid) {
       float best = __int_as_float(0x7f800000), second = __int_as_float(0x7f800000);
       const T* xr = s_x + (size_t)li * kRowStride;
-      for (int v0 = 0; v0 < g.nwin; v0 += kCB) {
-        float acc[kCB];
+      // the direct form in the summation order of cluster_tc.cuh (D/4 partial sums of 4 dims, halving tree): the labels and the
+      // Lowe ratio of the tensor-pipe kernel are those of this kernel bit for bit
+      for (int v = 0; v < g.nwin; ++v) {
+        float pr[D / 4];
 #pragma unroll
-        for (int j = 0; j < kCB; ++j) acc[j] = 0.f;
         for (int c0 = 0; c0 < D; c0 += 8) {
           float x[8];
           load8(xr + c0, x);
-#pragma unroll
-          for (int j = 0; j < kCB; ++j) {
-            int v = min(v0 + j, g.nwin - 1);
-            const float4 m0 = *reinterpret_cast<const float4*>(s_mu + (size_t)v * D + c0);
-            const float4 m1 = *reinterpret_cast<const float4*>(s_mu + (size_t)v * D + c0 + 4);
-            float d;
-            d = x[0] - m0.x; acc[j] = fmaf(d, d, acc[j]);
-            d = x[1] - m0.y; acc[j] = fmaf(d, d, acc[j]);
-            d = x[2] - m0.z; acc[j] = fmaf(d, d, acc[j]);
-            d = x[3] - m0.w; acc[j] = fmaf(d, d, acc[j]);
-            d = x[4] - m1.x; acc[j] = fmaf(d, d, acc[j]);
-            d = x[5] - m1.y; acc[j] = fmaf(d, d, acc[j]);
-            d = x[6] - m1.z; acc[j] = fmaf(d, d, acc[j]);
-            d = x[7] - m1.w; acc[j] = fmaf(d, d, acc[j]);
-          }
+          const float4 m0 = *reinterpret_cast<const float4*>(s_mu + (size_t)v * D + c0);
+          const float4 m1 = *reinterpret_cast<const float4*>(s_mu + (size_t)v * D + c0 + 4);
+          pr[c0 / 4] = hva_tc_dev::hva_sq4(x[0], x[1], x[2], x[3], m0);
+          pr[c0 / 4 + 1] = hva_tc_dev::hva_sq4(x[4], x[5], x[6], x[7], m1);
         }
-#pragma unroll
-        for (int j = 0; j < kCB; ++j) {
-          if (v0 + j < g.nwin) {
-            float dd = acc[j];
-            if (dd < best) { second = best; best = dd; lab = v0 + j; }
-            else if (dd < second) second = dd;
-          }
-        }
+        const float dd = hva_tc_dev::hva_tree_sum(pr);
+        if (dd < best) { second = best; best = dd; lab = v; }
+        else if (dd < second) second = dd;
       }
       size_t tok = (size_t)(t * g.H + h) * g.W + w;
       if (p.assign) {
@@ -340,7 +325,7 @@ size_t assign_smem_bytes(const HvaGrid& g, int D, int esize) {
 }
 
 struct ClusterWs {
-  float* part; int* part_cnt; __nv_bfloat16 *hi, *lo; float* musq; int* counter;
+  float* part; int* part_cnt; __nv_bfloat16 *hi, *lo; float* musq; int* counter; float* xsq;
 };
 
 template <typename T, int D>
@@ -375,8 +360,9 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
   for (int it = 0; it < iters; ++it) {
     bool last = (it == iters - 1);
     if (tc) {
+      // the |x|^2 bound of the filter margin is the same in every pass: written by the first, read by the others
       HVA_TRY(hva_assign_tc_launch(atc, g, BH, mu, ws.musq, ws.part, ws.part_cnt, last ? assign : nullptr, last ? lowe : nullptr,
-                                   ws.counter, probe, st));
+                                   ws.xsq, iters == 1 ? 0 : (it == 0 ? 1 : 2), ws.counter, probe, st));
     } else {
       ClusterParams p{g, BH, X, mu, ws.part, ws.part_cnt, last ? assign : nullptr, last ? lowe : nullptr};
       hva_assign_kernel<T, D><<<grid, kThreads, smem, st>>>(p);
@@ -393,7 +379,8 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
 size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D) {
   const size_t cs = (size_t)hva_assign_tc_csplit(g);
   return hva_align((size_t)BH * g.Nc * cs * g.nwin * D * sizeof(float)) + hva_align((size_t)BH * g.Nc * cs * g.nwin * sizeof(int)) +
-         2 * hva_align((size_t)BH * g.Nc * D * sizeof(__nv_bfloat16)) + hva_align((size_t)BH * g.Nc * sizeof(float)) + hva_align(sizeof(int));
+         2 * hva_align((size_t)BH * g.Nc * D * sizeof(__nv_bfloat16)) + hva_align((size_t)BH * g.Nc * sizeof(float)) + hva_align(sizeof(int)) +
+         hva_align((size_t)BH * g.n * sizeof(float));
 }
 
 int hva_mu_split_launch(int BH, int Nc, int D, const float* mu, void* mu_hi, void* mu_lo, float* musq, cudaStream_t st) {
@@ -429,6 +416,20 @@ extern "C" int hva_cluster_ex(const hva_shape* s, const int32_t cell[3], const i
   if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
   HvaGrid g = hva_make_grid(s, cell, win);
   int BH = s->B * s->heads;
+#ifdef HVA_HEAD_GROUP
+  if (BH > HVA_HEAD_GROUP && s->B == 1) {   // EXPERIMENT: all iterations of a few heads back to back (X of a head stays in L2)
+    const size_t es = s->dtype == HVA_F32 ? 4 : 2;
+    for (int h0 = 0; h0 < BH; h0 += HVA_HEAD_GROUP) {
+      hva_shape sub = *s;
+      sub.heads = std::min(HVA_HEAD_GROUP, BH - h0);
+      const size_t o = (size_t)h0;
+      HVA_TRY(hva_cluster_ex(&sub, cell, win, iters, (const char*)X + o * g.n * s->D * es, mu_init ? mu_init + o * g.Nc * s->D : nullptr,
+                             assign + o * g.n, mu + o * g.Nc * s->D, sizes + o * g.Nc, sums ? sums + o * g.Nc * s->D : nullptr,
+                             lowe ? lowe + o * g.n : nullptr, flags, probe, ws, ws_bytes, stream));
+    }
+    return HVA_OK;
+  }
+#endif
   if ((size_t)g.nwin * hva_assign_tc_csplit(g) > 1024 || (size_t)BH * g.Nc * g.nwin * hva_assign_tc_csplit(g) >= (1ull << 32)) return HVA_EUNSUPPORTED;
   if (ws_bytes < hva_cluster_ws_bytes(g, BH, s->D)) return HVA_EWORKSPACE;
   ClusterWs cw;
@@ -440,7 +441,8 @@ extern "C" int hva_cluster_ex(const hva_shape* s, const int32_t cell[3], const i
     cw.hi = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
     cw.lo = reinterpret_cast<__nv_bfloat16*>(w); w += hva_align((size_t)BH * g.Nc * s->D * sizeof(__nv_bfloat16));
     cw.musq = reinterpret_cast<float*>(w); w += hva_align((size_t)BH * g.Nc * sizeof(float));
-    cw.counter = reinterpret_cast<int*>(w);
+    cw.counter = reinterpret_cast<int*>(w); w += hva_align(sizeof(int));
+    cw.xsq = reinterpret_cast<float*>(w);
   }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
 #define HVA_DISPATCH(T, DD) return run_cluster<T, DD>(g, BH, iters, X, mu_init, assign, mu, sizes, sums, lowe, cw, s->dtype, flags, probe, st)

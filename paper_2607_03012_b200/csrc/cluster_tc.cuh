@@ -6,10 +6,11 @@
 struct HvaAssignTc {
   CUtensorMap map_x, map_hi, map_lo;
   int npad, rows_a, csplit, ct;
-  uint32_t tmem_cols;
+  int NT, NB, NW;      // token slots, centroid buffers, scan warpgroups of the persistent CTA
+  int cols;            // TMEM columns per token slot
   size_t smem;
   int one_pass;        // one MMA pass over the stacked [hi; lo] centroid tile
-  int grid;            // resident CTAs (SMs x CTAs per SM): the kernel is persistent
+  int grid;            // one persistent CTA per SM
   bool probe;          // prepared for the instrumented instantiation (hva_cluster_ex with a probe buffer)
 };
 
@@ -31,7 +32,7 @@ bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype);
 // X[BH,T,H,W,128] bf16; mu_hi / mu_lo [BH,Kt,Kh,Kw,128] bf16 (two-term split of the fp32 centroids)
 int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, bool probe, HvaAssignTc* out);
 int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const float* mu, const float* musq, float* part,
-                         int* part_cnt, int* assign, float* lowe, int* counter, float* probe, cudaStream_t st);
+                         int* part_cnt, int* assign, float* lowe, float* xsq, int xsq_mode, int* counter, float* probe, cudaStream_t st);
 
 // Window-less variant for the hybrid subset step (hybrid_tc.cu): subset tokens against ALL centroids.
 bool hva_subset_tc_supported(int D, int dtype, int Nc);
@@ -58,26 +59,39 @@ __device__ __forceinline__ void unpack8(const uint4& r, float x[8]) {   // bf16 
   x[6] = __uint_as_float(r.w << 16); x[7] = __uint_as_float(r.w & 0xffff0000u);
 }
 
-// exact direct form sum_c (x_c - mu_c)^2, fp32, sequential in c (Eq. 5)
+// The exact direct form sum_c (x_c - mu_c)^2 in fp32 (Eq. 5) with a FIXED summation order shared by every kernel that decides
+// a label (this file's users and the CUDA-core kernel of cluster.cu): D/4 partial sums over 4 consecutive dims each
+// (p = d0*d0; p = fma(d_k, d_k, p), k = 1..3), combined by the halving tree  p_j += p_{j + o},  o = D/8, D/16, ..., 1.
+// One 128-long dependent fma chain cost a refining lane ~6 K clk per candidate (and stalled the whole tile pipeline behind it);
+// the D/4 chains are independent.
+__device__ __forceinline__ float hva_sq4(float x0, float x1, float x2, float x3, const float4& m) {
+  float d = x0 - m.x, p = d * d;
+  d = x1 - m.y; p = fmaf(d, d, p);
+  d = x2 - m.z; p = fmaf(d, d, p);
+  d = x3 - m.w; p = fmaf(d, d, p);
+  return p;
+}
+template <int N>
+__device__ __forceinline__ float hva_tree_sum(float (&p)[N]) {
+#pragma unroll
+  for (int o = N / 2; o >= 1; o >>= 1) {
+#pragma unroll
+    for (int j = 0; j < o; ++j) p[j] += p[j + o];
+  }
+  return p[0];
+}
 __device__ __forceinline__ float direct_dist(const unsigned char* sA, int half_bytes, int r, const float* __restrict__ mu) {
-  float acc = 0.f;
-#pragma unroll 4
+  float pr[32];
+#pragma unroll
   for (int q = 0; q < 16; ++q) {
     float x[8];
     unpack8(*x_chunk(sA, half_bytes, r, q), x);
     const float4 m0 = __ldg(reinterpret_cast<const float4*>(mu) + 2 * q);
     const float4 m1 = __ldg(reinterpret_cast<const float4*>(mu) + 2 * q + 1);
-    float d;
-    d = x[0] - m0.x; acc = fmaf(d, d, acc);
-    d = x[1] - m0.y; acc = fmaf(d, d, acc);
-    d = x[2] - m0.z; acc = fmaf(d, d, acc);
-    d = x[3] - m0.w; acc = fmaf(d, d, acc);
-    d = x[4] - m1.x; acc = fmaf(d, d, acc);
-    d = x[5] - m1.y; acc = fmaf(d, d, acc);
-    d = x[6] - m1.z; acc = fmaf(d, d, acc);
-    d = x[7] - m1.w; acc = fmaf(d, d, acc);
+    pr[2 * q] = hva_sq4(x[0], x[1], x[2], x[3], m0);
+    pr[2 * q + 1] = hva_sq4(x[4], x[5], x[6], x[7], m1);
   }
-  return acc;
+  return hva_tree_sum(pr);
 }
 
 }  // namespace hva_tc_dev
