@@ -20,8 +20,8 @@
 // direct form; with the Lowe ratio requested (Eq. 6) the best and the second best are always exact.
 //
 // Round 2 organisation: ONE persistent CTA per SM (640 threads) that keeps NT tiles in flight in a ring of token slots
-// (5 x 30 KB at the 3x5x8 cells), each with its own TMEM score columns, slot table and mbarriers; tiles are drawn from a
-// device counter.  Roles (nothing but mbarriers between them, no block barrier in the steady state):
+// (5 x 30 KB at the 3x5x8 cells), each with its own TMEM score columns, slot table and mbarriers; CTA b takes the tiles
+// b, b + gridDim.x, ...  Roles (nothing but mbarriers between them, no block barrier in the steady state):
 //   warps 0-11   NW = 3 scan warpgroups, tile q goes to group q mod NW: thread = token row = TMEM lane: scan / refine /
 //                label store / one-hot write into the group's own one-hot tile
 //   warps 12-15  epilogue warpgroup, every tile in order: thread = feature dim = TMEM lane: partial-row stores
@@ -45,7 +45,7 @@ using namespace hva_tc_dev;
 
 constexpr int kD = 128;
 constexpr int kMaxNW = 3;                         // scan warpgroups
-constexpr int kMaxNT = 8;                         // token slots
+constexpr int kMaxNT = 8;                         // pipeline slots / token buffers
 constexpr int kEpiWarp0 = 4 * kMaxNW;             // first warp of the epilogue warpgroup
 constexpr int kLoadWarp = kEpiWarp0 + 4, kMma1Warp = kLoadWarp + 1, kMma2Warp = kLoadWarp + 2, kTableWarp = kLoadWarp + 3;
 constexpr int kThreads = 32 * (kTableWarp + 1);   // 640
@@ -65,12 +65,13 @@ struct AssignTcParams {
   int rows_a;          // tile tokens padded to the MMA K granule (16 rows)
   int csplit, ct;      // a cell of more than 128 tokens is split along t into csplit tiles of ct time slices
   uint32_t m_khw, m_kw, m_whw, m_ww;   // fast_div multipliers for k_h k_w, k_w, w_h w_w, w_w
-  int NT, NB, NW;      // token slots, centroid buffers, scan warpgroups (= one-hot tiles)
+  int NT, NB, NW;      // token buffers, centroid buffers, scan warpgroups (= one-hot tiles)
+  int NS;              // pipeline slots (TMEM columns, slot tables, barriers) >= NT: a token buffer is free once MMA 2 has read it, its
+                       // TMEM columns and tables only after the epilogue
   int cols;            // TMEM columns per token slot
   int one_pass;        // 2 npad <= 256: one MMA pass over [hi; lo] stacked as 2 npad score columns (the token tile is read once)
   unsigned long long d_khw, d_kw, d_cs, d_kt;   // fast_div64 multipliers of the tile decode: K_h K_w, K_w, csplit, K_t
-  int n_items;         // K_w * K_h * K_t * BH * csplit tiles: a CTA starts with tile blockIdx.x and draws the following ones
-  int* counter;        // from this device counter (zero at launch), so that the SMs finish together
+  int n_items;         // K_w * K_h * K_t * BH * csplit tiles: CTA b takes tiles b, b + gridDim.x, ...
   float* probe;        // instrumented instantiation: max |score_tc - score_exact| / (|x| max|mu|)
 };
 
@@ -131,7 +132,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int ctok = p.ct * g.kh * g.kw, nwin = g.nwin, npad = p.npad;   // token rows of a tile
   const int half_a = p.rows_a * 128, half_b = npad * 128;
-  const int NT = p.NT, NB = p.NB, NW = p.NW;
+  const int NT = p.NT, NB = p.NB, NW = p.NW, NS = p.NS;
 
   // Shared memory (offsets from a 1024-byte aligned base):
   //   sA  [NT][2 halves][rows_a][128 B]           token slots (A of MMA 1, K-major SW128; A of MMA 2, MN-major)
@@ -148,9 +149,9 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
   unsigned char* sB_all = sA_all + (size_t)NT * 2 * half_a;
   unsigned char* sP_all = sB_all + (size_t)NB * 4 * half_b;
   float* s_c_all = reinterpret_cast<float*>(sP_all + (size_t)NW * 2 * half_b);
-  int* s_cnt_all = reinterpret_cast<int*>(s_c_all + NT * npad);
-  uint16_t* s_u_all = reinterpret_cast<uint16_t*>(s_cnt_all + NT * npad);
-  AssignTcShared* SH = reinterpret_cast<AssignTcShared*>(reinterpret_cast<unsigned char*>(s_u_all + NT * npad) + ((8 - ((NT * npad * 2) & 7)) & 7));
+  int* s_cnt_all = reinterpret_cast<int*>(s_c_all + NS * npad);
+  uint16_t* s_u_all = reinterpret_cast<uint16_t*>(s_cnt_all + NS * npad);
+  AssignTcShared* SH = reinterpret_cast<AssignTcShared*>(reinterpret_cast<unsigned char*>(s_u_all + NS * npad) + ((8 - ((NS * npad * 2) & 7)) & 7));
 
   if (warp == kLoadWarp) tmem_alloc(&SH->tmem_base, kTmemCols);
 
@@ -166,7 +167,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
     return t;
   };
   if (tid == 0) {
-    for (int i = 0; i < NT; ++i) {
+    for (int i = 0; i < NS; ++i) {
       TileSlot* S = &SH->slot[i];
       mbar_init(&S->hdr_ready, 1); mbar_init(&S->table_ready, 32); mbar_init(&S->full, 1); mbar_init(&S->mma_done, 1);
       mbar_init(&S->onehot, 128); mbar_init(&S->sum_done, 1); mbar_init(&S->free_, 128);
@@ -209,17 +210,12 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
     const uint32_t tile_bytes = (uint32_t)(2 * ctok * 128 + 4 * nwin * 128);
     int item = blockIdx.x;                   // (the grid never exceeds n_items)
     int n_term = 0;
-    int i = 0, jb = 0, ib = 0;               // token slot of tile q, centroid buffer of tile q, token slot of tile q - NB
-    uint32_t par = 0, parb = 0;              // parity of the slot's barriers for tile q / for tile q - NB
+    int i = 0, jb = 0, ib = 0, ia = 0, ix = 0;   // slot / centroid buffer / token buffer of tile q; slots of tiles q - NB, q - NT
+    uint32_t par = 0, parb = 0, parx = 0;        // parity of the slot's barriers for tile q / q - NB / q - NT
     for (int q = 0; n_term < NW; ++q) {
       TileSlot* S = &SH->slot[i];
-      // the next tile id: the atomic is in flight while this tile is set up
-      // (one predicated instruction that writes its result over the initial value: a branch around the atom would merge the two
-      // values right behind it and wait for the round trip there)
-      int nxt = -1;
-      asm volatile("{\n\t.reg .pred pa;\n\tsetp.ne.b32 pa, %2, 0;\n\t@pa atom.global.add.u32 %0, [%1], 1;\n\t}" : "+r"(nxt) : "l"(p.counter), "r"((int)(item >= 0 && lane == 0)) : "memory");
       CMARK(0);
-      if (q >= NT) mbar_wait(&S->free_, par ^ 1u);          // the slot's previous tile has left the pipeline
+      if (q >= NS) mbar_wait(&S->free_, par ^ 1u);          // the slot's previous tile has left the pipeline
       CMARK(1);
       TRACE(0, q);
       Tile t{0, 0, 0, 0, 0};
@@ -230,9 +226,13 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
           CMARK(2);
           mbar_wait(&SH->slot[ib].mma_done, parb);
           CMARK(3);
-          if (++ib == NT) { ib = 0; parb ^= 1u; }
+          if (++ib == NS) { ib = 0; parb ^= 1u; }
         }
-        unsigned char* sA = sA_all + (size_t)i * 2 * half_a;
+        if (q >= NT) {                       // the token buffer is free once MMA 2 of the tile NT tiles back has read it
+          mbar_wait(&SH->slot[ix].sum_done, parx);
+          if (++ix == NS) { ix = 0; parx ^= 1u; }
+        }
+        unsigned char* sA = sA_all + (size_t)ia * 2 * half_a;
         unsigned char* sBhi = sB_all + (size_t)jb * 4 * half_b;
         unsigned char* sBlo = sBhi + half_b;
         const int st = hva_win_start(t.ut, g.wt, g.Kt), sh = hva_win_start(t.uh, g.wh, g.Kh), sw = hva_win_start(t.uw, g.ww, g.Kw);
@@ -249,21 +249,24 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
         __syncwarp();
         CMARK(4);
         TRACE(1, q);
-        nxt = __shfl_sync(0xffffffffu, nxt, 0) + (int)gridDim.x;
-        item = nxt < p.n_items ? nxt : -1;
+        // static round robin: every tile costs the same within ~1 %, so a device counter buys nothing here -- and ptxas turns a
+        // uniform-address atom into a warp-aggregated sequence whose shuffle waits for the round trip right behind it (1 K clk per tile)
+        item += (int)gridDim.x;
+        if (item >= p.n_items) item = -1;
         CMARK(5);
       } else {
         ++n_term;                            // one terminator header per scan group
       }
-      if (++i == NT) { i = 0; par ^= 1u; }
+      if (++i == NS) { i = 0; par ^= 1u; }
       if (++jb == NB) jb = 0;
+      if (++ia == NT) ia = 0;
     }
     CFLUSH(2);
   } else if (warp == kMma1Warp) {
     // ================================================================ MMA 1 (scores) as soon as a tile's boxes have landed
     const uint32_t idesc1 = umma_idesc_bf16(128, (uint32_t)(p.one_pass ? 2 * npad : npad), 0, 0);
     const uint32_t ha = (uint32_t)half_a >> 4, hb2 = (uint32_t)(2 * half_b) >> 4;
-    int i = 0, jb = 0;
+    int i = 0, jb = 0, ia = 0;
     uint32_t par = 0;
     for (;;) {
       TileSlot* S = &SH->slot[i];
@@ -276,7 +279,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       TRACE(2, tq);
       tc_fence_after();
       // descriptors in uniform registers; a k-step only adds a constant to the start-address field
-      const uint64_t da = umma_desc(smem_u32(sA_all + (size_t)i * 2 * half_a), 16, 1024);
+      const uint64_t da = umma_desc(smem_u32(sA_all + (size_t)ia * 2 * half_a), 16, 1024);
       const uint64_t dhi = umma_desc(smem_u32(sB_all + (size_t)jb * 4 * half_b), 16, 1024), dlo = dhi + ((uint32_t)half_b >> 4);
       const uint32_t d_t = tmem + (uint32_t)(i * p.cols);
       if (elect_one()) {
@@ -296,8 +299,9 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 #ifdef HVA_ASSIGN_TIMING
       ++tq;
 #endif
-      if (++i == NT) { i = 0; par ^= 1u; }
+      if (++i == NS) { i = 0; par ^= 1u; }
       if (++jb == NB) jb = 0;
+      if (++ia == NT) ia = 0;
     }
     CFLUSH(3);
   } else if (warp == kTableWarp) {
@@ -329,7 +333,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
         if (lane == 0) S->cmax = m;
       }
       mbar_arrive(&S->table_ready);
-      if (++i == NT) { i = 0; par ^= 1u; }
+      if (++i == NS) { i = 0; par ^= 1u; }
     }
   } else if (warp == kMma2Warp) {
     // ================================================================ MMA 2: z^T[dim, slot] = sum_token x[token, dim] P^T[slot, token]
@@ -338,7 +342,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
     const uint32_t idesc2 = umma_idesc_bf16(128, (uint32_t)npad, 1, 0);
     const uint32_t hb = (uint32_t)half_b >> 4;
     const int ksteps2 = p.rows_a >> 4;
-    int i = 0, jw = 0;
+    int i = 0, jw = 0, ia = 0;
     uint32_t par = 0;
     for (;;) {
       TileSlot* S = &SH->slot[i];
@@ -350,7 +354,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       CMARK(2);
       TRACE(10, tq);
       tc_fence_after();
-      const uint64_t dx = umma_desc(smem_u32(sA_all + (size_t)i * 2 * half_a), half_a, 1024);
+      const uint64_t dx = umma_desc(smem_u32(sA_all + (size_t)ia * 2 * half_a), half_a, 1024);
       const uint64_t dp = umma_desc(smem_u32(sP_all + (size_t)jw * 2 * half_b), 16, 1024);
       const uint32_t d_t = tmem + (uint32_t)(i * p.cols);
       if (elect_one()) {
@@ -368,8 +372,9 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 #ifdef HVA_ASSIGN_TIMING
       ++tq;
 #endif
-      if (++i == NT) { i = 0; par ^= 1u; }
+      if (++i == NS) { i = 0; par ^= 1u; }
       if (++jw == NW) jw = 0;
+      if (++ia == NT) ia = 0;
     }
     CFLUSH(4);
   } else if (warp >= kEpiWarp0) {
@@ -413,7 +418,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 #ifdef HVA_ASSIGN_TIMING
       ++tq;
 #endif
-      if (++i == NT) { i = 0; par ^= 1u; }
+      if (++i == NS) { i = 0; par ^= 1u; }
     }
     CFLUSH(1);
   } else {
@@ -428,7 +433,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
     const bool single_chunk = nwin <= 32;
     unsigned char* sP = sP_all + (size_t)w * 2 * half_b;
     uint32_t prev_p = 0;      // shared-space address of the one-hot element set for the group's previous tile (0: none)
-    int i = w, pi = 0;                       // token slot of the group's tile / of its previous tile (NW < NT)
+    int i = w, pi = 0, ia = w;               // slot of the group's tile / of its previous tile, token buffer (NW < NT <= NS)
     uint32_t par = 0, ppar = 0;
     for (bool first_tile = true;; first_tile = false) {
       TileSlot* S = &SH->slot[i];
@@ -442,7 +447,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       if (S->item < 0) break;
       struct { uint32_t cmax; } T{S->cmax};
       const float* s_c = s_c_all + i * npad; const uint16_t* s_u = s_u_all + i * npad; int* s_cnt = s_cnt_all + i * npad;
-      const unsigned char* sA = sA_all + (size_t)i * 2 * half_a;
+      const unsigned char* sA = sA_all + (size_t)ia * 2 * half_a;
       const uint32_t trow = tmem + lane_base + (uint32_t)(i * p.cols);
       const int uw = S->uw, uh = S->uh, ut = S->ut, bh = S->bh, chunk = S->chunk;
       const int dt0 = chunk * p.ct;                        // first time slice of this tile inside the cell
@@ -694,7 +699,9 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 #endif
       pi = i; ppar = par;
       i += NW;
-      if (i >= NT) { i -= NT; par ^= 1u; }
+      if (i >= NS) { i -= NS; par ^= 1u; }
+      ia += NW;
+      if (ia >= NT) ia -= NT;
     }
     CFLUSH(0);
     }
@@ -705,22 +712,23 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 }
 
 // shared memory of a configuration (NT token slots, NB centroid buffers, NW one-hot tiles)
-size_t assign_tc_smem(int npad, int rows_a, int NT, int NB, int NW) {
+size_t assign_tc_smem(int npad, int rows_a, int NT, int NB, int NW, int NS) {
   const size_t half_a = (size_t)rows_a * 128, half_b = (size_t)npad * 128;
   size_t bytes = (size_t)NT * 2 * half_a + (size_t)NB * 4 * half_b + (size_t)NW * 2 * half_b;
   // MMA 1 reads 128 token rows of its A operand: keep the over-read of the last slot inside the allocation
   bytes = std::max(bytes, (size_t)(NT - 1) * 2 * half_a + half_a + 16384);
-  bytes += (size_t)NT * npad * (sizeof(float) + sizeof(int) + sizeof(uint16_t)) + 8 + sizeof(AssignTcShared) + 16;
+  bytes += (size_t)NS * npad * (sizeof(float) + sizeof(int) + sizeof(uint16_t)) + 8 + sizeof(AssignTcShared) + 16;
   return bytes + 1024;
 }
 
 // the largest pipeline that fits 227 KB of shared memory and 512 TMEM columns: three scan groups if possible
-bool assign_tc_config(int npad, int rows_a, int cols, int* NT, int* NB, int* NW) {
+bool assign_tc_config(int npad, int rows_a, int cols, int* NT, int* NB, int* NW, int* NS) {
+  const int ns = std::min(kMaxNT, (int)kTmemCols / cols);      // pipeline slots: as many as TMEM holds
   for (int nw = kMaxNW; nw >= 1; --nw)
     for (int nb = 2; nb >= 1; --nb)
-      for (int nt = kMaxNT; nt >= nw + 1; --nt) {
-        if (nt * cols > (int)kTmemCols || nt <= nb) continue;
-        if (assign_tc_smem(npad, rows_a, nt, nb, nw) <= 227 * 1024) { *NT = nt; *NB = nb; *NW = nw; return true; }
+      for (int nt = ns; nt >= nw + 1; --nt) {
+        if (nt <= nb) continue;
+        if (assign_tc_smem(npad, rows_a, nt, nb, nw, ns) <= 227 * 1024) { *NT = nt; *NB = nb; *NW = nw; *NS = ns; return true; }
       }
   return false;
 }
@@ -732,8 +740,8 @@ bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype) {
         g.kw <= 256 && g.wt <= 256 && g.wh <= 256 && g.ww <= 256))
     return false;
   const int ctok = hva_assign_tc_slices(g) * g.kh * g.kw, npad = (g.nwin + 15) & ~15;
-  int NT, NB, NW;
-  return assign_tc_config(npad, (ctok + 15) & ~15, 2 * npad <= 256 ? 2 * npad : npad, &NT, &NB, &NW);
+  int NT, NB, NW, NS;
+  return assign_tc_config(npad, (ctok + 15) & ~15, 2 * npad <= 256 ? 2 * npad : npad, &NT, &NB, &NW, &NS);
 }
 
 namespace {
@@ -762,8 +770,8 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
   a->rows_a = (ctok + 15) & ~15;
   a->one_pass = 2 * a->npad <= 256;
   a->cols = a->one_pass ? 2 * a->npad : a->npad;
-  if (!assign_tc_config(a->npad, a->rows_a, a->cols, &a->NT, &a->NB, &a->NW)) return HVA_EUNSUPPORTED;
-  a->smem = assign_tc_smem(a->npad, a->rows_a, a->NT, a->NB, a->NW);
+  if (!assign_tc_config(a->npad, a->rows_a, a->cols, &a->NT, &a->NB, &a->NW, &a->NS)) return HVA_EUNSUPPORTED;
+  a->smem = assign_tc_smem(a->npad, a->rows_a, a->NT, a->NB, a->NW, a->NS);
   if ((long long)g.Kw * g.Kh * g.Kt * BH * a->csplit > 0x7fffffffLL) return HVA_EUNSUPPORTED;
   if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, a->ct, g.kh, g.kw)) return HVA_ECUDA;
   if (!make_map5(&a->map_hi, mu_hi, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
@@ -780,9 +788,9 @@ int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const f
   auto magic = [](int d) -> uint32_t { return d <= 1 ? 0u : (uint32_t)(((1ull << 32) + d - 1) / d); };
   auto magic64 = [](int d) -> unsigned long long { return d <= 1 ? 0ull : ~0ull / (unsigned long long)d + 1ull; };
   AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, xsq, xsq ? xsq_mode : 0, a.npad, a.rows_a, a.csplit, a.ct, magic(g.kh * g.kw),
-                   magic(g.kw), magic(g.wh * g.ww), magic(g.ww), a.NT, a.NB, a.NW, a.cols, a.one_pass, magic64(g.Kw * g.Kh), magic64(g.Kw),
-                   magic64(a.csplit), magic64(g.Kt), g.Kw * g.Kh * g.Kt * BH * a.csplit, counter, probe};
-  if (cudaMemsetAsync(counter, 0, sizeof(int), st) != cudaSuccess) return HVA_ECUDA;
+                   magic(g.kw), magic(g.wh * g.ww), magic(g.ww), a.NT, a.NB, a.NW, a.NS, a.cols, a.one_pass, magic64(g.Kw * g.Kh), magic64(g.Kw),
+                   magic64(a.csplit), magic64(g.Kt), g.Kw * g.Kh * g.Kt * BH * a.csplit, probe};
+  (void)counter;
   if (a.probe != (probe != nullptr)) return HVA_EINVAL;
   if (probe) hva_assign_tc_kernel<true><<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   else hva_assign_tc_kernel<false><<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);

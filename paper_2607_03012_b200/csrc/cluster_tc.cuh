@@ -6,7 +6,7 @@
 struct HvaAssignTc {
   CUtensorMap map_x, map_hi, map_lo;
   int npad, rows_a, csplit, ct;
-  int NT, NB, NW;      // token slots, centroid buffers, scan warpgroups of the persistent CTA
+  int NT, NB, NW, NS;  // token buffers, centroid buffers, scan warpgroups, pipeline slots of the persistent CTA
   int cols;            // TMEM columns per token slot
   size_t smem;
   int one_pass;        // one MMA pass over the stacked [hi; lo] centroid tile
