@@ -31,65 +31,91 @@ __host__ PlanPtrs plan_ptrs(void* plan, const hva_plan_layout& L) {
   return p;
 }
 
-// ---- group / cluster bookkeeping: one CTA per (b, head)
+// block-wide exclusive scan of one int per thread (1024 threads); *total receives the block sum
+__device__ __forceinline__ int block_excl_scan(int v, int* s_warp, int* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+  if (lane == 31) s_warp[warp] = x;
+  __syncthreads();
+  if (warp == 0) {
+    int w = s_warp[lane], t = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, t, o); if (lane >= o) t += y; }
+    s_warp[lane] = t - w;
+    if (lane == 31) *total = t;
+  }
+  __syncthreads();
+  const int r = s_warp[warp] + x - v;
+  __syncthreads();          // s_warp may be reused by the next call
+  return r;
+}
+
+// ---- group / cluster bookkeeping: one CTA per (b, head), 1024 threads; Nq, Nk <= 2048 (two items per thread).  Every list is
+// built by block-wide scans (round 1 ran the prefix sums, the group list and the work list on thread 0: 0.59 ms at C4).
 __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, int Nk, const int* __restrict__ sizes_q,
                                                                const int* __restrict__ sizes_k,
                                                                const int* __restrict__ group_of,
                                                                const uint8_t* __restrict__ group_mask, int tile_q,
                                                                int tile_k, PlanPtrs P, int* __restrict__ qbase) {
   const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int* sq = sizes_q + (size_t)bh * Nq;
-  const int* sk = sizes_k + (size_t)bh * Nk;
-  const int* gof = group_of + (size_t)bh * Nq;
   int* koff = P.koff + (size_t)bh * (Nk + 1);
   int* gid = P.gid + (size_t)bh * Nq;
   int* goff = P.goff + (size_t)bh * (Nq + 1);
   int* kappa = P.kappa + (size_t)bh * Nq;
   int* run_cnt = P.run_cnt + (size_t)bh * Nq;
   int* qb = qbase + (size_t)bh * Nq;
-  __shared__ int s_ng;
-  // the serial parts below are chains of dependent loads: run them on shared-memory copies (global latency made this kernel
-  // 0.67 ms at C4)
+  __shared__ int s_warp[32];
+  __shared__ int s_tot;
   extern __shared__ int s_stage[];
-  int* s_sq = s_stage;            // [Nq]
-  int* s_gof = s_sq + Nq;         // [Nq]
-  int* s_sk = s_gof + Nq;         // [Nk]
-  int* s_goff = s_sk + Nk;        // [Nq + 1]
-  int* s_kap = s_goff + Nq + 1;   // [Nq]
-  for (int u = tid; u < Nq; u += blockDim.x) { s_sq[u] = sizes_q[(size_t)bh * Nq + u]; s_gof[u] = group_of[(size_t)bh * Nq + u]; }
-  for (int j = tid; j < Nk; j += blockDim.x) s_sk[j] = sizes_k[(size_t)bh * Nk + j];
+  int* s_sq = s_stage;            // [Nq] s^q
+  int* s_gof = s_sq + Nq;         // [Nq] gid of each query cluster
+  int* s_sk = s_gof + Nq;         // [Nk] s^k
+  int* s_gsz = s_sk + Nk;         // [Nq] rows of the group led by g (0 if g leads nothing)
+  int* s_rank = s_gsz + Nq;       // [Nq] position of group g among the active groups (ascending gid)
+  int* s_goff = s_rank + Nq;      // [Nq + 1] Q' row offset of active group k
+  int* s_kap = s_goff + Nq + 1;   // [Nq] kappa of active group k
+  for (int u = tid; u < Nq; u += 1024) { s_sq[u] = sizes_q[(size_t)bh * Nq + u]; s_gof[u] = group_of[(size_t)bh * Nq + u]; s_gsz[u] = 0; }
+  for (int j = tid; j < Nk; j += 1024) s_sk[j] = sizes_k[(size_t)bh * Nk + j];
   __syncthreads();
-  sq = s_sq; sk = s_sk; gof = s_gof;
-  // Q' row offset of query cluster u: clusters ordered by (gid(u), u)   (R-P1)
-  for (int u = tid; u < Nq; u += blockDim.x) {
-    int gu = gof[u], off = 0;
-    for (int v = 0; v < Nq; ++v) {
-      int gv = gof[v];
-      if (gv < gu || (gv == gu && v < u)) off += sq[v];
-    }
-    qb[u] = off;
+  // rows of every group (integer atomics: order-free)
+  for (int u = tid; u < Nq; u += 1024) if (s_sq[u] > 0) atomicAdd(&s_gsz[s_gof[u]], s_sq[u]);
+  // K' row offsets: exclusive scan of s^k, two consecutive clusters per thread
+  {
+    const int j0 = 2 * tid, a = j0 < Nk ? s_sk[j0] : 0, b = j0 + 1 < Nk ? s_sk[j0 + 1] : 0;
+    const int e = block_excl_scan(a + b, s_warp, &s_tot);
+    if (j0 < Nk) koff[j0] = e;
+    if (j0 + 1 < Nk) koff[j0 + 1] = e + a;
+    if (tid == 0) koff[Nk] = s_tot;
   }
-  if (tid == 0) {  // K' row offsets; active groups in ascending gid
-    int a = 0;
-    for (int j = 0; j < Nk; ++j) { koff[j] = a; a += sk[j]; }
-    koff[Nk] = a;
-    int c = 0;
-    for (int g = 0; g < Nq; ++g) {
-      if (gof[g] != g) continue;
-      int s = 0;                      // a leader with an empty group (s^q = 0) is not active
-      if (sq[g] > 0) s = 1;
-      else for (int v = g + 1; v < Nq && !s; ++v) s = (gof[v] == g && sq[v] > 0);
-      if (s) gid[c++] = g;
-    }
-    s_ng = c; P.n_groups[bh] = c;
+  // active groups in ascending gid (a leader whose group has no rows is not active) and their Q' row offsets
+  int ng;
+  {
+    const int g0 = 2 * tid;
+    const int f0 = g0 < Nq && s_gof[g0] == g0 && s_gsz[g0] > 0, f1 = g0 + 1 < Nq && s_gof[g0 + 1] == g0 + 1 && s_gsz[g0 + 1] > 0;
+    const int e = block_excl_scan(f0 + f1, s_warp, &s_tot);
+    ng = s_tot;
+    if (f0) { gid[e] = g0; s_rank[g0] = e; }
+    if (f1) { gid[e + f0] = g0 + 1; s_rank[g0 + 1] = e + f0; }
+    const int z0 = f0 ? s_gsz[g0] : 0, z1 = f1 ? s_gsz[g0 + 1] : 0;
+    const int o = block_excl_scan(z0 + z1, s_warp, &s_tot);
+    if (f0) { goff[e] = o; s_goff[e] = o; }
+    if (f1) { goff[e + f0] = o + z0; s_goff[e + f0] = o + z0; }
+    if (tid == 0) { goff[ng] = n; s_goff[ng] = n; P.n_groups[bh] = ng; }
   }
   __syncthreads();
-  const int ng = s_ng;
-  for (int k = tid; k < ng; k += blockDim.x) { const int o = qb[gid[k]]; goff[k] = o; s_goff[k] = o; }   // leader = first cluster of its group
-  if (tid == 0) { goff[ng] = n; s_goff[ng] = n; }
+  // Q' row offset of query cluster u: clusters ordered by (gid(u), u)   (R-P1) = offset of its group + rows of the group's
+  // members below u
+  for (int u = tid; u < Nq; u += 1024) {
+    const int gu = s_gof[u];
+    int off = 0;
+    for (int v = gu; v < u; ++v) off += (s_gof[v] == gu) ? s_sq[v] : 0;      // members of a group are >= its gid
+    qb[u] = (s_sq[u] > 0 ? s_goff[s_rank[gu]] : 0) + off;
+  }
   // packed key runs of each group: maximal runs of consecutive selected key clusters (l.109)
   const uint8_t* gm = group_mask + (size_t)bh * Nq * Nk;
-  for (int k = warp; k < ng; k += blockDim.x / 32) {
+  for (int k = warp; k < ng; k += 32) {
     uint16_t* r16 = reinterpret_cast<uint16_t*>(P.runs + ((size_t)bh * Nq + k) * P.run_stride);
     const uint8_t* grow = gm + (size_t)k * Nk;
     int nstart = 0, nend = 0, kap = 0;
@@ -102,7 +128,7 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
         const int j = jb + 32 * w + lane;
         const int bit = (j < Nk) ? grow[j] : 0;
         const unsigned word = __ballot_sync(0xffffffffu, bit);
-        kap += bit ? sk[j] : 0;
+        kap += bit ? s_sk[j] : 0;
         if (w == lane) mine = word;
       }
       const unsigned prev_w = __shfl_up_sync(0xffffffffu, mine, 1), next_w = __shfl_down_sync(0xffffffffu, mine, 1);
@@ -128,29 +154,60 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
     if (lane == 0) { run_cnt[k] = nstart; kappa[k] = kap; s_kap[k] = kap; }
   }
   __syncthreads();
-  if (tid == 0) {  // work list (group, q-tile) in group order + statistics (Eq. 7-8; Fig. 5c terms)
+  // work list (group, q-tile) in group order + statistics (Eq. 7-8; Fig. 5c terms): two groups per thread
+  {
     int* work = P.work + (size_t)bh * P.work_cap;
-    hva_stats s = {};
-    int wc = 0;
-    for (int k = 0; k < ng; ++k) {
-      int rows = s_goff[k + 1] - s_goff[k], kp = s_kap[k];
-      int rt = (rows + tile_q - 1) / tile_q, kt = (kp + tile_k - 1) / tile_k;
-      for (int t = 0; t < rt; ++t) work[wc++] = k | (t << 16);
-      s.q_rows_valid += rows; s.q_rows_padded += (int64_t)rt * tile_q;
-      s.k_cols_valid += kp; s.k_cols_padded += (int64_t)kt * tile_k;
-      s.tiles_executed += (int64_t)rt * kt; s.pairs_valid += (int64_t)rows * kp;
+    const int k0 = 2 * tid;
+    int rt[2] = {0, 0};
+    long long st[6] = {0, 0, 0, 0, 0, 0};    // q_rows_valid, q_rows_padded, k_cols_valid, k_cols_padded, tiles_executed, pairs_valid
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const int k = k0 + e;
+      if (k < ng) {
+        const int rows = s_goff[k + 1] - s_goff[k], kp = s_kap[k];
+        rt[e] = (rows + tile_q - 1) / tile_q;
+        const int kt = (kp + tile_k - 1) / tile_k;
+        st[0] += rows; st[1] += (long long)rt[e] * tile_q; st[2] += kp; st[3] += (long long)kt * tile_k;
+        st[4] += (long long)rt[e] * kt; st[5] += (long long)rows * kp;
+      }
     }
-    s.n_groups = ng; s.q_tiles = wc;
-    P.work_cnt[bh] = wc;
-    P.stats[bh] = s;
+    const int wo = block_excl_scan(rt[0] + rt[1], s_warp, &s_tot);
+    const int wc = s_tot;
+    for (int t = 0; t < rt[0]; ++t) work[wo + t] = k0 | (t << 16);
+    for (int t = 0; t < rt[1]; ++t) work[wo + rt[0] + t] = (k0 + 1) | (t << 16);
+    // statistics: warp shuffles, then one 64-bit shared atomic per warp and field (integers: order-free)
+    __shared__ unsigned long long s_st[6];
+    if (tid < 6) s_st[tid] = 0ull;
+    __syncthreads();
+#pragma unroll
+    for (int f = 0; f < 6; ++f) {
+      long long v = st[f];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      if (lane == 0 && v) atomicAdd(&s_st[f], (unsigned long long)v);
+    }
+    __syncthreads();
+    if (tid == 0) {
+      hva_stats s = {};
+      s.n_groups = ng; s.q_tiles = wc;
+      s.q_rows_valid = (int64_t)s_st[0]; s.q_rows_padded = (int64_t)s_st[1]; s.k_cols_valid = (int64_t)s_st[2];
+      s.k_cols_padded = (int64_t)s_st[3]; s.tiles_executed = (int64_t)s_st[4]; s.pairs_valid = (int64_t)s_st[5];
+      P.work_cnt[bh] = wc;
+      P.stats[bh] = s;
+    }
   }
 }
 
 // ---- pass A: per-tile histogram
-__global__ void __launch_bounds__(kSortWarps * 32) hva_sort_hist_kernel(int n, int Nc, int ntile,
-                                                                        const int* __restrict__ assign,
-                                                                        int* __restrict__ hist) {
+// (blockIdx.z selects the tensor: 0 = keys, 1 = queries -- both sorts run in the same three launches)
+struct SortPass { int Nc; const int* assign; int* hist; const int* base; int base_stride; int* perm; int* inv; };
+struct SortArgs { SortPass p[2]; };
+
+__global__ void __launch_bounds__(kSortWarps * 32) hva_sort_hist_kernel(int n, int ntile, SortArgs A) {
   extern __shared__ int s_h[];  // [kSortWarps][Nc]
+  const int Nc = A.p[blockIdx.z].Nc;
+  const int* __restrict__ assign = A.p[blockIdx.z].assign;
+  int* __restrict__ hist = A.p[blockIdx.z].hist;
   const int bh = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int tile = blockIdx.x * kSortWarps + warp;
   int* h = s_h + warp * Nc;
@@ -172,8 +229,10 @@ __global__ void __launch_bounds__(kSortWarps * 32) hva_sort_hist_kernel(int n, i
 }
 
 // ---- pass B: per-label exclusive scan over tiles, seeded with the cluster's row offset
-__global__ void hva_sort_scan_kernel(int Nc, int ntile, const int* __restrict__ base, int base_stride,
-                                     int* __restrict__ hist) {
+__global__ void hva_sort_scan_kernel(int ntile, SortArgs A) {
+  const int Nc = A.p[blockIdx.z].Nc, base_stride = A.p[blockIdx.z].base_stride;
+  const int* __restrict__ base = A.p[blockIdx.z].base;
+  int* __restrict__ hist = A.p[blockIdx.z].hist;
   int c = blockIdx.x * blockDim.x + threadIdx.x, bh = blockIdx.y;
   if (c >= Nc) return;
   int run = base[(size_t)bh * base_stride + c];
@@ -182,11 +241,12 @@ __global__ void hva_sort_scan_kernel(int Nc, int ntile, const int* __restrict__ 
 }
 
 // ---- pass C: stable scatter
-__global__ void __launch_bounds__(kSortWarps * 32) hva_sort_scatter_kernel(int n, int Nc, int ntile,
-                                                                           const int* __restrict__ assign,
-                                                                           const int* __restrict__ hist,
-                                                                           int* __restrict__ perm,
-                                                                           int* __restrict__ inv) {
+__global__ void __launch_bounds__(kSortWarps * 32) hva_sort_scatter_kernel(int n, int ntile, SortArgs A) {
+  const int Nc = A.p[blockIdx.z].Nc;
+  const int* __restrict__ assign = A.p[blockIdx.z].assign;
+  const int* __restrict__ hist = A.p[blockIdx.z].hist;
+  int* __restrict__ perm = A.p[blockIdx.z].perm;
+  int* __restrict__ inv = A.p[blockIdx.z].inv;
   extern __shared__ int s_h[];
   const int bh = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int tile = blockIdx.x * kSortWarps + warp;
@@ -266,7 +326,7 @@ extern "C" int hva_plan_describe(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, 
 
 size_t hva_plan_ws_bytes(int BH, int n, int Nq, int Nk) {
   int ntile = (n + kTile - 1) / kTile, Nc = Nq > Nk ? Nq : Nk;
-  return hva_align((size_t)BH * ntile * Nc * 4) + hva_align((size_t)BH * Nq * 4);
+  return 2 * hva_align((size_t)BH * ntile * Nc * 4) + hva_align((size_t)BH * Nq * 4);
 }
 
 extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, const int32_t* assign_q,
@@ -285,27 +345,27 @@ extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, con
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   PlanPtrs P = plan_ptrs(plan, L);
   const int ntile = (n + kTile - 1) / kTile, Ncmax = Nq > Nk ? Nq : Nk;
-  int* hist = reinterpret_cast<int*>(ws);
-  int* qbase = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + hva_align((size_t)BH * ntile * Ncmax * 4));
-  const size_t gsmem = sizeof(int) * (4 * (size_t)Nq + Nk + 1);
+  int* hist_k = reinterpret_cast<int*>(ws);
+  int* hist_q = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + hva_align((size_t)BH * ntile * Ncmax * 4));
+  int* qbase = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + 2 * hva_align((size_t)BH * ntile * Ncmax * 4));
+  const size_t gsmem = sizeof(int) * (6 * (size_t)Nq + Nk + 1);
   if (gsmem > 48 * 1024 && cudaFuncSetAttribute(hva_plan_groups_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem) != cudaSuccess)
     return HVA_EUNSUPPORTED;
   hva_plan_groups_kernel<<<BH, 1024, gsmem, st>>>(n, Nq, Nk, sizes_q, sizes_k, group_of_cluster, group_mask, tile_q, tile_k,
                                               P, qbase);
   HVA_CHECK_LAUNCH();
-  dim3 gsort((ntile + kSortWarps - 1) / kSortWarps, BH);
-  for (int pass = 0; pass < 2; ++pass) {  // 0: keys (perm_k), 1: queries (perm_q, inv_perm_q)
-    const int Nc = pass ? Nq : Nk;
-    const int* assign = pass ? assign_q : assign_k;
-    size_t smem = (size_t)kSortWarps * Nc * sizeof(int);
-    hva_sort_hist_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, Nc, ntile, assign, hist);
-    HVA_CHECK_LAUNCH();
-    hva_sort_scan_kernel<<<dim3((Nc + 127) / 128, BH), 128, 0, st>>>(Nc, ntile, pass ? qbase : P.koff, pass ? Nq : Nk + 1, hist);
-    HVA_CHECK_LAUNCH();
-    hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, Nc, ntile, assign, hist, pass ? P.perm_q : P.perm_k,
-                                                                 pass ? P.inv_perm_q : nullptr);
-    HVA_CHECK_LAUNCH();
-  }
+  // keys (perm_k) and queries (perm_q, inv_perm_q) in the same three launches
+  SortArgs A;
+  A.p[0] = SortPass{Nk, assign_k, hist_k, P.koff, Nk + 1, P.perm_k, nullptr};
+  A.p[1] = SortPass{Nq, assign_q, hist_q, qbase, Nq, P.perm_q, P.inv_perm_q};
+  dim3 gsort((ntile + kSortWarps - 1) / kSortWarps, BH, 2);
+  const size_t smem = (size_t)kSortWarps * Ncmax * sizeof(int);
+  hva_sort_hist_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scan_kernel<<<dim3((Ncmax + 127) / 128, BH, 2), 128, 0, st>>>(ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
   return HVA_OK;
 }
 
