@@ -12,6 +12,7 @@ namespace {
 
 constexpr int kTile = 1024;       // tokens per warp tile
 constexpr int kSortWarps = 4;     // warps per CTA in passes A and C
+constexpr int kGroupSplit = 6;    // CTAs per (b, head) sharing the key-run extraction (24 heads x 6 = 144 CTAs at C4)
 
 struct PlanPtrs {
   int *perm_q, *inv_perm_q, *perm_k, *koff, *n_groups, *gid, *goff, *kappa, *run_cnt, *work_cnt, *work;
@@ -59,7 +60,10 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
                                                                const int* __restrict__ group_of,
                                                                const uint8_t* __restrict__ group_mask, int tile_q,
                                                                int tile_k, PlanPtrs P, int* __restrict__ qbase) {
+  // blockIdx.y: the key-run extraction (the long part: one pass over the group's mask row per group) is split over the
+  // gridDim.y CTAs of a head; the scans are cheap and every CTA does them, CTA 0 of the head writes their results
   const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool lead = blockIdx.y == 0;
   int* koff = P.koff + (size_t)bh * (Nk + 1);
   int* gid = P.gid + (size_t)bh * Nq;
   int* goff = P.goff + (size_t)bh * (Nq + 1);
@@ -75,7 +79,6 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
   int* s_gsz = s_sk + Nk;         // [Nq] rows of the group led by g (0 if g leads nothing)
   int* s_rank = s_gsz + Nq;       // [Nq] position of group g among the active groups (ascending gid)
   int* s_goff = s_rank + Nq;      // [Nq + 1] Q' row offset of active group k
-  int* s_kap = s_goff + Nq + 1;   // [Nq] kappa of active group k
   for (int u = tid; u < Nq; u += 1024) { s_sq[u] = sizes_q[(size_t)bh * Nq + u]; s_gof[u] = group_of[(size_t)bh * Nq + u]; s_gsz[u] = 0; }
   for (int j = tid; j < Nk; j += 1024) s_sk[j] = sizes_k[(size_t)bh * Nk + j];
   __syncthreads();
@@ -85,9 +88,9 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
   {
     const int j0 = 2 * tid, a = j0 < Nk ? s_sk[j0] : 0, b = j0 + 1 < Nk ? s_sk[j0 + 1] : 0;
     const int e = block_excl_scan(a + b, s_warp, &s_tot);
-    if (j0 < Nk) koff[j0] = e;
-    if (j0 + 1 < Nk) koff[j0 + 1] = e + a;
-    if (tid == 0) koff[Nk] = s_tot;
+    if (lead && j0 < Nk) koff[j0] = e;
+    if (lead && j0 + 1 < Nk) koff[j0 + 1] = e + a;
+    if (lead && tid == 0) koff[Nk] = s_tot;
   }
   // active groups in ascending gid (a leader whose group has no rows is not active) and their Q' row offsets
   int ng;
@@ -96,18 +99,18 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
     const int f0 = g0 < Nq && s_gof[g0] == g0 && s_gsz[g0] > 0, f1 = g0 + 1 < Nq && s_gof[g0 + 1] == g0 + 1 && s_gsz[g0 + 1] > 0;
     const int e = block_excl_scan(f0 + f1, s_warp, &s_tot);
     ng = s_tot;
-    if (f0) { gid[e] = g0; s_rank[g0] = e; }
-    if (f1) { gid[e + f0] = g0 + 1; s_rank[g0 + 1] = e + f0; }
+    if (f0) { if (lead) gid[e] = g0; s_rank[g0] = e; }
+    if (f1) { if (lead) gid[e + f0] = g0 + 1; s_rank[g0 + 1] = e + f0; }
     const int z0 = f0 ? s_gsz[g0] : 0, z1 = f1 ? s_gsz[g0 + 1] : 0;
     const int o = block_excl_scan(z0 + z1, s_warp, &s_tot);
-    if (f0) { goff[e] = o; s_goff[e] = o; }
-    if (f1) { goff[e + f0] = o + z0; s_goff[e + f0] = o + z0; }
-    if (tid == 0) { goff[ng] = n; s_goff[ng] = n; P.n_groups[bh] = ng; }
+    if (f0) { if (lead) goff[e] = o; s_goff[e] = o; }
+    if (f1) { if (lead) goff[e + f0] = o + z0; s_goff[e + f0] = o + z0; }
+    if (tid == 0) { s_goff[ng] = n; if (lead) { goff[ng] = n; P.n_groups[bh] = ng; } }
   }
   __syncthreads();
   // Q' row offset of query cluster u: clusters ordered by (gid(u), u)   (R-P1) = offset of its group + rows of the group's
   // members below u
-  for (int u = tid; u < Nq; u += 1024) {
+  for (int u = tid; lead && u < Nq; u += 1024) {
     const int gu = s_gof[u];
     int off = 0;
     for (int v = gu; v < u; ++v) off += (s_gof[v] == gu) ? s_sq[v] : 0;      // members of a group are >= its gid
@@ -115,7 +118,7 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
   }
   // packed key runs of each group: maximal runs of consecutive selected key clusters (l.109)
   const uint8_t* gm = group_mask + (size_t)bh * Nq * Nk;
-  for (int k = warp; k < ng; k += 32) {
+  for (int k = warp + 32 * blockIdx.y; k < ng; k += 32 * gridDim.y) {
     uint16_t* r16 = reinterpret_cast<uint16_t*>(P.runs + ((size_t)bh * Nq + k) * P.run_stride);
     const uint8_t* grow = gm + (size_t)k * Nk;
     int nstart = 0, nend = 0, kap = 0;
@@ -151,10 +154,18 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
       carry = __shfl_sync(0xffffffffu, mine, 31) >> 31;
     }
     for (int o = 16; o > 0; o >>= 1) kap += __shfl_xor_sync(0xffffffffu, kap, o);
-    if (lane == 0) { run_cnt[k] = nstart; kappa[k] = kap; s_kap[k] = kap; }
+    if (lane == 0) { run_cnt[k] = nstart; kappa[k] = kap; }
   }
-  __syncthreads();
-  // work list (group, q-tile) in group order + statistics (Eq. 7-8; Fig. 5c terms): two groups per thread
+}
+
+// ---- work list (group, q-tile) in group order + statistics (Eq. 7-8; Fig. 5c terms): one CTA per (b, head), two groups per thread
+__global__ void __launch_bounds__(1024) hva_plan_work_kernel(int Nq, int tile_q, int tile_k, PlanPtrs P) {
+  const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+  __shared__ int s_warp[32];
+  __shared__ int s_tot;
+  const int ng = P.n_groups[bh];
+  const int* s_goff = P.goff + (size_t)bh * (Nq + 1);
+  const int* s_kap = P.kappa + (size_t)bh * Nq;
   {
     int* work = P.work + (size_t)bh * P.work_cap;
     const int k0 = 2 * tid;
@@ -229,15 +240,24 @@ __global__ void __launch_bounds__(kSortWarps * 32) hva_sort_hist_kernel(int n, i
 }
 
 // ---- pass B: per-label exclusive scan over tiles, seeded with the cluster's row offset
-__global__ void hva_sort_scan_kernel(int ntile, SortArgs A) {
+__global__ void __launch_bounds__(128) hva_sort_scan_kernel(int ntile, SortArgs A) {
+  // one warp per label: the lanes take 32 tiles at a time (independent loads), warp scan, running offset carried along
   const int Nc = A.p[blockIdx.z].Nc, base_stride = A.p[blockIdx.z].base_stride;
   const int* __restrict__ base = A.p[blockIdx.z].base;
   int* __restrict__ hist = A.p[blockIdx.z].hist;
-  int c = blockIdx.x * blockDim.x + threadIdx.x, bh = blockIdx.y;
+  const int lane = threadIdx.x & 31, c = blockIdx.x * 4 + (threadIdx.x >> 5), bh = blockIdx.y;
   if (c >= Nc) return;
   int run = base[(size_t)bh * base_stride + c];
   int* h = hist + (size_t)bh * ntile * Nc + c;
-  for (int t = 0; t < ntile; ++t) { int v = h[(size_t)t * Nc]; h[(size_t)t * Nc] = run; run += v; }
+  for (int t0 = 0; t0 < ntile; t0 += 32) {
+    const int t = t0 + lane;
+    const int v = t < ntile ? h[(size_t)t * Nc] : 0;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (t < ntile) h[(size_t)t * Nc] = run + x - v;
+    run += __shfl_sync(0xffffffffu, x, 31);
+  }
 }
 
 // ---- pass C: stable scatter
@@ -348,11 +368,13 @@ extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, con
   int* hist_k = reinterpret_cast<int*>(ws);
   int* hist_q = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + hva_align((size_t)BH * ntile * Ncmax * 4));
   int* qbase = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + 2 * hva_align((size_t)BH * ntile * Ncmax * 4));
-  const size_t gsmem = sizeof(int) * (6 * (size_t)Nq + Nk + 1);
+  const size_t gsmem = sizeof(int) * (5 * (size_t)Nq + Nk + 1);
   if (gsmem > 48 * 1024 && cudaFuncSetAttribute(hva_plan_groups_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem) != cudaSuccess)
     return HVA_EUNSUPPORTED;
-  hva_plan_groups_kernel<<<BH, 1024, gsmem, st>>>(n, Nq, Nk, sizes_q, sizes_k, group_of_cluster, group_mask, tile_q, tile_k,
-                                              P, qbase);
+  hva_plan_groups_kernel<<<dim3(BH, kGroupSplit), 1024, gsmem, st>>>(n, Nq, Nk, sizes_q, sizes_k, group_of_cluster, group_mask, tile_q,
+                                                                 tile_k, P, qbase);
+  HVA_CHECK_LAUNCH();
+  hva_plan_work_kernel<<<BH, 1024, 0, st>>>(Nq, tile_q, tile_k, P);
   HVA_CHECK_LAUNCH();
   // keys (perm_k) and queries (perm_q, inv_perm_q) in the same three launches
   SortArgs A;
@@ -362,7 +384,7 @@ extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, con
   const size_t smem = (size_t)kSortWarps * Ncmax * sizeof(int);
   hva_sort_hist_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
   HVA_CHECK_LAUNCH();
-  hva_sort_scan_kernel<<<dim3((Ncmax + 127) / 128, BH, 2), 128, 0, st>>>(ntile, A);
+  hva_sort_scan_kernel<<<dim3((Ncmax + 3) / 4, BH, 2), 128, 0, st>>>(ntile, A);
   HVA_CHECK_LAUNCH();
   hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
   HVA_CHECK_LAUNCH();
