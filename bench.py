@@ -24,9 +24,32 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 from paper_2607_03012_b200 import inputs, sharding  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one hva_attn_tc_kernel launch at C4 (top-p 0.9, merging on), from the `ncu --set full`
-# capture summarised in profiles/r1f_ncu_full.md (11.72 GB + 0.78 GB); algorithmic minimum 2.9 GB (Q', K', V' once + O)
-ATTN_DRAM_BYTES_C4 = 12.49e9
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of one hva_attn_tc_kernel launch at C4 (top-p 0.9, merging on), read
+# from the committed `ncu --set full` export named here (profiles/*.md beside it gives the command); algorithmic minimum 2.9 GB
+NCU_FULL_CSV = os.path.join("profiles", "r2_ncu_full_raw.csv")
+
+
+def attn_dram_bytes():
+    """(bytes per launch, source file) from the committed ncu raw export, or (None, None)."""
+    path = os.path.join(ROOT, NCU_FULL_CSV)
+    if not os.path.exists(path):
+        return None, None
+    import csv
+    rows = list(csv.reader(open(path)))
+    hdr = next((r for r in rows if "Kernel Name" in r), None)
+    if hdr is None:
+        return None, None
+    try:
+        kn, rd, wr = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    except ValueError:
+        return None, None
+    units = rows[rows.index(hdr) + 1]
+    mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    for r in rows[rows.index(hdr) + 2:]:
+        if len(r) > max(rd, wr) and "hva_attn_tc_kernel" in r[kn]:
+            f = lambda i: float(r[i].replace(",", "")) * mult.get(units[i], 1.0)
+            return f(rd) + f(wr), NCU_FULL_CSV
+    return None, None
 
 METRIC = "sparse-attn ms/call + clustering ms/step at 118,800-token HunyuanVideo shape"
 
@@ -87,9 +110,11 @@ def ev_time(fn, reps):
     return a.elapsed_time(b) / reps
 
 
-def oracle_sample(wl, head=0, attn_rows=32, merge_rounds=None):
-    """The CPU oracle, as it stands, on a bounded sample of the workload: one head's clustering (Q and K), mask,
-    merge, plan, and `attn_rows` attention rows.  Returns (seconds by stage, extrapolated ms per full call)."""
+def oracle_sample(wl, head=0, attn_rows=256):
+    """The CPU oracle, as it stands, on a bounded sample of the workload: ONE head in full through clustering (Q and K), mask,
+    merge (all R rounds), plan, and `attn_rows` attention rows chosen to cover merged groups, groups of several q-tiles and ragged
+    last tiles.  Returns (seconds by stage, ms per full call: the per-head stages x heads, the attention rows
+    x n / attn_rows x heads -- both extrapolations are labelled by the caller)."""
     import oracle
     x = inputs.make_head(wl, head)
     Q, K, V = [inputs.to_f64(t) for t in x]
@@ -100,16 +125,35 @@ def oracle_sample(wl, head=0, attn_rows=32, merge_rounds=None):
     scale = float(np.float32(1 / math.sqrt(wl.D)))
     t0 = time.perf_counter(); M = oracle.build_mask(cq["mu"], ck["mu"], ck["sizes"], scale, float(np.float32(wl.top_p)))
     t["mask"] = time.perf_counter() - t0
-    R = wl.merge_rounds if merge_rounds is None else merge_rounds
-    t0 = time.perf_counter(); gof, gids, chi = oracle.merge_clusters(cq["sizes"], ck["sizes"], M, wl.tile[0], wl.tile[1], R, seed=wl.seed, bh=head)
+    t0 = time.perf_counter(); gof, gids, chi = oracle.merge_clusters(cq["sizes"], ck["sizes"], M, wl.tile[0], wl.tile[1], wl.merge_rounds, seed=wl.seed, bh=head)
     t["merge"] = time.perf_counter() - t0
-    t0 = time.perf_counter(); oracle.build_plan(cq["assign"], ck["assign"], gof, len(cq["sizes"]), len(ck["sizes"]))
+    t0 = time.perf_counter(); po = oracle.build_plan(cq["assign"], ck["assign"], gof, len(cq["sizes"]), len(ck["sizes"]))
     t["plan"] = time.perf_counter() - t0
-    rows = np.sort(np.random.default_rng(0).choice(wl.n, attn_rows, replace=False))
+    # rows: a third from groups of more than one q-tile (first and last row of the group included), a third from merged groups,
+    # the rest uniform
+    rng = np.random.default_rng(0)
+    rows_g = np.diff(po["goff"])
+    members = np.bincount(np.searchsorted(np.asarray(gids), gof[cq["sizes"] > 0]), minlength=len(gids))
+    pick = []
+    for sel in (np.nonzero(rows_g > wl.tile[0])[0], np.nonzero(members > 1)[0]):
+        for k in sel[: max(1, attn_rows // 12)]:
+            seg = po["perm_q"][po["goff"][k]:po["goff"][k + 1]]
+            pick += [seg[0], seg[-1]] + list(rng.choice(seg, min(2, len(seg)), replace=False))
+    pick = np.unique(np.array(pick, dtype=np.int64))[: 2 * attn_rows // 3]
+    rest = rng.choice(wl.n, attn_rows, replace=False)
+    rows = np.unique(np.concatenate([pick, rest]))[:attn_rows]
     t0 = time.perf_counter(); oracle.masked_attention_rows(Q, K, V, rows, cq["assign"], ck["assign"], gof, gids, chi, scale)
     t["attn_rows"] = time.perf_counter() - t0
-    per_head = t["cluster"] + t["mask"] + t["merge"] + t["plan"] + t["attn_rows"] * (wl.n / attn_rows)
+    t["n_rows"] = len(rows)
+    per_head = t["cluster"] + t["mask"] + t["merge"] + t["plan"] + t["attn_rows"] * (wl.n / len(rows))
     return t, per_head * wl.heads * 1e3
+
+
+def oracle_sample_text(wl, t):
+    return ("one head of %s in full through the oracle: clustering Q,K %.1f s, mask %.2f s, merge (%d rounds) %.1f s, plan %.2f s "
+            "[measured; x %d heads extrapolated]; attention %d rows (merged, multi-tile and ragged groups included) %.2f s "
+            "[measured; x n/%d rows x %d heads extrapolated]" % (wl.name, t["cluster"], t["mask"], wl.merge_rounds, t["merge"], t["plan"],
+                                                                 wl.heads, t["n_rows"], t["attn_rows"], t["n_rows"], wl.heads))
 
 
 def oracle_threads():
@@ -138,13 +182,12 @@ def run_reference(args, wl):
         return
     vals = []
     for i in range(args.warmup + args.steps):
-        t, ms = oracle_sample(wl, head=i % wl.heads, attn_rows=16, merge_rounds=1 if wl.n > 50000 else None)
+        t, ms = oracle_sample(wl, head=i % wl.heads, attn_rows=64 if wl.n > 50000 else 256)
         if i >= args.warmup:
             vals.append(ms)
     v = float(np.mean(vals))
     cores = oracle_threads()
-    sample = ("per step: one head of %s through oracle clustering (Q,K), mask, 1 merge round, plan and 16 attention rows; "
-              "extrapolated x heads and x n/16 rows" % wl.name)
+    sample = "per step: " + oracle_sample_text(wl, t)
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f64", "data": "synthetic",
@@ -167,10 +210,16 @@ def main():
                          "with CTA tile occupancy, 'hybrid' = the 50-step anchor / subset sequence (use --config C5), 'selfbase' = "
                          "on-box self-baselines: the dense (HVA_DENSE) call next to the sparse one, clustering over window sizes")
     ap.add_argument("--seq-steps", type=int, default=50)
+    ap.add_argument("--hybrid-heads", type=int, default=24, help="--report hybrid: heads of the call to run (the sequence stays on the device)")
+    ap.add_argument("--verbose", action="store_true", help="--report hybrid: one JSON line per step besides the summaries")
     ap.add_argument("--cell-q", default=None, help="k_t,k_h,k_w of the Q grid (default: the workload's); e.g. the paper's 11,5,5")
     ap.add_argument("--cell-k", default=None, help="k_t,k_h,k_w of the K grid; e.g. the paper's 11,3,3")
     ap.add_argument("--win", default=None, help="w_t,w_h,w_w of both windows; e.g. the paper's 3,8,8")
     ap.add_argument("--min-kc", type=float, default=0.0)
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: 'weak' = every rank runs one full-size call (value = max ms / N); 'strong' = ONE call whose heads are "
+                         "sharded round-robin over the ranks (sharding.shard_heads; no collective), value = max ms over ranks")
+    ap.add_argument("--no-paper-setting", action="store_true", help="skip the secondary measurement at the paper's own hyper-parameters")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stages", action="store_true")
     args = ap.parse_args()
@@ -190,6 +239,7 @@ def main():
         return report_selfbase(b, wl, args)
     if args.report == "assign-phases":
         return report_assign_phases(b, wl, args)
+    import dataclasses
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -200,9 +250,14 @@ def main():
     pk = peaks()
 
     # ---- inputs: generated on the host, resident in HBM before the timed region
-    import dataclasses
-    wl_r = dataclasses.replace(wl, seed=wl.seed + 1000 * rank) if rank else wl
-    hQ, hK, hV = [t.contiguous().pin_memory() for t in inputs.make_qkv(wl_r)]
+    strong = args.scaling == "strong" and world > 1
+    if strong:      # one call, heads sharded over the ranks: every rank generates and runs only its own heads of the SAME call
+        my_heads = sharding.shard_heads(wl.heads, rank, world)
+        hQ, hK, hV = [t.contiguous().pin_memory() for t in inputs.make_qkv(wl, my_heads)]
+        wl_full, wl = wl, dataclasses.replace(wl, heads=len(my_heads))
+    else:
+        wl_r = dataclasses.replace(wl, seed=wl.seed + 1000 * rank) if rank else wl
+        hQ, hK, hV = [t.contiguous().pin_memory() for t in inputs.make_qkv(wl_r)]
     Q, K, V = hQ.cuda(), hK.cuda(), hV.cuda()
     shape = b.make_shape(wl)
     cfg = b.make_config(wl, top_p=args.top_p, merge_rounds=args.merge_rounds, min_kc=args.min_kc)
@@ -241,28 +296,49 @@ def main():
     nbytes = Q.numel() * Q.element_size()
     del dev4
 
-    out = {"metric": METRIC, "value": sharding.whole_job_value(ms, world), "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-           "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+    out = {"metric": METRIC, "value": ms if strong else sharding.whole_job_value(ms, world), "unit": "ms", "n_gpus": world, "steps": args.steps,
+           "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "strong" if strong else "weak", "vs_baseline": None,
            "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
-           "config": workload_config(wl, list(cfg.cell_q), list(cfg.cell_k), list(cfg.win_q), float(cfg.min_kc), float(cfg.top_p),
-                                     int(cfg.merge_rounds), custom),
+           "config": workload_config(wl_full if strong else wl, list(cfg.cell_q), list(cfg.cell_k), list(cfg.win_q), float(cfg.min_kc),
+                                     float(cfg.top_p), int(cfg.merge_rounds), custom),
            "clocks": clocks,
-           "e2e": {"value": e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
-           "gpu_launches": args.steps * (2 * (2 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 7 + 3 + 1)}
+           "e2e": {"value": e2e_ms if strong else e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
+           # kernels of one hva_forward: per tensor init + split + iters x (assign, finalize); mask; merge init (+ nterms) + R x (overlap,
+           # propose, apply) + rank + out; plan groups + work + hist + scan + scatter; 3 permutes; attention
+           "gpu_launches": args.steps * (2 * (2 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 5 + 3 + 1)}
 
     # ---- per-stage times and rooflines (rank 0)
     if rank == 0 and not args.no_stages:
         out.update(stage_report(b, wl, shape, cfg, Q, K, V, stats, pk))
+    if rank == 0 and world == 1 and not custom and not args.no_paper_setting and wl.name == "C4-hunyuan":
+        out["paper_setting"] = paper_setting(b, wl, shape, Q, K, V, O)
     if rank == 0 and not args.no_cpu_baseline and not custom:
-        t, cpu_ms = oracle_sample(wl, attn_rows=32, merge_rounds=1 if wl.n > 50000 else None)
-        out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": oracle_threads(), "kind": "oracle",
-                               "sample": "one head of %s: oracle clustering Q,K %.1fs, mask %.2fs, merge(1 round) %.1fs, plan %.2fs, "
-                                         "32 attention rows %.2fs; extrapolated x%d heads, x n/32 rows" % (
-                                             wl.name, t["cluster"], t["mask"], t["merge"], t["plan"], t["attn_rows"], wl.heads)}
+        t, cpu_ms = oracle_sample(wl, attn_rows=256)
+        out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": oracle_threads(), "kind": "oracle", "sample": oracle_sample_text(wl, t)}
     if rank == 0:
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def paper_setting(b, wl, shape, Q, K, V, O):
+    """Secondary number: the same call at the paper's own HunyuanVideo hyper-parameters (Table 2 l.338 / SURVEY App. A; 10 iterations
+    l.215) instead of BASELINE.json configs[3]'s: Q grid (11,5,5) -> 432 clusters, K grid (11,3,3) -> 1215, (3,8,8) windows = 192
+    candidates per token, top-p 0.9, min-kc 0.15, R = 3.  The JSON line's `value` stays on the config BASELINE.json names."""
+    cfg = b.make_config(wl, min_kc=0.15)
+    i3 = type(cfg.cell_q)
+    cfg.cell_q, cfg.cell_k, cfg.win_q, cfg.win_k, cfg.iters = i3(11, 5, 5), i3(11, 3, 3), i3(3, 8, 8), i3(3, 8, 8), 10
+    fwd = b.Forward(shape, cfg)
+    for _ in range(2):
+        fwd(Q, K, V, O)
+    ms = ev_time(lambda: fwd(Q, K, V, O), 3)
+    cl = ev_time(lambda: (b.hva_cluster(shape, list(cfg.cell_q), list(cfg.win_q), 10, Q, want_lowe=False, want_sums=False),
+                          b.hva_cluster(shape, list(cfg.cell_k), list(cfg.win_k), 10, K, want_lowe=False, want_sums=False)), 2)
+    occ = occupancy(wl, fwd.stats_dicts())
+    return {"config": {"cell_q": [11, 5, 5], "cell_k": [11, 3, 3], "win": [3, 8, 8], "iters": 10, "top_p": float(cfg.top_p), "min_kc": 0.15,
+                       "merge_rounds": int(cfg.merge_rounds), "N_q": 432, "N_k": 1215},
+            "ms_per_call": ms, "clustering_qk_ms": cl, "groups": occ["groups"], "theoretical_density": occ["theoretical_density"],
+            "cta_density": occ["cta_density"]}
 
 
 def occupancy(wl, stats):
@@ -372,72 +448,85 @@ def report_assign_phases(b, wl, args):
 
 
 def report_hybrid(b, wl, args):
-    """BASELINE.json configs[4]: X_s = 0.98 X_{s-1} + 0.2 fresh_s for Q, K, V; full clustering at anchor steps (every 10th), subset
-    update (l.101-103) in between.  Per step: ms of the whole call and of its clustering part, label agreement with a cold-start
-    full re-clustering of X_s (ours, and the frozen anchor labels for comparison), relative k-means objective."""
-    import math as _m
-    heads = list(range(wl.heads))
-    shape = b.make_shape(wl)
-    cfg = b.make_config(wl, subset_frac=0.15)
-    fwd = b.Forward(shape, cfg, with_state=True)
+    """BASELINE.json configs[4]: X_s = 0.98 X_{s-1} + 0.2 fresh_s for Q, K, V; full clustering at anchor steps, subset update (l.101-103)
+    in between.  The input sequence is generated once (first `--hybrid-heads` heads, `--seq-steps` steps, resident on the device) and
+    replayed for every variant: reading R-H3 / R-H3' (hybrid_refresh_all), anchors every 10 steps (BASELINE.json) / every 2 (the paper,
+    l.322), subset fraction 0.05 / 0.15 / 0.30.  Per step: ms of the whole call and of its clustering part; label agreement with a
+    cold-start full re-clustering of X_s (ours, and the frozen anchor labels for comparison); k-means objective of (labels, centroids)
+    relative to the full re-clustering's, for the hybrid state and for the frozen anchor state."""
+    from concurrent.futures import ThreadPoolExecutor
+    heads = list(range(min(args.hybrid_heads, wl.heads)))
+    nh = len(heads)
+    shape = b.make_shape(wl, heads=nh)
     cur = [inputs.make_head(wl, h, 0) for h in heads]                      # per head [3, n, D]
     rms0 = [c.float().pow(2).mean(dim=(1, 2)).sqrt() for c in cur]
-    from concurrent.futures import ThreadPoolExecutor
-    O = None
-    frozen = None
-    rows = []
+    seq = []
     for s in range(args.seq_steps):
         if s > 0:
             with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 8)) as ex:
-                cur = list(ex.map(lambda h: inputs.hybrid_next(wl, cur[h], h, s, rms0[h]), heads))
+                cur = list(ex.map(lambda h: inputs.hybrid_next(wl, cur[h], heads[h], s, rms0[h]), range(nh)))
         X = torch.stack(cur, dim=1).unsqueeze(1).cuda()                    # [3, 1, heads, n, D]
-        Q, K, V = X[0].contiguous(), X[1].contiguous(), X[2].contiguous()
-        O = torch.empty_like(Q) if O is None else O
-        kind = b.HVA_ANCHOR if s % 10 == 0 else b.HVA_INTERMEDIATE
-        a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize(); a.record()
-        fwd(Q, K, V, O, step_kind=kind)
-        e.record(); torch.cuda.synchronize()
-        ms = a.elapsed_time(e)
-        st = {k: v.clone() for k, v in fwd.state_views().items()}
-        # clustering part of the step, timed on copies of the cache
-        if kind == b.HVA_ANCHOR:
-            def clus():
-                for X_, t in ((Q, "q"), (K, "k")):
-                    r = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X_, want_lowe=True)
-                    b.hva_select_subset(r["lowe"], st["subset_" + t].shape[1])
-            frozen = {t: st["assign_" + t].clone() for t in "qk"}
-        else:
-            prev = prev_state
-            def clus():
-                for X_, t in ((Q, "q"), (K, "k")):
-                    c2 = {k: prev[k + "_" + t].clone() for k in ("assign", "mu", "sums", "sizes")}
-                    b.hva_cluster_update(shape, X_, prev["subset_" + t], c2["assign"], c2["mu"], c2["sums"], c2["sizes"])
-        clus()
-        ms_cl = ev_time(clus, 1)
-        prev_state = st
-        agree, agree_frozen, obj = {}, {}, {}
-        for X_, t in ((Q, "q"), (K, "k")):
-            full = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X_, want_lowe=False, want_sums=False)
-            agree[t] = float((st["assign_" + t] == full["assign"]).float().mean())
-            agree_frozen[t] = float((frozen[t] == full["assign"]).float().mean())
-            Xf = X_[0].float()
-            def J(lab, mu):
-                idx = lab.long().unsqueeze(-1).expand(-1, -1, wl.D)
-                return float((Xf - torch.gather(mu, 1, idx)).pow(2).sum())
-            obj[t] = J(st["assign_" + t], st["mu_" + t]) / J(full["assign"], full["mu"])
-        row = {"report": "hybrid", "step": s, "kind": "anchor" if kind == b.HVA_ANCHOR else "subset", "ms_call": round(ms, 3),
-               "ms_clustering": round(ms_cl, 3), "agree_q": round(agree["q"], 4), "agree_k": round(agree["k"], 4),
-               "agree_frozen_q": round(agree_frozen["q"], 4), "agree_frozen_k": round(agree_frozen["k"], 4),
-               "rel_objective_q": round(obj["q"], 4), "rel_objective_k": round(obj["k"], 4)}
-        rows.append(row)
-        print(json.dumps(row), flush=True)
-    anc = [r for r in rows if r["kind"] == "anchor"]; sub = [r for r in rows if r["kind"] == "subset"]
-    mean = lambda xs, k: round(sum(x[k] for x in xs) / max(len(xs), 1), 4)
-    print(json.dumps({"report": "hybrid-summary", "workload": wl.name, "steps": len(rows), "subset_frac": 0.15,
-                      "anchor": {k: mean(anc, k) for k in ("ms_call", "ms_clustering")},
-                      "subset": {k: mean(sub, k) for k in ("ms_call", "ms_clustering", "agree_q", "agree_k", "agree_frozen_q",
-                                                           "agree_frozen_k", "rel_objective_q", "rel_objective_k")}}))
+        seq.append((X[0].contiguous(), X[1].contiguous(), X[2].contiguous()))
+    full = []                                                              # cold-start full re-clustering of every step (the yardstick)
+    for Q, K, V in seq:
+        fq = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, Q, want_lowe=False, want_sums=False)
+        fk = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, K, want_lowe=False, want_sums=False)
+        full.append({"q": (fq["assign"], fq["mu"]), "k": (fk["assign"], fk["mu"])})
+
+    def J(X, lab, mu):
+        idx = lab.long().unsqueeze(-1).expand(-1, -1, wl.D)
+        return float((X[0].float() - torch.gather(mu, 1, idx)).pow(2).sum())
+
+    variants = [(0, 10, 0.15), (1, 10, 0.15), (0, 2, 0.15), (1, 2, 0.15), (0, 10, 0.05), (0, 10, 0.30)]
+    O = torch.empty_like(seq[0][0])
+    for refresh, every, frac in variants:
+        cfg = b.make_config(wl, subset_frac=frac, refresh_all=refresh)
+        fwd = b.Forward(shape, cfg, with_state=True)
+        rows, frozen, prev_state = [], None, None
+        for s, (Q, K, V) in enumerate(seq):
+            kind = b.HVA_ANCHOR if s % every == 0 else b.HVA_INTERMEDIATE
+            a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); a.record()
+            fwd(Q, K, V, O, step_kind=kind)
+            e.record(); torch.cuda.synchronize()
+            ms = a.elapsed_time(e)
+            st = {k: v.clone() for k, v in fwd.state_views().items()}
+            if kind == b.HVA_ANCHOR:          # clustering part of the step, timed on copies of the cache
+                def clus():
+                    for X_, t in ((Q, "q"), (K, "k")):
+                        r = b.hva_cluster(shape, wl.cell, wl.win, wl.iters, X_, want_lowe=True)
+                        b.hva_select_subset(r["lowe"], st["subset_" + t].shape[1])
+                frozen = {t: (st["assign_" + t].clone(), st["mu_" + t].clone()) for t in "qk"}
+            else:
+                prev = prev_state
+                def clus():
+                    for X_, t in ((Q, "q"), (K, "k")):
+                        c2 = {k: prev[k + "_" + t].clone() for k in ("assign", "mu", "sums", "sizes")}
+                        b.hva_cluster_update(shape, X_, prev["subset_" + t], c2["assign"], c2["mu"], c2["sums"], c2["sizes"], refresh)
+            clus()
+            ms_cl = ev_time(clus, 1)
+            prev_state = st
+            row = {"report": "hybrid", "refresh_all": refresh, "anchor_every": every, "subset_frac": frac, "step": s,
+                   "kind": "anchor" if kind == b.HVA_ANCHOR else "subset", "ms_call": round(ms, 3), "ms_clustering": round(ms_cl, 3)}
+            for X_, t in ((Q, "q"), (K, "k")):
+                fl, fm = full[s][t]
+                jf = J(X_, fl, fm)
+                row["agree_" + t] = round(float((st["assign_" + t] == fl).float().mean()), 4)
+                row["agree_frozen_" + t] = round(float((frozen[t][0] == fl).float().mean()), 4)
+                row["rel_objective_" + t] = round(J(X_, st["assign_" + t], st["mu_" + t]) / jf, 4)
+                row["rel_objective_frozen_" + t] = round(J(X_, frozen[t][0], frozen[t][1]) / jf, 4)
+            rows.append(row)
+            if args.verbose:
+                print(json.dumps(row), flush=True)
+        anc = [r for r in rows if r["kind"] == "anchor"]; sub = [r for r in rows if r["kind"] == "subset"]
+        mean = lambda xs, k: round(sum(x[k] for x in xs) / max(len(xs), 1), 4)
+        keys = ("ms_call", "ms_clustering", "agree_q", "agree_k", "agree_frozen_q", "agree_frozen_k", "rel_objective_q", "rel_objective_k",
+                "rel_objective_frozen_q", "rel_objective_frozen_k")
+        print(json.dumps({"report": "hybrid-summary", "workload": wl.name, "heads": nh, "steps": len(rows), "refresh_all": refresh,
+                          "anchor_every": every, "subset_frac": frac, "anchor": {k: mean(anc, k) for k in ("ms_call", "ms_clustering")},
+                          "subset": {k: mean(sub, k) for k in keys},
+                          "last_subset_step_before_anchor": {k: mean([r for r in sub if (r["step"] + 1) % every == 0], k) for k in keys}}), flush=True)
+        del fwd
 
 
 def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
@@ -472,6 +561,8 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
     dense_flop = 4.0 * BH * float(n) * n * D
     t_att = st["attention"] * 1e-3
     ach = exec_flop / t_att / 1e12
+    default_cfg = (wl.name == "C4-hunyuan" and abs(float(cfg.top_p) - 0.9) < 1e-6 and int(cfg.merge_rounds) == 3 and
+                   list(cfg.cell_q) == list(wl.cell) and list(cfg.cell_k) == list(wl.cell) and list(cfg.win_q) == list(wl.win))
     pairs = sum(s["pairs_valid"] for s in stats)
     padded = tiles * tq * tk
     cl_bytes = 2 * wl.iters * BH * n * D * es + 2 * BH * n * 4      # X read once per iteration (Q and K) + labels
@@ -480,7 +571,7 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk):
         "stages_ms": {k: round(v, 4) for k, v in st.items()},
         "roofline": {"bound": "tensor", "kernel": "hva_attn_tc_kernel", "achieved": ach, "peak": pk["tf_sust"], "unit": "TFLOP/s",
                      "frac": ach / pk["tf_sust"], "frac_of_burst": ach / pk["tf_burst"], "peak_source": pk["src"] + " (sustained)",
-                     "traffic": ATTN_DRAM_BYTES_C4 if (wl.name == "C4-hunyuan" and abs(float(cfg.top_p) - 0.9) < 1e-6 and int(cfg.merge_rounds) == 3) else None,
+                     "traffic": attn_dram_bytes()[0] if default_cfg else None, "traffic_source": attn_dram_bytes()[1] if default_cfg else None,
                      "executed_tflop": exec_flop / 1e12, "dense_equiv_tflops": dense_flop / t_att / 1e12},
         "roofline_cluster": {"bound": "hbm", "kernel": "hva_assign_tc_kernel+hva_finalize_kernel", "achieved": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9,
                              "peak": pk["hbm"], "unit": "GB/s", "frac": cl_bytes / (st["cluster_qk"] * 1e-3) / 1e9 / pk["hbm"],

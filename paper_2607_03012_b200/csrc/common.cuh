@@ -75,3 +75,7 @@ size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D);
 size_t hva_merge_ws_bytes(int BH, int Nq, int Nk);
 size_t hva_plan_ws_bytes(int BH, int n, int Nq, int Nk);
 size_t hva_hybrid_ws_bytes(int BH, int n, int Nc, int m, int D);
+size_t hva_refresh_ws_bytes(int BH, int n, int Nc);
+// R-H3': mu, sums, sizes of every cluster recomputed from the current X and labels (plan.cu: label sort + segment means)
+int hva_refresh_centroids(int BH, int n, int Nc, int D, int dtype, const void* X, const int* assign, float* mu, float* sums, int* sizes,
+                          void* ws, size_t ws_bytes, cudaStream_t st);

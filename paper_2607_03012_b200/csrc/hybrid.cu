@@ -270,27 +270,9 @@ __global__ void hva_subset_commit_kernel(int n, int m, const int* __restrict__ s
   if (i < m) assign[(size_t)bh * n + subset[(size_t)bh * m + i]] = newlab[(size_t)bh * m + i];
 }
 
-// ---- R-H3': every centroid = mean of the current features of its members (token order => deterministic)
-template <typename T, int D>
-__global__ void __launch_bounds__(D) hva_refresh_kernel(int n, int Nc, const T* __restrict__ X, const int* __restrict__ assign,
-                                                        float* __restrict__ mu, float* __restrict__ sums, int* __restrict__ sizes) {
-  const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
-  float z = 0.f;
-  int cnt = 0;
-  for (int tok = 0; tok < n; ++tok) {
-    if (assign[(size_t)bh * n + tok] != u) continue;
-    z += HvaElem<T>::ld(X + ((size_t)bh * n + tok) * D + c);
-    ++cnt;
-  }
-  const size_t o = ((size_t)bh * Nc + u) * D + c;
-  sums[o] = z;
-  if (c == 0) sizes[(size_t)bh * Nc + u] = cnt;
-  if (cnt > 0) mu[o] = __fdiv_rn(z, (float)cnt);
-}
-
 template <typename T, int D>
 int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, int refresh_all, int* assign, float* mu,
-               float* sums, int* sizes, int* newlab, char* split, int dtype, uint32_t flags, cudaStream_t st) {
+               float* sums, int* sizes, int* newlab, char* split, int dtype, uint32_t flags, void* rws, size_t rws_bytes, cudaStream_t st) {
   int* oldlab = newlab + (size_t)BH * (m > 0 ? m : 1);
   const T* x = reinterpret_cast<const T*>(X);
   if (m > 0 && hva_subset_tc_supported(D, dtype, Nc) && !(flags & HVA_FLAG_CLUSTER_SIMT)) {
@@ -325,19 +307,18 @@ int run_update(int BH, int n, int Nc, int m, const void* X, const int* subset, i
     hva_subset_commit_kernel<<<dim3((m + 255) / 256, BH), 256, 0, st>>>(n, m, subset, newlab, assign);
     HVA_CHECK_LAUNCH();
   }
-  if (refresh_all) {
-    hva_refresh_kernel<T, D><<<dim3(Nc, BH), D, 0, st>>>(n, Nc, x, assign, mu, sums, sizes);
-    HVA_CHECK_LAUNCH();
-  }
+  if (refresh_all) HVA_TRY(hva_refresh_centroids(BH, n, Nc, D, dtype, X, assign, mu, sums, sizes, rws, rws_bytes, st));
   return HVA_OK;
 }
 
 }  // namespace
 
-size_t hva_hybrid_ws_bytes(int BH, int n, int Nc, int m, int D) {
-  (void)n;
+static size_t hybrid_step_bytes(int BH, int Nc, int m, int D) {
   return hva_align((size_t)BH * (m > 0 ? m : 1) * 8) + 2 * hva_align((size_t)BH * Nc * D * 2) + hva_align((size_t)BH * Nc * 4) +
          hva_align((size_t)BH * (Nc + 1) * 4) + hva_align((size_t)BH * Nc * 4) + hva_align((size_t)BH * 2 * (m > 0 ? m : 1) * 4);
+}
+size_t hva_hybrid_ws_bytes(int BH, int n, int Nc, int m, int D) {
+  return hybrid_step_bytes(BH, Nc, m, D) + hva_refresh_ws_bytes(BH, n, Nc);      // (the refresh of R-H3' sorts the tokens by label)
 }
 
 extern "C" size_t hva_cluster_update_workspace_bytes(const hva_shape* s, int32_t Nc, int32_t m) {
@@ -374,7 +355,9 @@ extern "C" int hva_cluster_update_ex(const hva_shape* s, int32_t Nc, const void*
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   int* newlab = reinterpret_cast<int*>(ws);
   char* split = reinterpret_cast<char*>(ws) + hva_align((size_t)BH * (m > 0 ? m : 1) * 8);
-#define HVA_DISPATCH(T, DD) return run_update<T, DD>(BH, n, Nc, m, X, subset, refresh_all, assign, mu, sums, sizes, newlab, split, s->dtype, flags, st)
+  void* rws = reinterpret_cast<char*>(ws) + hybrid_step_bytes(BH, Nc, m, s->D);
+  const size_t rws_bytes = hva_refresh_ws_bytes(BH, n, Nc);
+#define HVA_DISPATCH(T, DD) return run_update<T, DD>(BH, n, Nc, m, X, subset, refresh_all, assign, mu, sums, sizes, newlab, split, s->dtype, flags, rws, rws_bytes, st)
   if (s->dtype == HVA_F32) { if (s->D == 64) HVA_DISPATCH(float, 64); HVA_DISPATCH(float, 128); }
   if (s->D == 64) HVA_DISPATCH(__nv_bfloat16, 64);
   HVA_DISPATCH(__nv_bfloat16, 128);

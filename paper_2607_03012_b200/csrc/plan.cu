@@ -293,6 +293,50 @@ __global__ void __launch_bounds__(kSortWarps * 32) hva_sort_scatter_kernel(int n
   }
 }
 
+// ---- R-H3' (hybrid_refresh_all): every centroid = mean of the CURRENT features of its members.  Tokens are counting-sorted by
+// label with the kernels above; the per-label counts (= sizes) and their prefix come from the tile histograms.
+// one CTA per (b, head): count[c] = sum over tiles of hist[tile][c] (two labels per thread), block scan -> base[c]
+__global__ void __launch_bounds__(1024) hva_label_offsets_kernel(int Nc, int ntile, const int* __restrict__ hist, int* __restrict__ base,
+                                                                 int* __restrict__ sizes) {
+  const int bh = blockIdx.x, tid = threadIdx.x;
+  __shared__ int s_warp[32];
+  __shared__ int s_tot;
+  const int* h = hist + (size_t)bh * ntile * Nc;
+  int cnt[2] = {0, 0};
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const int c = 2 * tid + e;
+    if (c < Nc) for (int t = 0; t < ntile; ++t) cnt[e] += h[(size_t)t * Nc + c];
+  }
+  const int o = block_excl_scan(cnt[0] + cnt[1], s_warp, &s_tot);
+  if (2 * tid < Nc) { base[(size_t)bh * (Nc + 1) + 2 * tid] = o; sizes[(size_t)bh * Nc + 2 * tid] = cnt[0]; }
+  if (2 * tid + 1 < Nc) { base[(size_t)bh * (Nc + 1) + 2 * tid + 1] = o + cnt[0]; sizes[(size_t)bh * Nc + 2 * tid + 1] = cnt[1]; }
+  if (tid == 0) base[(size_t)bh * (Nc + 1) + Nc] = s_tot;
+}
+
+// one CTA per centroid, thread = feature dim: the members' rows are added in ascending token order (the sort is stable), four row
+// loads in flight; empty clusters keep mu (Alg. 2 line 23)
+template <typename T, int D>
+__global__ void __launch_bounds__(D) hva_segment_mean_kernel(int n, int Nc, const T* __restrict__ X, const int* __restrict__ perm,
+                                                             const int* __restrict__ base, float* __restrict__ mu,
+                                                             float* __restrict__ sums) {
+  const int u = blockIdx.x, bh = blockIdx.y, c = threadIdx.x;
+  const int b0 = base[(size_t)bh * (Nc + 1) + u], b1 = base[(size_t)bh * (Nc + 1) + u + 1];
+  const int* pm = perm + (size_t)bh * n;
+  const T* Xb = X + (size_t)bh * n * D;
+  float z = 0.f;
+  int i = b0;
+  for (; i + 4 <= b1; i += 4) {
+    const float x0 = HvaElem<T>::ld(Xb + (size_t)pm[i] * D + c), x1 = HvaElem<T>::ld(Xb + (size_t)pm[i + 1] * D + c);
+    const float x2 = HvaElem<T>::ld(Xb + (size_t)pm[i + 2] * D + c), x3 = HvaElem<T>::ld(Xb + (size_t)pm[i + 3] * D + c);
+    z += x0; z += x1; z += x2; z += x3;
+  }
+  for (; i < b1; ++i) z += HvaElem<T>::ld(Xb + (size_t)pm[i] * D + c);
+  const size_t o = ((size_t)bh * Nc + u) * D + c;
+  sums[o] = z;
+  if (b1 > b0) mu[o] = __fdiv_rn(z, (float)(b1 - b0));
+}
+
 // ---- S8 / S10: row gathers, 16 bytes per lane
 __global__ void hva_permute_kernel(size_t rows_total, int n, int row_chunks, const uint4* __restrict__ X,
                                    const int* __restrict__ perm, uint4* __restrict__ Y, int inverse) {
@@ -387,6 +431,46 @@ extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, con
   hva_sort_scan_kernel<<<dim3((Ncmax + 3) / 4, BH, 2), 128, 0, st>>>(ntile, A);
   HVA_CHECK_LAUNCH();
   hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
+}
+
+size_t hva_refresh_ws_bytes(int BH, int n, int Nc) {
+  const int ntile = (n + kTile - 1) / kTile;
+  return hva_align((size_t)BH * ntile * Nc * 4) + hva_align((size_t)BH * (Nc + 1) * 4) + hva_align((size_t)BH * n * 4);
+}
+
+// mu, sums, sizes of every cluster from the current X and labels (R-H3'); deterministic (token order)
+int hva_refresh_centroids(int BH, int n, int Nc, int D, int dtype, const void* X, const int* assign, float* mu, float* sums, int* sizes,
+                          void* ws, size_t ws_bytes, cudaStream_t st) {
+  if (Nc > 2048) return HVA_EUNSUPPORTED;
+  if (ws_bytes < hva_refresh_ws_bytes(BH, n, Nc)) return HVA_EWORKSPACE;
+  const int ntile = (n + kTile - 1) / kTile;
+  char* w = reinterpret_cast<char*>(ws);
+  int* hist = reinterpret_cast<int*>(w); w += hva_align((size_t)BH * ntile * Nc * 4);
+  int* base = reinterpret_cast<int*>(w); w += hva_align((size_t)BH * (Nc + 1) * 4);
+  int* perm = reinterpret_cast<int*>(w);
+  SortArgs A;
+  A.p[0] = SortPass{Nc, assign, hist, base, Nc + 1, perm, nullptr};
+  A.p[1] = A.p[0];
+  const dim3 gsort((ntile + kSortWarps - 1) / kSortWarps, BH, 1);
+  const size_t smem = (size_t)kSortWarps * Nc * sizeof(int);
+  hva_sort_hist_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_label_offsets_kernel<<<BH, 1024, 0, st>>>(Nc, ntile, hist, base, sizes);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scan_kernel<<<dim3((Nc + 3) / 4, BH, 1), 128, 0, st>>>(ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  const dim3 g(Nc, BH);
+  if (dtype == HVA_F32) {
+    if (D == 64) hva_segment_mean_kernel<float, 64><<<g, 64, 0, st>>>(n, Nc, reinterpret_cast<const float*>(X), perm, base, mu, sums);
+    else hva_segment_mean_kernel<float, 128><<<g, 128, 0, st>>>(n, Nc, reinterpret_cast<const float*>(X), perm, base, mu, sums);
+  } else {
+    if (D == 64) hva_segment_mean_kernel<__nv_bfloat16, 64><<<g, 64, 0, st>>>(n, Nc, reinterpret_cast<const __nv_bfloat16*>(X), perm, base, mu, sums);
+    else hva_segment_mean_kernel<__nv_bfloat16, 128><<<g, 128, 0, st>>>(n, Nc, reinterpret_cast<const __nv_bfloat16*>(X), perm, base, mu, sums);
+  }
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }
