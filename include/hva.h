@@ -49,6 +49,9 @@ extern "C" {
 #define HVA_FLAG_ATTN_SIMT 2u       /* S9: CUDA-core attention kernel instead of the tcgen05 kernel                            */
 #define HVA_FLAG_MASK_BLOCKSORT 4u  /* S5: block-level shared-memory sort instead of the warp-per-row register sort           */
 #define HVA_FLAG_MERGE_SIMT 8u      /* S6: per-pair bit-loop union sizes instead of the tcgen05 overlap contraction           */
+#define HVA_FLAG_Q_UNPERMUTED 16u   /* hva_sparse_attention: `Qp` is the UNPERMUTED Q; the tcgen05 kernel gathers its rows through the
+                                       plan's perm_q (Eq. 1 fused into the load, TMA tile::gather4).  hva_forward works this way: Q' is
+                                       never materialised.  EUNSUPPORTED with the CUDA-core kernel                            */
 
 /* Bipartition hash of Alg. 1 line 6 ("randomly bipartition", l.141; DESIGN.md R-M1):
  *   h  = seed*0x9E3779B1 ^ bh*0x85EBCA77 ^ round*0xC2B2AE3D ^ gid*0x27D4EB2F   (mod 2^32)
@@ -124,7 +127,8 @@ typedef struct {              /* byte offsets inside the workspace of hva_forwar
   size_t n_groups;            /* [BH] int32                                                                    */
   size_t group_mask;          /* [BH,Nq,Nk] uint8 chi of the active groups in gid order                        */
   size_t plan, plan_bytes;    /* the plan buffer (hva_plan_describe(BH, n, max(Nq,1), max(Nk,1), tile_q))      */
-  size_t qp, kp, vp;          /* permuted tensors Q', K', V' [B,heads,n,D] (Eq. 1)                             */
+  size_t qp, kp, vp;          /* permuted tensors Q', K', V' [B,heads,n,D] (Eq. 1); Q' has size 0 on the tensor-pipe path,
+                                 where the attention kernel gathers the rows of Q itself (HVA_FLAG_Q_UNPERMUTED)      */
   size_t scratch;             /* stage scratch                                                                 */
   size_t state;               /* where the per-tensor state lives when hva_forward is called with state == NULL */
   size_t total;               /* = hva_workspace_bytes()                                                       */

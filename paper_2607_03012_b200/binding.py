@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libhva.so")
 
 HVA_F32, HVA_BF16 = 0, 1
 HVA_ANCHOR, HVA_INTERMEDIATE, HVA_DENSE = 0, 1, 2
-HVA_FLAG_CLUSTER_SIMT, HVA_FLAG_ATTN_SIMT, HVA_FLAG_MASK_BLOCKSORT, HVA_FLAG_MERGE_SIMT = 1, 2, 4, 8
+HVA_FLAG_CLUSTER_SIMT, HVA_FLAG_ATTN_SIMT, HVA_FLAG_MASK_BLOCKSORT, HVA_FLAG_MERGE_SIMT, HVA_FLAG_Q_UNPERMUTED = 1, 2, 4, 8, 16
 
 EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_state_describe", "hva_workspace_describe",
            "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes", "hva_merge_workspace_bytes", "hva_plan_workspace_bytes",

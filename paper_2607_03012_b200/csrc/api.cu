@@ -14,6 +14,7 @@ struct FwdLayout {
   // per-call workspace
   size_t lowe, mask, group_of, n_groups, group_mask, plan, qp, kp, vp, scratch, scratch_bytes, ws_total;
   int Nq, Nk, n, BH, m;
+  bool fuse_q;
   hva_plan_layout PL;
 };
 
@@ -48,7 +49,9 @@ int make_layout(const hva_shape* s, const hva_config* c, FwdLayout* F) {
   o = 0;
   F->lowe = take(BH * n * 4); F->mask = take(BH * (size_t)F->Nq * F->Nk); F->group_of = take(BH * F->Nq * 4);
   F->n_groups = take(BH * 4); F->group_mask = take(BH * (size_t)F->Nq * F->Nk); F->plan = take(F->PL.total);
-  F->qp = take(BH * n * D * es); F->kp = take(BH * n * D * es); F->vp = take(BH * n * D * es);
+  // Q' is never materialised on the tensor-pipe path: the attention kernel gathers the Q rows through perm_q (TMA gather4)
+  F->fuse_q = s->dtype == HVA_BF16 && s->D == 128 && c->tile_q == 128 && c->tile_k == 128 && !(c->flags & HVA_FLAG_ATTN_SIMT);
+  F->qp = take(F->fuse_q ? 0 : BH * n * D * es); F->kp = take(BH * n * D * es); F->vp = take(BH * n * D * es);
   HvaGrid gq = hva_make_grid(s, c->cell_q, c->win_q), gk = hva_make_grid(s, c->cell_k, c->win_k);
   size_t sc = hva_cluster_ws_bytes(gq, F->BH, s->D);
   sc = std::max(sc, hva_cluster_ws_bytes(gk, F->BH, s->D));
@@ -129,7 +132,9 @@ extern "C" int hva_sparse_attention(const hva_shape* s, const hva_config* c, con
   const float scale = c->softmax_scale > 0.f ? c->softmax_scale : 1.0f / sqrtf((float)s->D);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const bool tc_ok = s->dtype == HVA_BF16 && s->D == 128 && c->tile_q == 128 && c->tile_k == 128;
-  if (tc_ok && !(c->flags & HVA_FLAG_ATTN_SIMT)) return hva_attention_tc_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st);
+  if (tc_ok && !(c->flags & HVA_FLAG_ATTN_SIMT))
+    return hva_attention_tc_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, (c->flags & HVA_FLAG_Q_UNPERMUTED) != 0, st);
+  if (c->flags & HVA_FLAG_Q_UNPERMUTED) return HVA_EUNSUPPORTED;
   return hva_attention_simt_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st, c->tile_q);
 }
 
@@ -192,10 +197,13 @@ int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const v
                          (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), group_of, n_groups, gmask, c->tile_q,
                          c->tile_k, plan, F.PL.total, w + F.scratch, F.scratch_bytes, stream));
   const char* pb = reinterpret_cast<const char*>(plan);
-  HVA_TRY(hva_permute(s, Q, (const int32_t*)(pb + F.PL.perm_q), w + F.qp, stream));
+  if (!F.fuse_q) HVA_TRY(hva_permute(s, Q, (const int32_t*)(pb + F.PL.perm_q), w + F.qp, stream));
   HVA_TRY(hva_permute(s, K, (const int32_t*)(pb + F.PL.perm_k), w + F.kp, stream));
   HVA_TRY(hva_permute(s, V, (const int32_t*)(pb + F.PL.perm_k), w + F.vp, stream));
-  HVA_TRY(hva_sparse_attention(s, c, w + F.qp, w + F.kp, w + F.vp, plan, F.PL.total, F.Nq, F.Nk, O, 1, nullptr, 0, stream));
+  hva_config ca = *c;
+  if (F.fuse_q) ca.flags |= HVA_FLAG_Q_UNPERMUTED;
+  HVA_TRY(hva_sparse_attention(s, &ca, F.fuse_q ? Q : (const void*)(w + F.qp), w + F.kp, w + F.vp, plan, F.PL.total, F.Nq, F.Nk, O, 1, nullptr, 0,
+                               stream));
   if (stats_out && cudaMemcpyAsync(stats_out, pb + F.PL.stats, sizeof(hva_stats) * BH, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
     return HVA_ECUDA;
   return HVA_OK;

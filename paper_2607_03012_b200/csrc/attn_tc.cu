@@ -38,13 +38,13 @@ constexpr float kRescaleThreshold = 8.0f;      // log2 units
 constexpr int kPolyPairs = 0;
 
 struct TcMaps {
-  CUtensorMap q;
+  CUtensorMap q;        // Q' (permuted) as 128-row boxes, or -- gather mode -- the UNPERMUTED Q as 1-row boxes for tile::gather4
   CUtensorMap k[kNumBoxes];
   CUtensorMap v[kNumBoxes];
 };
 
 struct TcParams {
-  int n, Nq, Nk, run_stride, work_cap, unpermute;
+  int n, Nq, Nk, run_stride, work_cap, unpermute, gather_q;
   float scale_log2;
   const int *goff, *koff, *kappa, *run_cnt, *work_cnt, *work, *perm_q;
   const uint32_t* runs;
@@ -190,10 +190,29 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     // the K ring is on the critical path (QK_{j+2} is issued two tiles ahead): one warp per 64-dim half; one warp for the V ring
     const bool is_k = (warp == 8 || warp == 11);   // 8: K dims 0-63 (+Q), 11: K dims 64-127, 10: V dims 0-63, 12: V dims 64-127
     const int half = warp >= 11;
-    if (warp == 8 && elect_one()) {
+    if (warp == 8 && !p.gather_q && elect_one()) {
       mbar_expect_tx(&B->q_full, kTileBytes);
       tma_load_2d(&maps.q, &B->q_full, sQ, 0, base_row + row0);
       tma_load_2d(&maps.q, &B->q_full, sQ + kHalfBytes, 64, base_row + row0);
+    }
+    if (warp == 8 && p.gather_q) {
+      // Q' = Pi^q Q fused into the load (Eq. 1): the tile's 128 rows are gathered from the unpermuted Q through perm_q, four rows per
+      // TMA tile::gather4 instruction (each lands as four consecutive 128-byte rows of the swizzled tile).  Rows past the end of the
+      // group repeat its last row (finite, never stored).
+      const int* pq = p.perm_q + (size_t)base_row + row0;
+      int tok[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) tok[k] = base_row + pq[min(4 * lane + k, row1 - row0 - 1)];
+      if (lane == 0) mbar_expect_tx(&B->q_full, kTileBytes);
+      for (int i = 0; i < 32; ++i) {
+        const int t0 = __shfl_sync(0xffffffffu, tok[0], i), t1 = __shfl_sync(0xffffffffu, tok[1], i);
+        const int t2 = __shfl_sync(0xffffffffu, tok[2], i), t3 = __shfl_sync(0xffffffffu, tok[3], i);
+        if (lane == 0) {
+          tma_gather4_2d(&maps.q, &B->q_full, sQ + i * 512, 0, t0, t1, t2, t3);
+          tma_gather4_2d(&maps.q, &B->q_full, sQ + kHalfBytes + i * 512, 64, t0, t1, t2, t3);
+        }
+      }
+      __syncwarp();
     }
     RunWalker w{p.runs + ((size_t)bh * p.Nq + g) * p.run_stride, p.koff + (size_t)bh * (p.Nk + 1),
                 p.run_cnt[(size_t)bh * p.Nq + g], 0, 0, 0, 0};
@@ -465,21 +484,21 @@ extern "C" void hva_debug_attn_timing(unsigned long long* dev16) { g_attn_timing
 #endif
 
 int hva_attention_tc_launch(const hva_shape* s, float scale, const void* Qp, const void* Kp, const void* Vp,
-                            const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute,
+                            const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute, int gather_q,
                             cudaStream_t st) {
   if (s->D != kD || s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
   const int n = s->T * s->H * s->W, BH = s->B * s->heads;
   const uint64_t rows = (uint64_t)BH * n;
   if (rows >= (1ull << 31)) return HVA_EUNSUPPORTED;
   TcMaps maps;
-  if (!make_map(&maps.q, Qp, rows, kBM)) return HVA_ECUDA;
+  if (!make_map(&maps.q, Qp, rows, gather_q ? 1 : kBM)) return HVA_ECUDA;
   for (int b = 0; b < kNumBoxes; ++b) {
     if (!make_map(&maps.k[b], Kp, rows, 1u << b)) return HVA_ECUDA;
     if (!make_map(&maps.v[b], Vp, rows, 1u << b)) return HVA_ECUDA;
   }
   const char* b = reinterpret_cast<const char*>(plan);
   TcParams p;
-  p.n = n; p.Nq = Nq; p.Nk = Nk; p.run_stride = (int)L.run_stride; p.work_cap = (int)L.work_cap; p.unpermute = unpermute;
+  p.n = n; p.Nq = Nq; p.Nk = Nk; p.run_stride = (int)L.run_stride; p.work_cap = (int)L.work_cap; p.unpermute = unpermute; p.gather_q = gather_q;
   p.scale_log2 = scale * 1.4426950408889634f;
   p.goff = (const int*)(b + L.goff); p.koff = (const int*)(b + L.koff); p.kappa = (const int*)(b + L.kappa);
   p.run_cnt = (const int*)(b + L.run_cnt); p.work_cnt = (const int*)(b + L.work_cnt); p.work = (const int*)(b + L.work);

@@ -58,7 +58,7 @@ template <> struct HvaElem<__nv_bfloat16> {
 
 // Entry points implemented across translation units (internal linkage to the library).
 int hva_attention_tc_launch(const hva_shape* s, float scale, const void* Qp, const void* Kp, const void* Vp,
-                            const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute,
+                            const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute, int gather_q,
                             cudaStream_t st);
 int hva_attention_simt_launch(const hva_shape* s, float scale, const void* Qp, const void* Kp, const void* Vp,
                               const void* plan, const hva_plan_layout& L, int Nq, int Nk, void* O, int unpermute,

@@ -34,6 +34,15 @@ __device__ __forceinline__ void tma_load_2d(const CUtensorMap* map, uint64_t* ba
       "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
       : "memory");
 }
+// four rows (row coordinates r0..r3) x one box width of a 2-D tensor map whose box is {cols, 1 row}: they land as four consecutive
+// rows of the (swizzled) shared-memory tile
+__device__ __forceinline__ void tma_gather4_2d(const CUtensorMap* map, uint64_t* bar, void* dst, int c0, int r0, int r1, int r2, int r3) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
+      : "memory");
+}
 // one lane of a converged warp (the rest of the warp keeps executing the surrounding, warp-uniform code: addresses and
 // descriptors then live in uniform registers, which is what UTCHMMA / UTMALDG take)
 __device__ __forceinline__ bool elect_one() {

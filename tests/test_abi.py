@@ -39,7 +39,8 @@ def test_host_only_entry_points(lib):
     shape, cfg = b.make_shape(wl), b.make_config(wl)
     assert b.hva_num_clusters(shape, wl.cell) == 990       # 11 x 9 x 10 (BASELINE.json configs[3])
     ws, st = b.hva_workspace_bytes(shape, cfg), lib.hva_state_bytes(C.byref(shape), C.byref(cfg))
-    assert ws > 3 * wl.heads * wl.n * wl.D * 2 and 0 < st < ws          # Q', K', V' live in the workspace
+    assert ws > 2 * wl.heads * wl.n * wl.D * 2 and 0 < st < ws          # K', V' live in the workspace (Q' is gathered inside the kernel)
+    assert ws < 3 * wl.heads * wl.n * wl.D * 2
     L = b.hva_plan_describe(24, wl.n, 990, 990, 128)
     assert L.work_cap >= -(-wl.n // 128) + 990 and L.total > 3 * 24 * wl.n * 4
     assert lib.hva_cluster_workspace_bytes(C.byref(shape), (C.c_int32 * 3)(*wl.cell), (C.c_int32 * 3)(*wl.win)) > 0
@@ -95,4 +96,4 @@ def test_library_reads_no_environment_and_keeps_no_probe_pointers():
         src = open(os.path.join(csrc, f)).read()
         assert "getenv" not in src and "strtoull" not in src, f
     cfg = b.make_config(inputs.C2, flags=b.HVA_FLAG_ATTN_SIMT | b.HVA_FLAG_MERGE_SIMT)
-    assert cfg.flags == 10 and C.sizeof(b.hva_config) == 4 * (12 + 12)
+    assert cfg.flags == 10 and C.sizeof(b.hva_config) == 4 * (12 + 12) and b.HVA_FLAG_Q_UNPERMUTED == 16

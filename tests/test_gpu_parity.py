@@ -280,6 +280,9 @@ def run_downstream_parity(wl, heads, top_p, rounds, rows_per_head=None, seed_row
     Operm = b.hva_sparse_attention(shape, cfg, Qp, Kp, Vp, plan, unpermute=False)
     torch.cuda.synchronize()
     assert torch.equal(b.hva_unpermute(shape, Operm, plan.perm_q), O)
+    if wl.dtype == "bf16" and wl.D == 128:             # Eq. 1 fused into the load: the kernel gathers the rows of the UNPERMUTED Q (TMA gather4)
+        cfg_g = b.make_config(wl, top_p=top_p, merge_rounds=rounds, max_q_tiles=max_q_tiles, flags=b.HVA_FLAG_Q_UNPERMUTED)
+        assert torch.equal(b.hva_sparse_attention(shape, cfg_g, dev[0], Kp, Vp, plan, unpermute=True), O)
     check_attention(wl, heads, f64, O, [(c[0]["assign"], c[1]["assign"]) for c in cl], merged, rows_per_head, seed_rows)
     return plan, stats
 
