@@ -131,35 +131,41 @@ __global__ void __launch_bounds__(kMaskThreads) hva_mask_kernel(int Nq, int Nk, 
 // (thread = key cluster, every mu^k element read once for 8 fp64 dot products); then warp w owns row w: each lane holds E
 // of the row's P = 32 E (weight, j) pairs in registers (position = lane E + i) and the bitonic network runs without shared
 // memory or block barriers: distances < E are register-to-register inside a lane, distances >= E are lane-to-lane shuffles.
+// One element = ONE 64-bit key: the weight's fp64 bits (w >= 0: bit order == value order) with the low 11 mantissa bits replaced
+// by 2047 - j, so that "weight descending, ties -> lower j" is a single unsigned compare and a swap moves two registers (round 1
+// sorted (double, int) pairs with two fp64 compares per exchange: 19.5 % fp64 pipe, 1.66 ms at C4).  The weight loses 11 of its 52
+// mantissa bits (relative 4.5e-13): the cumulative sums below use the truncated weights, far inside R-K3's 1e-9 Z exemption; two
+// DIFFERENT weights that agree in their leading 41 mantissa bits are ordered by index instead of by value (probability ~1e-10 per
+// adjacent pair, and it only matters if the cut falls between the two).  Exact ties, empty clusters (w = 0) and pads (key 0,
+// j >= N_k) order exactly as the oracle's.
 template <int E>
 struct WarpSort {
-  double w[E];
-  int j[E];
-  __device__ __forceinline__ void cex(int a, int b, bool up) {      // positions a < b inside the lane
-    const bool sw = up ? before(w[b], j[b], w[a], j[a]) : before(w[a], j[a], w[b], j[b]);
-    if (sw) { double tw = w[a]; w[a] = w[b]; w[b] = tw; int tj = j[a]; j[a] = j[b]; j[b] = tj; }
+  unsigned long long k[E];
+  __device__ __forceinline__ void cex(int a, int b, bool up) {      // positions a < b inside the lane; `up`: larger key first
+    const unsigned long long x = k[a], y = k[b];
+    const bool sw = up ? (y > x) : (x > y);
+    k[a] = sw ? y : x; k[b] = sw ? x : y;
   }
   __device__ __forceinline__ void sort(int lane) {
 #pragma unroll
-    for (int k = 2; k <= 32 * E; k <<= 1) {
+    for (int kk = 2; kk <= 32 * E; kk <<= 1) {
 #pragma unroll
-      for (int d = k >> 1; d > 0; d >>= 1) {
+      for (int d = kk >> 1; d > 0; d >>= 1) {
         if (d >= E) {                                                 // partner lane, same register index
           const int lm = d / E;
-          const bool up = ((lane * E) & k) == 0, lower = (lane & lm) == 0;
-          const bool keep_first = (lower == up);                      // this position keeps the pair's `before` element
+          const bool up = ((lane * E) & kk) == 0, lower = (lane & lm) == 0;
+          const bool keep_larger = (lower == up);                     // this position keeps the pair's larger key
 #pragma unroll
           for (int i = 0; i < E; ++i) {
-            const double ow = __shfl_xor_sync(0xffffffffu, w[i], lm);
-            const int oj = __shfl_xor_sync(0xffffffffu, j[i], lm);
-            const bool mine_first = before(w[i], j[i], ow, oj);
-            if (mine_first != keep_first) { w[i] = ow; j[i] = oj; }
+            const unsigned long long o = __shfl_xor_sync(0xffffffffu, k[i], lm);
+            const bool mine_larger = k[i] > o;
+            if (mine_larger != keep_larger) k[i] = o;
           }
         } else {
 #pragma unroll
           for (int i = 0; i < E; ++i) {
             if ((i & d) == 0) {
-              const bool up = k < E ? ((i & k) == 0) : ((((lane * E) | i) & k) == 0);
+              const bool up = kk < E ? ((i & kk) == 0) : ((((lane * E) | i) & kk) == 0);
               cex(i, i | d, up);
             }
           }
@@ -168,6 +174,11 @@ struct WarpSort {
     }
   }
 };
+__device__ __forceinline__ unsigned long long mask_key(double w, int j) {     // w >= 0
+  return ((unsigned long long)__double_as_longlong(w) & ~0x7FFull) | (unsigned long long)(2047 - j);
+}
+__device__ __forceinline__ double mask_key_w(unsigned long long k) { return __longlong_as_double((long long)(k & ~0x7FFull)); }
+__device__ __forceinline__ int mask_key_j(unsigned long long k) { return 2047 - (int)(k & 0x7FFull); }
 
 constexpr int kWarpRows = 8;
 
@@ -211,23 +222,25 @@ __global__ void __launch_bounds__(256, 2) hva_mask_warp_kernel(int Nq, int Nk, c
   const double* sc = s_sc + (size_t)warp * P;
   WarpSort<E> ws;
   double smax = -1.0 / 0.0;
+  double wv[E];
 #pragma unroll
   for (int i = 0; i < E; ++i) {                              // initial placement is arbitrary: key j = 32 i + lane (conflict-free)
     const int jj = 32 * i + lane;
-    ws.j[i] = jj;
-    ws.w[i] = jj < Nk ? sc[jj] : -1.0 / 0.0;
-    smax = fmax(smax, ws.w[i]);
+    wv[i] = jj < Nk ? sc[jj] : -1.0 / 0.0;
+    smax = fmax(smax, wv[i]);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
 #pragma unroll
-  for (int i = 0; i < E; ++i)                                // w_j = s^k_j exp(S_j - max); pads (-1) sort last
-    ws.w[i] = ws.j[i] < Nk ? (double)sizes_k[(size_t)bh * Nk + ws.j[i]] * exp(ws.w[i] - smax) : -1.0;
+  for (int i = 0; i < E; ++i) {                              // w_j = s^k_j exp(S_j - max); pads get the smallest key of all (0, j >= N_k)
+    const int jj = 32 * i + lane;
+    ws.k[i] = jj < Nk ? mask_key((double)sizes_k[(size_t)bh * Nk + jj] * exp(wv[i] - smax), jj) : (unsigned long long)(2047 - jj);
+  }
   ws.sort(lane);
   // inclusive scan of the sorted weights: sequential inside a lane (positions lane E .. lane E + E - 1), shuffle scan across lanes
   double run = 0.0;
 #pragma unroll
-  for (int i = 0; i < E; ++i) run += ws.w[i] > 0.0 ? ws.w[i] : 0.0;
+  for (int i = 0; i < E; ++i) run += mask_key_w(ws.k[i]);
   double incl = run;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
@@ -239,15 +252,17 @@ __global__ void __launch_bounds__(256, 2) hva_mask_warp_kernel(int Nq, int Nk, c
   int first = Nk;                                            // smallest k with cum_k >= p Z   (Eq. 3)
 #pragma unroll
   for (int i = 0; i < E; ++i) {
-    a += ws.w[i] > 0.0 ? ws.w[i] : 0.0;
+    a += mask_key_w(ws.k[i]);
     if (a >= thr && first == Nk && lane * E + i < Nk) first = lane * E + i + 1;
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) first = min(first, __shfl_xor_sync(0xffffffffu, first, o));
   const int kcut = first < kmin ? kmin : first;
 #pragma unroll
-  for (int i = 0; i < E; ++i)
-    if (ws.j[i] < Nk) mrow[ws.j[i]] = (lane * E + i < kcut) ? 1 : 0;
+  for (int i = 0; i < E; ++i) {
+    const int jj = mask_key_j(ws.k[i]);
+    if (jj < Nk) mrow[jj] = (lane * E + i < kcut) ? 1 : 0;
+  }
 }
 
 template <int D, int E>
