@@ -31,22 +31,24 @@ __device__ __forceinline__ uint4 expand8(uint32_t bits, const uint4& v4) {
   return make_uint4(v4.x & m0, v4.y & m1, v4.z & m2, v4.w & m3);
 }
 
-constexpr int kRowsPerThread = 3;      // (1 + 4) tiles x 128 rows = 640 rows over 256 threads
+constexpr int kColBlocks = 2;          // 128-group column blocks per CTA: 256 TMEM columns and 48 KB of tiles, so that TWO CTAs share an SM and
+                                       // one expands its tiles while the other's MMAs run (4 blocks / one CTA per SM: 0.31 ms per round at C4)
+constexpr int kRowsPerThread = ((1 + kColBlocks) * 128 + 255) / 256;      // (1 + kColBlocks) tiles x 128 rows over 256 threads
 
-__global__ void __launch_bounds__(kThreadsG, 1) hva_merge_inter_kernel(InterParams p) {
-  const int bh = blockIdx.z, mb = blockIdx.x, cg = blockIdx.y;          // rows [128 mb, +128), column blocks 4 cg .. 4 cg + 3
+__global__ void __launch_bounds__(kThreadsG, 2) hva_merge_inter_kernel(InterParams p) {
+  const int bh = blockIdx.z, mb = blockIdx.x, cg = blockIdx.y;          // rows [128 mb, +128), column blocks kColBlocks cg ...
   const int tid = threadIdx.x, warp = tid >> 5;
-  const int ncb = min(4, p.Nqp / 128 - 4 * cg);                         // column blocks of this CTA
+  const int ncb = min(kColBlocks, p.Nqp / 128 - kColBlocks * cg);      // column blocks of this CTA
   const int nt = p.nterms[bh];
   extern __shared__ unsigned char raw[];
   unsigned char* smem = raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);
   unsigned char* sA = smem;                                             // [128][128 B]   chi(A) as 1.0 / 0
-  unsigned char* sB = smem + kTileB;                                    // [4 column blocks][128][128 B]  chi(B) . digit_t(s^k)
-  uint4* s_v = reinterpret_cast<uint4*>(sB + 4 * kTileB);               // [8] the chunk's 64 bf16 digits of s^k, 8 per entry
+  unsigned char* sB = smem + kTileB;                                    // [kColBlocks][128][128 B]  chi(B) . digit_t(s^k)
+  uint4* s_v = reinterpret_cast<uint4*>(sB + kColBlocks * kTileB);      // [8] the chunk's 64 bf16 digits of s^k, 8 per entry
   __shared__ uint64_t bar;
   __shared__ uint32_t tbase;
   if (tid == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
-  if (warp == 0) tmem_alloc(&tbase, 512);
+  if (warp == 0) tmem_alloc(&tbase, 128 * kColBlocks);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -64,7 +66,7 @@ __global__ void __launch_bounds__(kThreadsG, 1) hva_merge_inter_kernel(InterPara
     const int e = tid + 256 * k, tile = e >> 7, r = e & 127;
     grp[k] = -1; dst[k] = sA;
     if (tile < 1 + ncb) {
-      const int gg = tile == 0 ? 128 * mb + r : 128 * (4 * cg + tile - 1) + r;
+      const int gg = tile == 0 ? 128 * mb + r : 128 * (kColBlocks * cg + tile - 1) + r;
       grp[k] = gg < p.Nq ? gg : -2;                                      // -2: row of zeros
       dst[k] = (tile == 0 ? sA : sB + (size_t)(tile - 1) * kTileB) + r * 128;
     }
@@ -136,7 +138,7 @@ __global__ void __launch_bounds__(kThreadsG, 1) hva_merge_inter_kernel(InterPara
           uint32_t v[32];
           tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + cb * 128 + cc * 32, v);
           if (r < p.Nq) {
-            int* out = p.inter + ((size_t)bh * p.Nqp + r) * p.Nqp + 128 * (4 * cg + cb) + cc * 32;
+            int* out = p.inter + ((size_t)bh * p.Nqp + r) * p.Nqp + 128 * (kColBlocks * cg + cb) + cc * 32;
 #pragma unroll
             for (int i = 0; i < 32; i += 4) {
               int4 o = make_int4((int)__uint_as_float(v[i]) << (8 * t), (int)__uint_as_float(v[i + 1]) << (8 * t),
@@ -152,7 +154,7 @@ __global__ void __launch_bounds__(kThreadsG, 1) hva_merge_inter_kernel(InterPara
     __syncthreads();     // TMEM read before the next digit overwrites it (accumulate flag restarts at c == 0)
     tc_fence_after();
   }
-  if (warp == 0) tmem_dealloc(tmem, 512);
+  if (warp == 0) tmem_dealloc(tmem, 128 * kColBlocks);
 }
 
 __global__ void hva_merge_nterms_kernel(int Nk, const int* __restrict__ sizes_k, int* __restrict__ nterms) {
@@ -184,11 +186,11 @@ int hva_merge_nterms_launch(int BH, int Nk, const int* sizes_k, int* nterms, cud
 
 int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, cudaStream_t st) {
   InterParams p{Nq, Nk, (Nk + 31) / 32, (Nq + 127) / 128 * 128, chi, sizes_k, nterms, inter};
-  const size_t smem = 1024 + 5 * (size_t)kTileB + 8 * 16 + 64;
+  const size_t smem = 1024 + (1 + kColBlocks) * (size_t)kTileB + 8 * 16 + 64;
   // (per device and cheap: set on every call rather than behind a process-wide flag)
   if (cudaFuncSetAttribute(hva_merge_inter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return HVA_ECUDA;
   const int nrb = p.Nqp / 128;
-  hva_merge_inter_kernel<<<dim3(nrb, (nrb + 3) / 4, BH), kThreadsG, smem, st>>>(p);
+  hva_merge_inter_kernel<<<dim3(nrb, (nrb + kColBlocks - 1) / kColBlocks, BH), kThreadsG, smem, st>>>(p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }
