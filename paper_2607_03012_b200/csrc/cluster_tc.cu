@@ -208,6 +208,8 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
   if (warp == kLoadWarp) {
     // ================================================================ loader
     const uint32_t tile_bytes = (uint32_t)(2 * ctok * 128 + 4 * nwin * 128);
+    // the tokens stream through L2 once per pass (evict first); the centroids and the partial rows are what should stay there
+    const uint64_t pol_x = l2_policy_evict_first(), pol_mu = l2_policy_evict_last();
     int item = blockIdx.x;                   // (the grid never exceeds n_items)
     int n_term = 0;
     int i = 0, jb = 0, ib = 0, ia = 0, ix = 0;   // slot / centroid buffer / token buffer of tile q; slots of tiles q - NB, q - NT
@@ -239,12 +241,12 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
         const int t0 = t.ut * g.kt + t.chunk * p.ct;
         if (elect_one()) {
           mbar_expect_tx(&S->full, tile_bytes);
-          tma_load_5d(&map_hi, &S->full, sBhi, 0, sw, sh, st, t.bh);
-          tma_load_5d(&map_hi, &S->full, sBhi + 2 * half_b, 64, sw, sh, st, t.bh);
-          tma_load_5d(&map_lo, &S->full, sBlo, 0, sw, sh, st, t.bh);
-          tma_load_5d(&map_lo, &S->full, sBlo + 2 * half_b, 64, sw, sh, st, t.bh);
-          tma_load_5d(&map_x, &S->full, sA, 0, t.uw * g.kw, t.uh * g.kh, t0, t.bh);
-          tma_load_5d(&map_x, &S->full, sA + half_a, 64, t.uw * g.kw, t.uh * g.kh, t0, t.bh);
+          tma_load_5d_hint(&map_hi, &S->full, sBhi, 0, sw, sh, st, t.bh, pol_mu);
+          tma_load_5d_hint(&map_hi, &S->full, sBhi + 2 * half_b, 64, sw, sh, st, t.bh, pol_mu);
+          tma_load_5d_hint(&map_lo, &S->full, sBlo, 0, sw, sh, st, t.bh, pol_mu);
+          tma_load_5d_hint(&map_lo, &S->full, sBlo + 2 * half_b, 64, sw, sh, st, t.bh, pol_mu);
+          tma_load_5d_hint(&map_x, &S->full, sA, 0, t.uw * g.kw, t.uh * g.kh, t0, t.bh, pol_x);
+          tma_load_5d_hint(&map_x, &S->full, sA + half_a, 64, t.uw * g.kw, t.uh * g.kh, t0, t.bh, pol_x);
         }
         __syncwarp();
         CMARK(4);
