@@ -6,8 +6,10 @@ path (`paper_2607_03012_b200/csrc`, `paper_2607_03012_b200/binding.py`) and neit
 the other.  Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` /
 `--impl reference` legs may import this package.
 
-Parity status of each function is stated in its module header; the one step the paper does
-not pin (the hybrid intermediate update, reading R-H3 in DESIGN.md) says "parity unpinned".
+Parity status of each function is stated in its module header.  Every function has a pin that does
+not come from the oracle itself (hand fixtures, brute force, closed forms, invariants:
+tests/test_oracle_*.py); the hybrid intermediate update follows reading R-H3 / R-H3' of DESIGN.md and
+is pinned by the invariant "incremental update == recomputation from the labels" (see oracle/hybrid.py).
 """
 from .grid import grid_dims, clip_window, window_start, centre_token, home_cell, window_ids  # noqa: F401
 from .cluster import local_window_kmeans, lowe_ratio  # noqa: F401

@@ -1,7 +1,7 @@
 // S1 (+ the per-cell part of S2) on the tensor pipe (bf16 inputs, D = 128): assignment step of 3D local-window
 // k-means and the per-(cell, slot) partial centroid sums (Alg. 2 lines 14-21, l.367-381; Eq. 5 l.81; Eq. 6 l.97).
 //
-// The direct form sum_c (x_c - mu_c)^2 on CUDA cores is ALU-bound (profiles/r1b: 6.5 % of DRAM peak).
+// The direct form sum_c (x_c - mu_c)^2 on CUDA cores is ALU-bound (round 1, first ncu capture: 6.5 % of DRAM peak).
 // Here the 27.D dot products leave the FP32 pipe:
 //   score_v = |mu_v|^2 - 2 x.mu_v  ( = d^2_v - |x|^2 ),   x.mu_v = x.hi_v + x.lo_v
 // with mu split into two bf16 terms (hi = RN(mu), lo = RN(mu - hi); |mu - hi - lo| <= 2^-18 |mu|), so
@@ -32,7 +32,7 @@
 // (a single warp runs dependent integer code at one instruction per 4-8 clk: every role loop keeps its slot index and barrier
 // parity incrementally -- a runtime q % NT is ~40 instructions -- and no role does two long-latency things per tile)
 // Round 1's kernel ran these steps in line in four independent 128-thread CTAs per SM (9.5 K clk per tile, of which the
-// scan threads waited for TMA / MMA round trips and block barriers more than half: profiles/r1f, r2*): the same four tiles
+// scan threads waited for TMA / MMA round trips and block barriers more than half; now: profiles/r2_assign_phases.md): the same four tiles
 // per SM were in flight, but a warp that waits now has another tile to work on.
 #include "common.cuh"
 #include "ptx.cuh"
