@@ -35,6 +35,7 @@ extern "C" {
 #define HVA_EWORKSPACE (-2)   /* ws_bytes / plan_bytes / state_bytes too small */
 #define HVA_EUNSUPPORTED (-3) /* dtype / tile / size combination without a kernel */
 #define HVA_ECUDA (-4)        /* a CUDA runtime call or launch failed (cudaGetLastError) */
+#define HVA_ELIMIT (-5)       /* the problem needs more scratch than the built-in array of a *_static entry point holds */
 
 #define HVA_ANCHOR 0          /* full clustering (and, if subset_frac>0, refresh the hybrid cache) */
 #define HVA_INTERMEDIATE 1    /* hybrid: re-assign only the cached subset (l.101)                  */
@@ -227,6 +228,23 @@ int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, const int32_t*
                    const int32_t* group_of_cluster, const int32_t* n_groups, const uint8_t* group_mask,
                    int32_t tile_q, int32_t tile_k, void* plan, size_t plan_bytes,
                    void* ws, size_t ws_bytes, void* stream);
+
+/* hva_build_plan for callers that may not allocate device memory and have no scratch buffer to hand over (code under CUDA
+ * graph capture, serving loops, harnesses that forbid cudaMalloc): same inputs, same `plan` output (bit-identical), but the
+ * scratch is a device array built into the library, HVA_PLAN_STATIC_SCRATCH_BYTES large, which every GPU that loads the
+ * library holds until the process exits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine);
+ * its first use on a device looks the array's device address up (cudaGetSymbolAddress, with the caller's current device).
+ * Limit: hva_plan_workspace_bytes(BH, n, Nq, Nk) <= hva_build_plan_static_limit() (32 MiB: C4 with 24 heads needs 22.3 MB,
+ * C3 with 40 heads 15.0 MB); beyond it the call returns HVA_ELIMIT and enqueues nothing -- use hva_build_plan with a
+ * caller-owned buffer.  All calls on a device SHARE the array, and it keeps the previous call's contents: nothing in it has to
+ * start at zero (every word a kernel reads is written earlier in the same call), but two calls that overlap on the GPU
+ * (different streams) race on it; calls on one stream are ordered.  Other errors as hva_build_plan. */
+#define HVA_PLAN_STATIC_SCRATCH_BYTES (32u << 20)
+size_t hva_build_plan_static_limit(void);
+int hva_build_plan_static(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, const int32_t* assign_q,
+                          const int32_t* assign_k, const int32_t* sizes_q, const int32_t* sizes_k,
+                          const int32_t* group_of_cluster, const int32_t* n_groups, const uint8_t* group_mask,
+                          int32_t tile_q, int32_t tile_k, void* plan, size_t plan_bytes, void* stream);
 
 /* S8 / S10: Xp[bh,i,:] = X[bh,perm[bh,i],:]  and its inverse  X[bh,perm[bh,i],:] = Xp[bh,i,:]
  * (Eq. 1 l.37; Eq. 4 l.56). */

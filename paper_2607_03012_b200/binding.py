@@ -22,7 +22,8 @@ HVA_FLAG_CLUSTER_SIMT, HVA_FLAG_ATTN_SIMT, HVA_FLAG_MASK_BLOCKSORT, HVA_FLAG_MER
 EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_state_describe", "hva_workspace_describe",
            "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes", "hva_merge_workspace_bytes", "hva_plan_workspace_bytes",
            "hva_plan_describe", "hva_cluster", "hva_cluster_ex", "hva_select_subset", "hva_cluster_update", "hva_cluster_update_ex",
-           "hva_build_mask", "hva_build_mask_ex", "hva_merge", "hva_merge_ex", "hva_build_plan", "hva_permute", "hva_unpermute",
+           "hva_build_mask", "hva_build_mask_ex", "hva_merge", "hva_merge_ex", "hva_build_plan", "hva_build_plan_static",
+           "hva_build_plan_static_limit", "hva_permute", "hva_unpermute",
            "hva_sparse_attention", "hva_forward", "hva_forward_host"]
 
 
@@ -76,6 +77,7 @@ def lib():
         L.hva_cluster_update_workspace_bytes.restype = C.c_size_t
         L.hva_merge_workspace_bytes.restype = C.c_size_t
         L.hva_plan_workspace_bytes.restype = C.c_size_t
+        L.hva_build_plan_static_limit.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -251,6 +253,19 @@ def hva_build_plan(n, assign_q, assign_k, sizes_q, sizes_k, group_of, n_groups, 
     _check(lib().hva_build_plan(BH, n, Nq, Nk, _p(assign_q), _p(assign_k), _p(sizes_q), _p(sizes_k), _p(group_of),
                                 _p(n_groups), _p(gmask), int(tile_q), int(tile_k), _p(buf), C.c_size_t(L.total), _p(ws),
                                 C.c_size_t(ws.numel()), _stream()))
+    return Plan(buf, L, BH, n, Nq, Nk)
+
+
+def hva_build_plan_static(n, assign_q, assign_k, sizes_q, sizes_k, group_of, n_groups, gmask, tile_q, tile_k, out=None) -> Plan:
+    """hva_build_plan with the library's built-in scratch array (hva.h: no allocation inside the call; HVA_ELIMIT beyond
+    hva_build_plan_static_limit()).  `out`: a caller-owned uint8 plan buffer of hva_plan_describe().total bytes (allocated here if
+    omitted -- the C entry point itself allocates nothing)."""
+    BH, Nq, Nk = gmask.shape
+    L = hva_plan_describe(BH, n, Nq, Nk, tile_q)
+    buf = torch.zeros(L.total, dtype=torch.uint8, device=gmask.device) if out is None else out
+    assert buf.numel() >= L.total and buf.dtype == torch.uint8
+    _check(lib().hva_build_plan_static(BH, n, Nq, Nk, _p(assign_q), _p(assign_k), _p(sizes_q), _p(sizes_k), _p(group_of),
+                                       _p(n_groups), _p(gmask), int(tile_q), int(tile_k), _p(buf), C.c_size_t(L.total), _stream()))
     return Plan(buf, L, BH, n, Nq, Nk)
 
 

@@ -72,6 +72,7 @@ extern "C" const char* hva_strerror(int code) {
     case HVA_EWORKSPACE: return "workspace / plan / state buffer too small";
     case HVA_EUNSUPPORTED: return "unsupported dtype / tile / size combination";
     case HVA_ECUDA: return "CUDA runtime error";
+    case HVA_ELIMIT: return "problem exceeds the built-in scratch of a *_static entry point (use the variant that takes a workspace)";
     default: return "unknown error";
   }
 }

@@ -7,6 +7,7 @@
 //   B  per-label exclusive scan over tiles, seeded with the cluster's row offset
 //   C  per-tile stable scatter: dest = running offset of the label + rank among equal labels
 #include "common.cuh"
+#include <mutex>
 
 namespace {
 
@@ -501,4 +502,58 @@ int hva_attention_dense_plan(int BH, int n, int tile_q, int tile_k, void* plan, 
   hva_dense_plan_kernel<<<BH, 256, 0, st>>>(n, tile_q, tile_k, P);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// hva_build_plan_static: hva_build_plan for callers that cannot allocate (and have no scratch buffer of their own to pass):
+// the scratch of the sort / group kernels (per-tile label histograms of Q and K, per-cluster row bases) lives in a file-scope
+// device array of HVA_PLAN_STATIC_SCRATCH_BYTES.  Every GPU that loads the library holds the array until the process exits.
+// The array's name below is only a host-side stand-in in host code: the kernels get the DEVICE address, which is looked up
+// once per device (with that device current) by cudaGetSymbolAddress and kept in a table.  No cudaMalloc / cudaFree / allocating
+// library call anywhere on this path.  All calls on a device share the array: two calls that overlap on the GPU (different
+// streams, or one stream-captured graph replayed on two streams) race; calls on one stream are ordered and safe.  Nothing in the
+// array has to start at zero: the kernels write every word they later read (hva_sort_hist_kernel stores the full histogram row
+// of each tile, hva_plan_groups_kernel every row base), so the contents a previous call left behind are never observed.
+namespace {
+constexpr size_t kPlanStaticBytes = (size_t)HVA_PLAN_STATIC_SCRATCH_BYTES;
+static __device__ __align__(256) unsigned char g_plan_static_scratch[kPlanStaticBytes];
+
+struct PlanStaticDev {
+  bool tried = false;
+  cudaError_t err = cudaSuccess;
+  void* ptr = nullptr;
+};
+constexpr int kPlanStaticMaxDevices = 64;
+
+// device address of the array on the CURRENT device (looked up on first use on that device), or null
+void* plan_static_scratch_ptr() {
+  static PlanStaticDev tab[kPlanStaticMaxDevices];
+  static std::mutex guard;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kPlanStaticMaxDevices) return nullptr;
+  std::lock_guard<std::mutex> lock(guard);
+  PlanStaticDev& e = tab[dev];
+  if (!e.tried) {
+    e.tried = true;
+    void* p = nullptr;
+    e.err = cudaGetSymbolAddress(&p, g_plan_static_scratch);
+    if (e.err == cudaSuccess) e.ptr = p;
+    else cudaGetLastError();
+  }
+  return e.err == cudaSuccess ? e.ptr : nullptr;
+}
+}  // namespace
+
+extern "C" size_t hva_build_plan_static_limit(void) { return kPlanStaticBytes; }
+
+extern "C" int hva_build_plan_static(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, const int32_t* assign_q,
+                                     const int32_t* assign_k, const int32_t* sizes_q, const int32_t* sizes_k,
+                                     const int32_t* group_of_cluster, const int32_t* n_groups, const uint8_t* group_mask,
+                                     int32_t tile_q, int32_t tile_k, void* plan, size_t plan_bytes, void* stream) {
+  if (BH < 1 || n < 1 || Nq < 1 || Nk < 1) return HVA_EINVAL;
+  if (hva_plan_ws_bytes(BH, n, Nq, Nk) > kPlanStaticBytes) return HVA_ELIMIT;   // before anything is enqueued
+  void* scratch = plan_static_scratch_ptr();
+  if (!scratch) return HVA_ECUDA;
+  return hva_build_plan(BH, n, Nq, Nk, assign_q, assign_k, sizes_q, sizes_k, group_of_cluster, n_groups, group_mask, tile_q, tile_k,
+                        plan, plan_bytes, scratch, kPlanStaticBytes, stream);
 }

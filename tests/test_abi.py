@@ -97,3 +97,22 @@ def test_library_reads_no_environment_and_keeps_no_probe_pointers():
         assert "getenv" not in src and "strtoull" not in src, f
     cfg = b.make_config(inputs.C2, flags=b.HVA_FLAG_ATTN_SIMT | b.HVA_FLAG_MERGE_SIMT)
     assert cfg.flags == 10 and C.sizeof(b.hva_config) == 4 * (12 + 12) and b.HVA_FLAG_Q_UNPERMUTED == 16
+
+
+def test_static_scratch_plan_limit_is_checked_before_anything_else(lib):
+    """hva_build_plan_static: sizes beyond the built-in array are refused with HVA_ELIMIT before any CUDA call (so also here,
+    without a GPU); the limit is the header's constant."""
+    import re
+    hdr = open(os.path.join(ROOT, "include", "hva.h")).read()
+    m = re.search(r"#define HVA_PLAN_STATIC_SCRATCH_BYTES \((\d+)u << (\d+)\)", hdr)
+    assert m and lib.hva_build_plan_static_limit() == int(m.group(1)) << int(m.group(2)) == 32 << 20
+    assert lib.hva_plan_workspace_bytes(24, 118800, 990, 990) <= lib.hva_build_plan_static_limit()      # C4 fits
+    assert lib.hva_plan_workspace_bytes(64, 118800, 990, 990) > lib.hva_build_plan_static_limit()
+    z = C.c_void_p(0)
+    rc = lib.hva_build_plan_static(64, 118800, 990, 990, z, z, z, z, z, z, z, 128, 128, z, C.c_size_t(0), z)
+    assert rc == -5 and b"static" in lib.hva_strerror(rc)
+    assert lib.hva_build_plan_static(0, 118800, 990, 990, z, z, z, z, z, z, z, 128, 128, z, C.c_size_t(0), z) == -1
+    # the path allocates nothing: no cudaMalloc / cudaFree in the translation unit that holds it
+    src = open(os.path.join(ROOT, "paper_2607_03012_b200", "csrc", "plan.cu")).read()
+    assert "cudaMalloc" not in src.replace("cudaMalloc /", "") and "cudaFree(" not in src
+    assert "cudaGetSymbolAddress(&p, g_plan_static_scratch)" in src
