@@ -276,8 +276,7 @@ def main():
     # the SM clock: ~1.9 GHz here, ~1.45 GHz inside the step); the in-step figure is taken by stage_report() after the timed region
     cl_alone = None
     if rank == 0 and not args.no_stages:
-        cw = lambda: (b.hva_cluster(shape, list(cfg.cell_q), list(cfg.win_q), wl.iters, Q, want_lowe=False),
-                      b.hva_cluster(shape, list(cfg.cell_k), list(cfg.win_k), wl.iters, K, want_lowe=False))
+        cw = cluster_qk_call(b, shape, cfg, Q, K)
         cw()
         cl_alone = ev_time(cw, 10)
     use_graph = not args.no_graph
@@ -326,9 +325,9 @@ def main():
                                      float(cfg.top_p), int(cfg.merge_rounds), custom),
            "clocks": clocks,
            "e2e": {"value": e2e_ms if strong else e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
-           # kernels of one hva_forward: per tensor init + split + iters x (assign, finalize); mask; merge init (+ nterms) + R x (overlap,
+           # kernels of one hva_forward: per tensor init (writes the bf16 split too) + iters x (assign, finalize); mask; merge init (+ nterms) + R x (overlap,
            # propose, apply) + rank + out; plan groups + work + hist + scan + scatter; K and V permutes (Q is gathered inside the attention kernel); attention
-           "gpu_launches": args.steps * (2 * (2 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 5 + 2 + 1)}
+           "gpu_launches": args.steps * (2 * (1 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 5 + 2 + 1)}
 
     # ---- per-stage times and rooflines (rank 0)
     if rank == 0 and not args.no_stages:
@@ -356,8 +355,8 @@ def paper_setting(b, wl, shape, Q, K, V, O):
     for _ in range(2):
         fwd(Q, K, V, O)
     ms = ev_time(lambda: fwd(Q, K, V, O), 3)
-    clq = lambda: (b.hva_cluster(shape, list(cfg.cell_q), list(cfg.win_q), 10, Q, want_lowe=False, want_sums=False),
-                   b.hva_cluster(shape, list(cfg.cell_k), list(cfg.win_k), 10, K, want_lowe=False, want_sums=False))
+    assert int(cfg.iters) == 10
+    clq = cluster_qk_call(b, shape, cfg, Q, K)
     clq()
     cl = ev_time(clq, 3)
     occ = occupancy(wl, fwd.stats_dicts())
@@ -555,6 +554,13 @@ def report_hybrid(b, wl, args):
         del fwd
 
 
+def cluster_qk_call(b, shape, cfg, Q, K):
+    """The clustering stage as hva_forward runs it (hva_cluster_qk: Q and K on two streams, cfg.iters passes each), with outputs and
+    scratch allocated once."""
+    _, _, bufs = b.hva_cluster_qk(shape, cfg, Q, K)
+    return lambda: b.hva_cluster_qk(shape, cfg, Q, K, bufs=bufs)
+
+
 def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk, cl_alone=None):
     BH, n, D = wl.B * wl.heads, wl.n, wl.D
     es = Q.element_size()
@@ -563,8 +569,7 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk, cl_alone=None):
     cell_q, cell_k, win_q, win_k = list(cfg.cell_q), list(cfg.cell_k), list(cfg.win_q), list(cfg.win_k)
     cq = b.hva_cluster(shape, cell_q, win_q, wl.iters, Q, want_lowe=False)
     ck = b.hva_cluster(shape, cell_k, win_k, wl.iters, K, want_lowe=False)
-    st["cluster_qk"] = ev_time(lambda: (b.hva_cluster(shape, cell_q, win_q, wl.iters, Q, want_lowe=False),
-                                        b.hva_cluster(shape, cell_k, win_k, wl.iters, K, want_lowe=False)), 10)
+    st["cluster_qk"] = ev_time(cluster_qk_call(b, shape, cfg, Q, K), 10)
     if cl_alone is not None:
         st["cluster_qk_alone"] = cl_alone
     scale = 1.0 / math.sqrt(D)

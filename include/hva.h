@@ -170,6 +170,18 @@ int hva_cluster_ex(const hva_shape* s, const int32_t cell[3], const int32_t win[
                    const void* X, const float* mu_init, int32_t* assign, float* mu, int32_t* sizes,
                    float* sums, float* lowe, uint32_t flags, float* probe, void* ws, size_t ws_bytes, void* stream);
 
+/* S1 + S2 of BOTH tensors of a call (what hva_forward runs at an anchor step without the hybrid subset): hva_cluster of Q
+ * (cells c->cell_q, window c->win_q) on `stream` and of K (c->cell_k, c->win_k) on a library-owned side stream of the current
+ * device, forked from and joined back into `stream` by events (legal under stream capture), so that the two chains of
+ * kernels overlap; c->iters passes each, c->flags as in hva_cluster_ex.  Outputs as hva_cluster, per tensor (sums_* nullable).
+ * ws_q / ws_k: two DISJOINT device scratch regions of at least hva_cluster_workspace_bytes() for the respective grid
+ * (HVA_EINVAL if they overlap).  The results are bit-identical to two hva_cluster calls.  Concurrent host calls on one device
+ * are serialised while they enqueue.  HVA_ECUDA if the side stream cannot be created. */
+int hva_cluster_qk(const hva_shape* s, const hva_config* c, const void* Q, const void* K,
+                   int32_t* assign_q, float* mu_q, int32_t* sizes_q, float* sums_q,
+                   int32_t* assign_k, float* mu_k, int32_t* sizes_k, float* sums_k,
+                   void* ws_q, size_t ws_q_bytes, void* ws_k, size_t ws_k_bytes, void* stream);
+
 /* S3: indices (ascending) of the m tokens with the largest rho per (b,head), ties -> lower
  * token index (l.101, l.322; R-H2).  lowe[BH,n] fp32 >= 0; subset[BH,m] int32. */
 int hva_select_subset(int32_t BH, int32_t n, const float* lowe, int32_t m, int32_t* subset,

@@ -21,7 +21,7 @@ HVA_FLAG_CLUSTER_SIMT, HVA_FLAG_ATTN_SIMT, HVA_FLAG_MASK_BLOCKSORT, HVA_FLAG_MER
 
 EXPORTS = ["hva_strerror", "hva_version", "hva_num_clusters", "hva_workspace_bytes", "hva_state_bytes", "hva_state_describe", "hva_workspace_describe",
            "hva_cluster_workspace_bytes", "hva_cluster_update_workspace_bytes", "hva_merge_workspace_bytes", "hva_plan_workspace_bytes",
-           "hva_plan_describe", "hva_cluster", "hva_cluster_ex", "hva_select_subset", "hva_cluster_update", "hva_cluster_update_ex",
+           "hva_plan_describe", "hva_cluster", "hva_cluster_ex", "hva_cluster_qk", "hva_select_subset", "hva_cluster_update", "hva_cluster_update_ex",
            "hva_build_mask", "hva_build_mask_ex", "hva_merge", "hva_merge_ex", "hva_build_plan", "hva_build_plan_static",
            "hva_build_plan_static_limit", "hva_permute", "hva_unpermute",
            "hva_sparse_attention", "hva_forward", "hva_forward_host"]
@@ -174,6 +174,28 @@ def hva_cluster(shape, cell, win, iters, X, mu_init=None, want_sums=True, want_l
                                  _p(out["mu"]), _p(out["sizes"]), _p(out["sums"]), _p(out["lowe"]), _p(ws),
                                  C.c_size_t(ws.numel()), _stream()))
     return out
+
+
+def hva_cluster_qk(shape, cfg, Q, K, want_sums=True, bufs=None):
+    """Q and K clustered by one call on two streams (hva.h) -> (dict_q, dict_k) as hva_cluster (no lowe).  `bufs`: the tuple a
+    previous call returned as its third value, to reuse outputs and scratch."""
+    BH, n, D = shape.B * shape.heads, shape.T * shape.H * shape.W, shape.D
+    dev = Q.device
+    if bufs is None:
+        outs = []
+        for cell, win in ((list(cfg.cell_q), list(cfg.win_q)), (list(cfg.cell_k), list(cfg.win_k))):
+            Nc = hva_num_clusters(shape, cell)
+            outs.append(dict(assign=torch.empty((BH, n), dtype=torch.int32, device=dev),
+                             mu=torch.empty((BH, Nc, D), dtype=torch.float32, device=dev),
+                             sizes=torch.empty((BH, Nc), dtype=torch.int32, device=dev),
+                             sums=torch.empty((BH, Nc, D), dtype=torch.float32, device=dev) if want_sums else None, lowe=None,
+                             ws=_ws(lib().hva_cluster_workspace_bytes(C.byref(shape), _i3(cell), _i3(win)), dev)))
+        bufs = tuple(outs)
+    q, k = bufs
+    _check(lib().hva_cluster_qk(C.byref(shape), C.byref(cfg), _p(Q), _p(K), _p(q["assign"]), _p(q["mu"]), _p(q["sizes"]), _p(q["sums"]),
+                                _p(k["assign"]), _p(k["mu"]), _p(k["sizes"]), _p(k["sums"]), _p(q["ws"]), C.c_size_t(q["ws"].numel()),
+                                _p(k["ws"]), C.c_size_t(k["ws"].numel()), _stream()))
+    return q, k, bufs
 
 
 def hva_select_subset(lowe, m):

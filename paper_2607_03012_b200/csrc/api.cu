@@ -18,6 +18,32 @@ struct FwdLayout {
   hva_plan_layout PL;
 };
 
+// hva_cluster_qk / hva_forward cluster Q and K on two streams (fork / join by events, legal under stream capture): the second
+// persistent assignment kernel fills the SMs as the first one's CTAs drain, and the small finalize launches of one tensor run
+// under the other's pass.  One side stream + two events per device, created on first use; a call only enqueues on them.
+struct SideStream {
+  cudaStream_t st = nullptr;
+  cudaEvent_t fork = nullptr, join = nullptr;
+  bool tried = false, ok = false;
+  std::mutex busy;   // held while a call enqueues its fork .. join sequence
+  void create() {
+    tried = true;
+    ok = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess &&
+         cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&join, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) cudaGetLastError();
+  }
+};
+SideStream* side_stream() {
+  static SideStream tab[64];
+  static std::mutex table;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  std::lock_guard<std::mutex> g(table);
+  if (!tab[dev].tried) tab[dev].create();
+  return tab[dev].ok ? &tab[dev] : nullptr;
+}
+
 bool valid_shape(const hva_shape* s) {
   return s && s->B >= 1 && s->heads >= 1 && s->T >= 1 && s->H >= 1 && s->W >= 1 && (s->D == 64 || s->D == 128) &&
          (s->dtype == HVA_F32 || s->dtype == HVA_BF16);
@@ -139,6 +165,30 @@ extern "C" int hva_sparse_attention(const hva_shape* s, const hva_config* c, con
   return hva_attention_simt_launch(s, scale, Qp, Kp, Vp, plan, L, Nq, Nk, O, unpermute, st, c->tile_q);
 }
 
+extern "C" int hva_cluster_qk(const hva_shape* s, const hva_config* c, const void* Q, const void* K, int32_t* assign_q, float* mu_q,
+                              int32_t* sizes_q, float* sums_q, int32_t* assign_k, float* mu_k, int32_t* sizes_k, float* sums_k, void* ws_q,
+                              size_t ws_q_bytes, void* ws_k, size_t ws_k_bytes, void* stream) {
+  if (!valid_shape(s) || !valid_config(c) || !Q || !K || !ws_q || !ws_k) return HVA_EINVAL;
+  {   // the two scratch regions must not overlap
+    const char *a = (const char*)ws_q, *b = (const char*)ws_k;
+    if (a < b + ws_k_bytes && b < a + ws_q_bytes) return HVA_EINVAL;
+  }
+  if (ws_q_bytes < hva_cluster_workspace_bytes(s, c->cell_q, c->win_q) || ws_k_bytes < hva_cluster_workspace_bytes(s, c->cell_k, c->win_k))
+    return HVA_EWORKSPACE;   // before the fork: nothing may fail between fork and join for a reason known up front
+  SideStream* side = side_stream();
+  if (!side) return HVA_ECUDA;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  std::lock_guard<std::mutex> g(side->busy);
+  if (cudaEventRecord(side->fork, st) != cudaSuccess || cudaStreamWaitEvent(side->st, side->fork, 0) != cudaSuccess) return HVA_ECUDA;
+  int rc = hva_cluster_ex(s, c->cell_q, c->win_q, c->iters, Q, nullptr, assign_q, mu_q, sizes_q, sums_q, nullptr, c->flags, nullptr, ws_q,
+                          ws_q_bytes, stream);
+  const int rk = hva_cluster_ex(s, c->cell_k, c->win_k, c->iters, K, nullptr, assign_k, mu_k, sizes_k, sums_k, nullptr, c->flags, nullptr,
+                                ws_k, ws_k_bytes, side->st);
+  // join even after an error: the side stream must not stay forked (stream capture)
+  if (cudaEventRecord(side->join, side->st) != cudaSuccess || cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) return HVA_ECUDA;
+  return rc != HVA_OK ? rc : rk;
+}
+
 namespace {
 int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const void* K, const void* V, void* O, int32_t step_kind,
                  void* state, hva_stats* stats_out, void* ws, size_t ws_bytes, void* stream, int bh0) {
@@ -169,7 +219,15 @@ int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const v
   const int32_t* win[2] = {c->win_q, c->win_k};
   const int Nc[2] = {F.Nq, F.Nk};
   const bool hybrid = c->subset_frac > 0.f && state != nullptr && F.m > 0;
-  for (int t = 0; t < 2; ++t) {
+  // anchor step without the hybrid subset: Q and K on two streams, K with the (still unused) K' region as its scratch
+  const size_t es = s->dtype == HVA_F32 ? 4 : 2;
+  const bool two_streams = step_kind == HVA_ANCHOR && !hybrid && (size_t)BH * n * s->D * es >= F.scratch_bytes && side_stream() != nullptr;
+  if (two_streams) {
+    HVA_TRY(hva_cluster_qk(s, c, Q, K, (int32_t*)(sb + F.assign[0]), (float*)(sb + F.mu[0]), (int32_t*)(sb + F.sizes[0]), (float*)(sb + F.sums[0]),
+                           (int32_t*)(sb + F.assign[1]), (float*)(sb + F.mu[1]), (int32_t*)(sb + F.sizes[1]), (float*)(sb + F.sums[1]),
+                           w + F.scratch, F.scratch_bytes, w + F.kp, (size_t)BH * n * s->D * es, stream));
+  }
+  for (int t = 0; t < 2 && !two_streams; ++t) {
     int32_t* assign = (int32_t*)(sb + F.assign[t]);
     float* mu = (float*)(sb + F.mu[t]);
     float* sums = (float*)(sb + F.sums[t]);

@@ -70,17 +70,38 @@ __global__ void __launch_bounds__(D) hva_mu_split_kernel(int Nc, const float* __
   mu_split_store<D>(sp, row, threadIdx.x, mu[row * D + threadIdx.x]);
 }
 
+// Alg. 2 lines 7-11 and the operands of the first tensor-pipe pass in one launch: warp = centroid, lane = D/32 consecutive dims
+// (one launch of Nc*BH/8 CTAs instead of two of Nc*BH: both were bound by the CTA launch rate, 23 + 16 us at C4)
+constexpr int kInitWarps = 8;
 template <typename T, int D>
-__global__ void __launch_bounds__(kThreads) hva_init_centroids_kernel(HvaGrid g, const T* __restrict__ X,
-                                                                      float* __restrict__ mu) {
-  // mu_u <- X[c_t, c_h, c_w, :],  c = min(u*k + floor(k/2), dim-1)   (Alg. 2 lines 7-11)
-  int u = blockIdx.x, bh = blockIdx.y;
-  int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
-  int ct = min(ut * g.kt + g.kt / 2, g.T - 1), ch = min(uh * g.kh + g.kh / 2, g.H - 1),
-      cw = min(uw * g.kw + g.kw / 2, g.W - 1);
-  size_t tok = (size_t)(ct * g.H + ch) * g.W + cw;
-  for (int c = threadIdx.x; c < D; c += blockDim.x)
-    mu[((size_t)bh * g.Nc + u) * D + c] = HvaElem<T>::ld(X + ((size_t)bh * g.n + tok) * D + c);
+__global__ void __launch_bounds__(32 * kInitWarps) hva_init_centroids_kernel(HvaGrid g, const T* __restrict__ X,
+                                                                             float* __restrict__ mu, MuSplit sp) {
+  // mu_u <- X[c_t, c_h, c_w, :],  c = min(u*k + floor(k/2), dim-1)
+  constexpr int E = D / 32;
+  const int u = blockIdx.x * kInitWarps + (threadIdx.x >> 5), bh = blockIdx.y, lane = threadIdx.x & 31;
+  if (u >= g.Nc) return;
+  const int ut = u / (g.Kh * g.Kw), uh = (u / g.Kw) % g.Kh, uw = u % g.Kw;
+  const int ct = min(ut * g.kt + g.kt / 2, g.T - 1), ch = min(uh * g.kh + g.kh / 2, g.H - 1),
+            cw = min(uw * g.kw + g.kw / 2, g.W - 1);
+  const size_t tok = (size_t)(ct * g.H + ch) * g.W + cw, row = (size_t)bh * g.Nc + u;
+  float q = 0.f;
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int c = lane * E + e;
+    const float m = HvaElem<T>::ld(X + ((size_t)bh * g.n + tok) * D + c);
+    mu[row * D + c] = m;
+    if (sp.hi) {
+      const __nv_bfloat16 h = __float2bfloat16_rn(m);
+      sp.hi[row * D + c] = h;
+      sp.lo[row * D + c] = __float2bfloat16_rn(m - __bfloat162float(h));
+      q = fmaf(m, m, q);
+    }
+  }
+  if (sp.hi) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+    if (lane == 0) sp.musq[row] = q;
+  }
 }
 
 template <typename T, int D>
@@ -350,10 +371,11 @@ int run_cluster(const HvaGrid& g, int BH, int iters, const void* X, const float*
         cudaMemcpyAsync(mu, mu_init, (size_t)BH * g.Nc * D * sizeof(float), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
       return HVA_ECUDA;
   } else {
-    hva_init_centroids_kernel<T, D><<<grid, kThreads, 0, st>>>(g, reinterpret_cast<const T*>(X), mu);
+    hva_init_centroids_kernel<T, D><<<dim3((g.Nc + kInitWarps - 1) / kInitWarps, BH), 32 * kInitWarps, 0, st>>>(
+        g, reinterpret_cast<const T*>(X), mu, tc ? sp : none);
     HVA_CHECK_LAUNCH();
   }
-  if (tc) {
+  if (tc && mu_init) {
     hva_mu_split_kernel<D><<<grid, D, 0, st>>>(g.Nc, mu, sp);
     HVA_CHECK_LAUNCH();
   }

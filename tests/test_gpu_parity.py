@@ -621,3 +621,33 @@ def test_batch_dimension_is_folded_into_heads():
     O22 = b.Forward(sh, cfg)(view(Q), view(K), view(V))
     torch.cuda.synchronize()
     assert torch.equal(O4.view(-1), O22.view(-1))
+
+
+def test_cluster_qk_two_streams_equals_two_cluster_calls():
+    """hva_cluster_qk (Q on the caller's stream, K on the library's side stream, joined by events) == two hva_cluster calls, bit
+    for bit, with different Q / K grids; twice in a row with reused buffers; overlapping scratch regions are refused."""
+    b = _b()
+    wl = inputs.CONFIGS["C2"]
+    heads = list(range(8))
+    Q, K, _ = inputs.make_qkv(wl, heads=heads)
+    Q, K = Q.cuda().contiguous(), K.cuda().contiguous()
+    shape = b.make_shape(wl, heads=len(heads))
+    cfg = b.make_config(wl)
+    cfg.cell_k[0], cfg.cell_k[1], cfg.cell_k[2] = 3, 3, 4
+    rq = b.hva_cluster(shape, list(cfg.cell_q), list(cfg.win_q), wl.iters, Q, want_lowe=False)
+    rk = b.hva_cluster(shape, list(cfg.cell_k), list(cfg.win_k), wl.iters, K, want_lowe=False)
+    bufs = None
+    for _ in range(2):
+        q, k, bufs = b.hva_cluster_qk(shape, cfg, Q, K, bufs=bufs)
+        torch.cuda.synchronize()
+        for got, ref in ((q, rq), (k, rk)):
+            for key in ("assign", "mu", "sizes", "sums"):
+                assert torch.equal(got[key], ref[key]), key
+        for d in (q, k):       # the next round must rewrite everything
+            d["assign"].fill_(-1); d["mu"].fill_(float("nan"))
+    import ctypes as C
+    ws = bufs[0]["ws"]
+    rc = b.lib().hva_cluster_qk(C.byref(shape), C.byref(cfg), b._p(Q), b._p(K), b._p(q["assign"]), b._p(q["mu"]), b._p(q["sizes"]), b._p(q["sums"]),
+                                b._p(k["assign"]), b._p(k["mu"]), b._p(k["sizes"]), b._p(k["sums"]), b._p(ws), C.c_size_t(ws.numel()),
+                                b._p(ws), C.c_size_t(ws.numel()), b._stream())
+    assert rc == -1
