@@ -70,6 +70,7 @@ struct AssignTcParams {
                        // TMEM columns and tables only after the epilogue
   int cols;            // TMEM columns per token slot
   int one_pass;        // 2 npad <= 256: one MMA pass over [hi; lo] stacked as 2 npad score columns (the token tile is read once)
+  int coop;            // cooperative scan: every tile is scanned by all three groups, each taking a share of the window's 32-candidate chunks
   unsigned long long d_khw, d_kw, d_cs, d_kt;   // fast_div64 multipliers of the tile decode: K_h K_w, K_w, csplit, K_t
   int n_items;         // K_w * K_h * K_t * BH * csplit tiles: CTA b takes tiles b, b + gridDim.x, ...
   float* probe;        // instrumented instantiation: max |score_tc - score_exact| / (|x| max|mu|)
@@ -122,9 +123,16 @@ __device__ __forceinline__ int fast_div(int x, uint32_t m) { return m ? (int)__u
 // m d = 2^64 + e with e < d, so x m / 2^64 = x / d + x e / (d 2^64), and the excess is below 2^-32 < 1 / d
 __device__ __forceinline__ int fast_div64(int x, unsigned long long m) { return m ? (int)__umul64hi((unsigned long long)(uint32_t)x, m) : x; }
 
+__device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
 // kProbe = true is the instrumented instantiation behind hva_cluster_ex(probe != NULL) (tests: observed filter error);
 // the product instantiation carries none of that code.
-template <bool kProbe>
+// kVar selects a specialisation of the scan code: 0 = everything decided at run time (and the only one that carries the
+// cooperative wide-window scan); 1 = windows of at most 32 candidates, one MMA pass, labels only; 2 = the same with the Lowe
+// ratio.  The instrumented instantiation is generic.  (The 27-candidate path is sensitive to what is compiled next to it: a
+// score more instructions on its rare refine branch cost 7 %.)
+template <bool kProbe, int kVar>
 __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid_constant__ CUtensorMap map_x,
                                                                  const __grid_constant__ CUtensorMap map_hi,
                                                                  const __grid_constant__ CUtensorMap map_lo, AssignTcParams p) {
@@ -133,6 +141,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
   const int ctok = p.ct * g.kh * g.kw, nwin = g.nwin, npad = p.npad;   // token rows of a tile
   const int half_a = p.rows_a * 128, half_b = npad * 128;
   const int NT = p.NT, NB = p.NB, NW = p.NW, NS = p.NS;
+  const bool one_pass = kVar ? true : (bool)p.one_pass;
 
   // Shared memory (offsets from a 1024-byte aligned base):
   //   sA  [NT][2 halves][rows_a][128 B]           token slots (A of MMA 1, K-major SW128; A of MMA 2, MN-major)
@@ -152,6 +161,10 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
   int* s_cnt_all = reinterpret_cast<int*>(s_c_all + NS * npad);
   uint16_t* s_u_all = reinterpret_cast<uint16_t*>(s_cnt_all + NS * npad);
   AssignTcShared* SH = reinterpret_cast<AssignTcShared*>(reinterpret_cast<unsigned char*>(s_u_all + NS * npad) + ((8 - ((NS * npad * 2) & 7)) & 7));
+
+  // cooperative scan only: (s1, s2) of every group and row, two parities; contender word of every chunk and row
+  float2* coop_ex = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(SH + 1) + ((16 - (sizeof(AssignTcShared) & 15)) & 15));
+  uint32_t* coop_m = reinterpret_cast<uint32_t*>(coop_ex + 2 * 3 * 128);
 
   if (warp == kLoadWarp) tmem_alloc(&SH->tmem_base, kTmemCols);
 
@@ -266,7 +279,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
     CFLUSH(2);
   } else if (warp == kMma1Warp) {
     // ================================================================ MMA 1 (scores) as soon as a tile's boxes have landed
-    const uint32_t idesc1 = umma_idesc_bf16(128, (uint32_t)(p.one_pass ? 2 * npad : npad), 0, 0);
+    const uint32_t idesc1 = umma_idesc_bf16(128, (uint32_t)(one_pass ? 2 * npad : npad), 0, 0);
     const uint32_t ha = (uint32_t)half_a >> 4, hb2 = (uint32_t)(2 * half_b) >> 4;
     int i = 0, jb = 0, ia = 0;
     uint32_t par = 0;
@@ -288,7 +301,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 #pragma unroll
         for (int ks = 0; ks < kD / 16; ++ks)
           mma_ss(d_t, da + ((ks >> 2) * ha + (ks & 3) * 2), dhi + ((ks >> 2) * hb2 + (ks & 3) * 2), idesc1, ks > 0);
-        if (!p.one_pass) {
+        if (!one_pass) {
 #pragma unroll
           for (int ks = 0; ks < kD / 16; ++ks)
             mma_ss(d_t, da + ((ks >> 2) * ha + (ks & 3) * 2), dlo + ((ks >> 2) * hb2 + (ks & 3) * 2), idesc1, 1);
@@ -426,16 +439,30 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
   } else {
     // ================================================================ scan groups: thread = token row of the tile == TMEM lane
     asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
-    if (warp < 4 * NW) {
-    const int w = warp >> 2;                 // group: tiles q = w, w + NW, ...
+    // Cooperative scan (wide windows: shared memory holds ONE one-hot tile, so one tile at a time is in the scan stage): all three
+    // groups work on every tile, group w on its share of the window's 32-candidate chunks; they exchange their two smallest scores,
+    // mark the contenders of their chunks against the common threshold, and group 0 decides, stores and writes the one-hot tile.
+    const bool coop = kVar == 0 && p.coop != 0;
+    if (warp < 4 * NW || coop) {
+    const int w = warp >> 2;                 // group: tiles q = w, w + NW, ... (cooperative: every tile)
+    const int step = coop ? 1 : NW;
+    const int nchunk = (nwin + 31) >> 5;
+    int c_lo = 0, c_hi = nchunk;             // chunks of this group
+    if (coop) {                              // group 0 also runs the decision part of every tile: the smallest share
+      const int n0 = max(1, nchunk >> 2), n1 = (nchunk - n0) >> 1;
+      c_lo = w == 0 ? 0 : (w == 1 ? n0 : n0 + n1);
+      c_hi = w == 0 ? n0 : (w == 1 ? n0 + n1 : nchunk);
+    }
+    const int v_lo = 32 * c_lo, v_hi = min(nwin, 32 * c_hi);
+    uint32_t tpar = 0;                       // parity of the exchange buffer (cooperative scan)
     const int li = tid & 127;
     const int ldt = fast_div(li, p.m_khw), lr = li - ldt * g.kh * g.kw, ldh = fast_div(lr, p.m_kw), ldw = lr - ldh * g.kw;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-    const bool want2 = p.lowe != nullptr;
-    const bool single_chunk = nwin <= 32;
-    unsigned char* sP = sP_all + (size_t)w * 2 * half_b;
+    const bool want2 = kVar ? kVar == 2 : p.lowe != nullptr;
+    const bool single_chunk = kVar ? true : nwin <= 32;
+    unsigned char* sP = sP_all + (size_t)(coop ? 0 : w) * 2 * half_b;
     uint32_t prev_p = 0;      // shared-space address of the one-hot element set for the group's previous tile (0: none)
-    int i = w, pi = 0, ia = w;               // slot of the group's tile / of its previous tile, token buffer (NW < NT <= NS)
+    int i = coop ? 0 : w, pi = 0, ia = i;    // slot of the group's tile / of its previous tile, token buffer (NW < NT <= NS)
     uint32_t par = 0, ppar = 0;
     for (bool first_tile = true;; first_tile = false) {
       TileSlot* S = &SH->slot[i];
@@ -494,7 +521,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 #pragma unroll
           for (int j = 0; j < 4; ++j) xsq += __low2float(acc[j]) + __high2float(acc[j]);
           xsq *= 1.125f;
-          if (p.xsq_mode == 1) p.xsq[tok] = xsq;
+          if (p.xsq_mode == 1 && (!coop || w == 0)) p.xsq[tok] = xsq;
         }
       }
       CMARK(2);
@@ -514,7 +541,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 #pragma unroll
         for (int h = 0; h < 32; h += 16) {
           uint32_t raw[16], rlo[16];
-          if (p.one_pass) {      // x.hi in columns [0, npad), x.lo in [npad, 2 npad)
+          if (one_pass) {      // x.hi in columns [0, npad), x.lo in [npad, 2 npad)
             tmem_ld16_nowait(trow + v0 + h, raw);
             tmem_ld16_nowait(trow + npad + v0 + h, rlo);
             tmem_ld_wait16(raw);
@@ -542,7 +569,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       // pass 1: smallest filter score, and the second smallest when the Lowe ratio is wanted (independent chains, merged);
       // 3-input min keeps the chains short
       float s1 = kInf, s2 = kInf, r1 = kInf, r2 = kInf;
-      for (int v0 = 0; v0 < nwin; v0 += 32) {
+      for (int v0 = v_lo; v0 < v_hi; v0 += 32) {
         load_scores(v0);
         if (want2) {
 #pragma unroll
@@ -562,6 +589,17 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       }
       s2 = fminf(fminf(s2, r2), fmaxf(s1, r1));
       s1 = fminf(s1, r1);
+      if (coop) {       // the two smallest scores of the whole window from the three groups' shares
+        float2* ex = coop_ex + tpar * (3 * 128);
+        ex[w * 128 + li] = make_float2(s1, s2);
+        named_bar_sync(1, 384);
+#pragma unroll
+        for (int k = 1; k < 3; ++k) {
+          const float2 o = ex[(w + k >= 3 ? w + k - 3 : w + k) * 128 + li];
+          s2 = fminf(fminf(s2, o.y), fmaxf(s1, o.x));
+          s1 = fminf(s1, o.x);
+        }
+      }
       const float thr = (want2 ? s2 : s1) + margin;     // s2 = +inf (single candidate): every candidate is a contender
       // pass 2: contenders = candidates with score <= thr.  A single contender (without the Lowe ratio) is the direct-form
       // argmin; otherwise the exact direct form decides among them, ascending candidate id, strict '<'  (R-C1)
@@ -569,7 +607,7 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       const float* mu_b = p.mu + (size_t)bh * g.Nc * kD;
       int n_cont = 0, first = 0;
       uint32_t cand0 = 0;
-      for (int v0 = 0; v0 < nwin; v0 += 32) {
+      for (int v0 = v_lo; v0 < v_hi; v0 += 32) {
         if (!single_chunk) load_scores(v0);
         uint32_t cand = 0, cand_b = 0;
 #pragma unroll
@@ -583,13 +621,34 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
         if (n_cont == 0 && cand) first = v0 + __ffs(cand) - 1;
         n_cont += __popc(cand);
         if (v0 == 0) cand0 = cand;
+        if (coop) coop_m[(v0 >> 5) * 128 + li] = cand;
+      }
+      if (coop) {
+        tc_fence_before();                  // this group's score reads are complete (MMA 2 overwrites the columns after group 0's arrival)
+        __threadfence_block();
+        if (w != 0) {                       // groups 1 and 2 are done with the tile
+          named_bar_arrive(2, 384);
+          i += 1; if (i >= NS) { i = 0; par ^= 1u; }
+          ia += 1; if (ia >= NT) ia = 0;
+          tpar ^= 1u;
+          continue;
+        }
+        named_bar_sync(2, 384);
+        n_cont = 0; first = 0;
+        for (int c = 0; c < nchunk; ++c) {
+          const uint32_t m = coop_m[c * 128 + li];
+          if (n_cont == 0 && m) first = 32 * c + __ffs(m) - 1;
+          n_cont += __popc(m);
+        }
       }
       const bool refine = valid && (want2 || n_cont > 1);
       if (valid && !refine) lab = first;
       if (__any_sync(0xffffffffu, refine)) {            // tcgen05.ld is warp-collective: the chunk loop stays warp-uniform
         for (int v0 = 0; v0 < nwin; v0 += 32) {
           uint32_t cand = cand0;
-          if (!single_chunk) {
+          if (coop) {
+            cand = coop_m[(v0 >> 5) * 128 + li];
+          } else if (!single_chunk) {
             load_scores(v0);
             cand = 0;
 #pragma unroll
@@ -700,10 +759,11 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       tq += NW;
 #endif
       pi = i; ppar = par;
-      i += NW;
+      i += step;
       if (i >= NS) { i -= NS; par ^= 1u; }
-      ia += NW;
+      ia += step;
       if (ia >= NT) ia -= NT;
+      tpar ^= 1u;
     }
     CFLUSH(0);
     }
@@ -714,23 +774,28 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
 }
 
 // shared memory of a configuration (NT token slots, NB centroid buffers, NW one-hot tiles)
-size_t assign_tc_smem(int npad, int rows_a, int NT, int NB, int NW, int NS) {
+// exchange area of the cooperative scan: [2 parities][3 groups][128 rows] (s1, s2) + [8 chunks][128 rows] contender words
+constexpr size_t kCoopBytes = 2 * 3 * 128 * 8 + 8 * 128 * 4;
+size_t assign_tc_smem(int npad, int rows_a, int NT, int NB, int NW, int NS, int coop = 0) {
   const size_t half_a = (size_t)rows_a * 128, half_b = (size_t)npad * 128;
   size_t bytes = (size_t)NT * 2 * half_a + (size_t)NB * 4 * half_b + (size_t)NW * 2 * half_b;
   // MMA 1 reads 128 token rows of its A operand: keep the over-read of the last slot inside the allocation
   bytes = std::max(bytes, (size_t)(NT - 1) * 2 * half_a + half_a + 16384);
   bytes += (size_t)NS * npad * (sizeof(float) + sizeof(int) + sizeof(uint16_t)) + 8 + sizeof(AssignTcShared) + 16;
+  if (coop) bytes += kCoopBytes + 16;
   return bytes + 1024;
 }
 
 // the largest pipeline that fits 227 KB of shared memory and 512 TMEM columns: three scan groups if possible
-bool assign_tc_config(int npad, int rows_a, int cols, int* NT, int* NB, int* NW, int* NS) {
+bool assign_tc_config(int npad, int rows_a, int cols, int* NT, int* NB, int* NW, int* NS, int* coop) {
   const int ns = std::min(kMaxNT, (int)kTmemCols / cols);      // pipeline slots: as many as TMEM holds
   for (int nw = kMaxNW; nw >= 1; --nw)
     for (int nb = 2; nb >= 1; --nb)
       for (int nt = ns; nt >= nw + 1; --nt) {
         if (nt <= nb) continue;
-        if (assign_tc_smem(npad, rows_a, nt, nb, nw, ns) <= 227 * 1024) { *NT = nt; *NB = nb; *NW = nw; *NS = ns; return true; }
+        // one scan group only (wide windows): the two idle groups join in, if the exchange area fits as well
+        const int co = nw == 1 && npad > 32 && assign_tc_smem(npad, rows_a, nt, nb, nw, ns, 1) <= 227 * 1024;
+        if (assign_tc_smem(npad, rows_a, nt, nb, nw, ns, co) <= 227 * 1024) { *NT = nt; *NB = nb; *NW = nw; *NS = ns; *coop = co; return true; }
       }
   return false;
 }
@@ -742,8 +807,8 @@ bool hva_assign_tc_supported(const HvaGrid& g, int D, int dtype) {
         g.kw <= 256 && g.wt <= 256 && g.wh <= 256 && g.ww <= 256))
     return false;
   const int ctok = hva_assign_tc_slices(g) * g.kh * g.kw, npad = (g.nwin + 15) & ~15;
-  int NT, NB, NW, NS;
-  return assign_tc_config(npad, (ctok + 15) & ~15, 2 * npad <= 256 ? 2 * npad : npad, &NT, &NB, &NW, &NS);
+  int NT, NB, NW, NS, coop;
+  return assign_tc_config(npad, (ctok + 15) & ~15, 2 * npad <= 256 ? 2 * npad : npad, &NT, &NB, &NW, &NS, &coop);
 }
 
 namespace {
@@ -763,7 +828,6 @@ bool make_map5(CUtensorMap* m, const void* base, int BH, int d3, int d2, int d1,
 }  // namespace
 
 int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* mu_hi, const void* mu_lo, bool probe, HvaAssignTc* a) {
-  const void* kern = probe ? (const void*)hva_assign_tc_kernel<true> : (const void*)hva_assign_tc_kernel<false>;
   a->probe = probe;
   a->ct = hva_assign_tc_slices(g);
   a->csplit = (g.kt + a->ct - 1) / a->ct;
@@ -772,13 +836,16 @@ int hva_assign_tc_prepare(const HvaGrid& g, int BH, const void* X, const void* m
   a->rows_a = (ctok + 15) & ~15;
   a->one_pass = 2 * a->npad <= 256;
   a->cols = a->one_pass ? 2 * a->npad : a->npad;
-  if (!assign_tc_config(a->npad, a->rows_a, a->cols, &a->NT, &a->NB, &a->NW, &a->NS)) return HVA_EUNSUPPORTED;
-  a->smem = assign_tc_smem(a->npad, a->rows_a, a->NT, a->NB, a->NW, a->NS);
+  if (!assign_tc_config(a->npad, a->rows_a, a->cols, &a->NT, &a->NB, &a->NW, &a->NS, &a->coop)) return HVA_EUNSUPPORTED;
+  a->smem = assign_tc_smem(a->npad, a->rows_a, a->NT, a->NB, a->NW, a->NS, a->coop);
   if ((long long)g.Kw * g.Kh * g.Kt * BH * a->csplit > 0x7fffffffLL) return HVA_EUNSUPPORTED;
   if (!make_map5(&a->map_x, X, BH, g.T, g.H, g.W, a->ct, g.kh, g.kw)) return HVA_ECUDA;
   if (!make_map5(&a->map_hi, mu_hi, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
   if (!make_map5(&a->map_lo, mu_lo, BH, g.Kt, g.Kh, g.Kw, g.wt, g.wh, g.ww)) return HVA_ECUDA;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)a->smem) != cudaSuccess) return HVA_ECUDA;
+  const void* kerns[4] = {(const void*)hva_assign_tc_kernel<true, 0>, (const void*)hva_assign_tc_kernel<false, 0>,
+                          (const void*)hva_assign_tc_kernel<false, 1>, (const void*)hva_assign_tc_kernel<false, 2>};
+  for (int k = probe ? 0 : 1; k < (probe ? 1 : 4); ++k)
+    if (cudaFuncSetAttribute(kerns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)a->smem) != cudaSuccess) return HVA_ECUDA;
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HVA_ECUDA;
   a->grid = sms;         // one persistent CTA per SM
@@ -790,12 +857,16 @@ int hva_assign_tc_launch(const HvaAssignTc& a, const HvaGrid& g, int BH, const f
   auto magic = [](int d) -> uint32_t { return d <= 1 ? 0u : (uint32_t)(((1ull << 32) + d - 1) / d); };
   auto magic64 = [](int d) -> unsigned long long { return d <= 1 ? 0ull : ~0ull / (unsigned long long)d + 1ull; };
   AssignTcParams p{g, mu, musq, part, part_cnt, assign, lowe, xsq, xsq ? xsq_mode : 0, a.npad, a.rows_a, a.csplit, a.ct, magic(g.kh * g.kw),
-                   magic(g.kw), magic(g.wh * g.ww), magic(g.ww), a.NT, a.NB, a.NW, a.NS, a.cols, a.one_pass, magic64(g.Kw * g.Kh), magic64(g.Kw),
+                   magic(g.kw), magic(g.wh * g.ww), magic(g.ww), a.NT, a.NB, a.NW, a.NS, a.cols, a.one_pass, a.coop, magic64(g.Kw * g.Kh), magic64(g.Kw),
                    magic64(a.csplit), magic64(g.Kt), g.Kw * g.Kh * g.Kt * BH * a.csplit, probe};
   (void)counter;
   if (a.probe != (probe != nullptr)) return HVA_EINVAL;
-  if (probe) hva_assign_tc_kernel<true><<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
-  else hva_assign_tc_kernel<false><<<std::min(a.grid, p.n_items), kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  const int grid = std::min(a.grid, p.n_items);
+  const bool special = a.one_pass && g.nwin <= 32;
+  if (probe) hva_assign_tc_kernel<true, 0><<<grid, kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  else if (!special) hva_assign_tc_kernel<false, 0><<<grid, kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  else if (!lowe) hva_assign_tc_kernel<false, 1><<<grid, kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
+  else hva_assign_tc_kernel<false, 2><<<grid, kThreads, a.smem, st>>>(a.map_x, a.map_hi, a.map_lo, p);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }

@@ -10,6 +10,7 @@ struct HvaAssignTc {
   int cols;            // TMEM columns per token slot
   size_t smem;
   int one_pass;        // one MMA pass over the stacked [hi; lo] centroid tile
+  int coop;            // wide windows (shared memory holds one one-hot tile): the three scan groups share every tile's candidates
   int grid;            // one persistent CTA per SM
   bool probe;          // prepared for the instrumented instantiation (hva_cluster_ex with a probe buffer)
 };
