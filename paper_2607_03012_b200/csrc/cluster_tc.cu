@@ -417,11 +417,31 @@ __global__ void __launch_bounds__(kThreads, 1) hva_assign_tc_kernel(const __grid
       float* prow = p.part + pbase * kD + dim;
       const uint32_t trow = tmem + lane_base + (uint32_t)(i * p.cols);
       for (int v0 = 0; v0 < nwin; v0 += 32) {
-        uint32_t raw[32];
-        tmem_ld32(trow + v0, raw);
         // non-empty slots of this chunk as one ballot word: the stores below are then a bit test + STG with an immediate offset
         const unsigned nz = __ballot_sync(0xffffffffu, v0 + lane < nwin && s_cnt[v0 + lane] > 0);
         float* pr = prow + (size_t)v0 * kD;
+        if (kVar == 0 && __popc(nz) <= 16) {
+          // wide windows: most of a chunk's slots are empty, and TMEM reads (64 B per clock and SM) are what the kernel runs out of:
+          // only the non-empty columns are read, four single-column loads in flight
+          unsigned m = nz;
+          while (m) {
+            uint32_t val[4] = {0u, 0u, 0u, 0u};
+            int js[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              js[k] = m ? __ffs(m) - 1 : -1;
+              m &= m - 1;                    // 0 stays 0
+              if (js[k] >= 0) tmem_ld1_nowait(trow + v0 + js[k], val[k]);
+            }
+            tmem_ld_wait4(val);
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              if (js[k] >= 0) pr[js[k] * kD] = __uint_as_float(val[k]);
+          }
+          continue;
+        }
+        uint32_t raw[32];
+        tmem_ld32(trow + v0, raw);
 #pragma unroll
         for (int j = 0; j < 32; ++j)
           if ((nz >> j) & 1u) pr[j * kD] = __uint_as_float(raw[j]);
