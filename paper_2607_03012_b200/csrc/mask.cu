@@ -146,6 +146,18 @@ struct WarpSort {
     const bool sw = up ? (y > x) : (x > y);
     k[a] = sw ? y : x; k[b] = sw ? x : y;
   }
+  // descending sort of the lane's own E keys only (the within-lane stages of the network): no shuffles
+  __device__ __forceinline__ void sort_lane() {
+#pragma unroll
+    for (int kk = 2; kk <= E; kk <<= 1) {
+#pragma unroll
+      for (int d = kk >> 1; d > 0; d >>= 1) {
+#pragma unroll
+        for (int i = 0; i < E; ++i)
+          if ((i & d) == 0) cex(i, i | d, kk < E ? ((i & kk) == 0) : true);
+      }
+    }
+  }
   __device__ __forceinline__ void sort(int lane) {
 #pragma unroll
     for (int kk = 2; kk <= 32 * E; kk <<= 1) {
@@ -197,24 +209,40 @@ __global__ void __launch_bounds__(256, 2) hva_mask_warp_kernel(int Nq, int Nk, c
     s_q[e] = r < nrows ? (double)mu_q[((size_t)bh * Nq + i0 + r) * D + (e % D)] : 0.0;
   }
   __syncthreads();
-  // S_ij = <mu^q_i, mu^k_j> * scale   (Eq. 2), fp64 accumulation in ascending feature order
-  for (int jj = tid; jj < Nk; jj += 256) {
-    const float4* kr = reinterpret_cast<const float4*>(mu_k + ((size_t)bh * Nk + jj) * D);
-    double a[kWarpRows];
+  // S_ij = <mu^q_i, mu^k_j> * scale   (Eq. 2) in fp64 on the fp64 tensor path: one mma.m8n8k4 = the CTA's 8 query rows x 8 key
+  // clusters x 4 feature dims (256 FMAs per warp instruction, operands in registers; the CUDA-core form spent 6.6 K instructions
+  // per row on DFMA + shared-memory operand loads, half of the kernel).  Thread (g = lane / 4, t = lane % 4) holds A[g][t], B[t][g]
+  // and C[g][2t, 2t+1].  The k-steps walk the feature dims in the order 16 s + 4 t + e (s = 0 .. D/16 - 1, e = 0 .. 3), so that the
+  // thread's four B values of a step group are ONE 16-byte load of its key row; A is laid out to match and is loaded once per warp.
+  // The sum over the dims is associated as the tensor unit does it (fixed, deterministic); the products and the accumulation are
+  // fp64, so the scores agree with any other fp64 order to ~1e-16 relative (R-K3).
+  {
+    const int g = lane >> 2, t = lane & 3;
+    double aq[D / 4];
 #pragma unroll
-    for (int r = 0; r < kWarpRows; ++r) a[r] = 0.0;
-#pragma unroll 2
-    for (int c = 0; c < D / 4; ++c) {
-      const float4 v = __ldg(kr + c);
-      const double x0 = v.x, x1 = v.y, x2 = v.z, x3 = v.w;
+    for (int s4 = 0; s4 < D / 16; ++s4)
 #pragma unroll
-      for (int r = 0; r < kWarpRows; ++r) {
-        const double* q = s_q + r * D + 4 * c;
-        a[r] = fma(x0, q[0], a[r]); a[r] = fma(x1, q[1], a[r]); a[r] = fma(x2, q[2], a[r]); a[r] = fma(x3, q[3], a[r]);
+      for (int e = 0; e < 4; ++e) aq[4 * s4 + e] = s_q[g * D + 16 * s4 + 4 * t + e];
+    const int nblk = (Nk + 7) >> 3;
+    for (int blk = warp; blk < nblk; blk += 8) {
+      const int n = min(8 * blk + g, Nk - 1);                 // keys past N_k re-read the last row; their columns are not stored
+      const float4* kr = reinterpret_cast<const float4*>(mu_k + ((size_t)bh * Nk + n) * D) + t;
+      double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+      for (int s4 = 0; s4 < D / 16; ++s4) {
+        const float4 v = __ldg(kr + 4 * s4);
+        const double bv[4] = {(double)v.x, (double)v.y, (double)v.z, (double)v.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                       : "+d"(c0), "+d"(c1) : "d"(aq[4 * s4 + e]), "d"(bv[e]));
+      }
+      const int j0 = 8 * blk + 2 * t;
+      if (g < nrows) {
+        if (j0 < Nk) s_sc[(size_t)g * P + j0] = c0 * scale;
+        if (j0 + 1 < Nk) s_sc[(size_t)g * P + j0 + 1] = c1 * scale;
       }
     }
-#pragma unroll
-    for (int r = 0; r < kWarpRows; ++r) s_sc[(size_t)r * P + jj] = a[r] * scale;
   }
   __syncthreads();
   if (warp >= nrows) return;
@@ -236,32 +264,66 @@ __global__ void __launch_bounds__(256, 2) hva_mask_warp_kernel(int Nq, int Nk, c
     const int jj = 32 * i + lane;
     ws.k[i] = jj < Nk ? mask_key((double)sizes_k[(size_t)bh * Nk + jj] * exp(wv[i] - smax), jj) : (unsigned long long)(2047 - jj);
   }
-  ws.sort(lane);
-  // inclusive scan of the sorted weights: sequential inside a lane (positions lane E .. lane E + E - 1), shuffle scan across lanes
+  // Selection instead of a full sort of the row (round 2: 55 bitonic stages, two thirds of the kernel's instructions).  The cut is
+  // the LARGEST key c with  sum_{k >= c} w_k >= p Z  and  #{k >= c} >= kmin  (Eq. 3 + min-kc: the same prefix as "sort, then first
+  // cum >= p Z"; keys are unique, so "k >= c" is the sorted prefix that ends at c).  Each lane sorts only its own E keys (registers, no
+  // shuffles) and parks them in shared memory, skey[i][lane]; then a quickselect on the key VALUE: the pivot is the middle key of
+  // the longest still-undecided lane segment (keys j = 32 i + lane are an interleaved sample of the row, so it splits every lane's
+  // segment about in half), every lane counts its keys >= pivot by binary search and adds the weights of the keys that moved, and the
+  // warp decides.  ~12-15 rounds of ~90 instructions.  The sums are associated differently from a sequential cumulative sum (R-K3's
+  // 1e-9 Z exemption covers that, as it did the scan's).
+  ws.sort_lane();
+  unsigned long long* skey = reinterpret_cast<unsigned long long*>(s_sc + (size_t)warp * P);   // the row's scores are consumed
   double run = 0.0;
 #pragma unroll
   for (int i = 0; i < E; ++i) run += mask_key_w(ws.k[i]);
-  double incl = run;
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const double y = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += y;
+  for (int o = 16; o > 0; o >>= 1) run += __shfl_xor_sync(0xffffffffu, run, o);   // same bits in every lane (commutative tree)
+  const double thr = top_p * run;
+  __syncwarp();
+#pragma unroll
+  for (int i = 0; i < E; ++i) skey[i * 32 + lane] = ws.k[i];
+  __syncwarp();
+  const unsigned long long U0 = (unsigned long long)(2047 - Nk);   // below every real key, at or above every pad: "everything"
+  unsigned long long U = U0;                                     // largest key known to satisfy the condition
+  int a = 0;                                                     // keys [0, a) of this lane are >= L, the smallest key known to fail
+  int b = lane < Nk ? (Nk - lane + 31) >> 5 : 0;                 // keys [a, b) are undecided (the lane's real keys come first)
+  double S_hi = 0.0;                                             // sum of the weights of all keys >= L
+  int N_hi = 0;
+  for (;;) {
+    const unsigned best = __reduce_max_sync(0xffffffffu, ((unsigned)(b - a) << 5) | (unsigned)lane);
+    if ((best >> 5) == 0) break;
+    const int src = (int)(best & 31u);
+    const unsigned long long mine = b > a ? skey[((a + b) >> 1) * 32 + lane] : 0ull;
+    const unsigned long long pv = __shfl_sync(0xffffffffu, mine, src);
+    int lo = a, hi = b;                                          // c = number of this lane's keys >= pv
+#pragma unroll
+    for (int it = 0; it < 6; ++it) {
+      if (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (skey[mid * 32 + lane] >= pv) lo = mid + 1; else hi = mid;
+      }
+    }
+    const int c = lo;
+    double sum = 0.0;
+    for (int idx = a; idx < c; ++idx) sum += mask_key_w(skey[idx * 32 + lane]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    const int cn = __reduce_add_sync(0xffffffffu, c - a);
+    const double S = S_hi + sum;
+    const int N = N_hi + cn;
+    if (S >= thr && N >= kmin) {     // warp-uniform: S, N are the same bits in every lane
+      U = pv;
+      b = c - (lane == src ? 1 : 0);                             // undecided: the keys above pv
+    } else {
+      a = c; S_hi = S; N_hi = N;                                 // pv fails and becomes L
+    }
   }
-  const double Z = __shfl_sync(0xffffffffu, incl, 31), thr = top_p * Z;
-  double a = incl - run;
-  int first = Nk;                                            // smallest k with cum_k >= p Z   (Eq. 3)
 #pragma unroll
   for (int i = 0; i < E; ++i) {
-    a += mask_key_w(ws.k[i]);
-    if (a >= thr && first == Nk && lane * E + i < Nk) first = lane * E + i + 1;
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) first = min(first, __shfl_xor_sync(0xffffffffu, first, o));
-  const int kcut = first < kmin ? kmin : first;
-#pragma unroll
-  for (int i = 0; i < E; ++i) {
-    const int jj = mask_key_j(ws.k[i]);
-    if (jj < Nk) mrow[jj] = (lane * E + i < kcut) ? 1 : 0;
+    const unsigned long long k = skey[i * 32 + lane];
+    const int jj = mask_key_j(k);
+    if (jj < Nk) mrow[jj] = k >= U ? 1 : 0;
   }
 }
 
