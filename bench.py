@@ -326,8 +326,8 @@ def main():
            "clocks": clocks,
            "e2e": {"value": e2e_ms if strong else e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
            # kernels of one hva_forward: per tensor init (writes the bf16 split too) + iters x (assign, finalize); mask; merge init (+ nterms) + R x (overlap,
-           # propose, apply) + rank + out; plan groups + work + hist + scan + scatter; K and V permutes (Q is gathered inside the attention kernel); attention
-           "gpu_launches": args.steps * (2 * (1 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 5 + 2 + 1)}
+           # propose, apply) + rank + out; plan: key half (koff, hist, scan, scatter; side stream) + query half (groups, work, hist, scan, scatter); one K, V gather (Q is gathered inside the attention kernel); attention
+           "gpu_launches": args.steps * (2 * (1 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 9 + 1 + 1)}
 
     # ---- per-stage times and rooflines (rank 0)
     if rank == 0 and not args.no_stages:
@@ -617,7 +617,7 @@ def stage_report(b, wl, shape, cfg, Q, K, V, stats, pk, cl_alone=None):
                              "timed": "inside the step (right after the timed region, GPU at its power-capped clock)",
                              "frac_timed_alone": (cl_bytes / (cl_alone * 1e-3) / 1e9 / pk["hbm"]) if cl_alone else None,
                              "algorithmic_bytes": cl_bytes},
-        "roofline_permute": {"bound": "hbm", "kernel": "hva_permute_kernel", "achieved": pm_bytes / (st["permute_kv"] * 1e-3) / 1e9,
+        "roofline_permute": {"bound": "hbm", "kernel": "hva_gather_kv_kernel", "achieved": pm_bytes / (st["permute_kv"] * 1e-3) / 1e9,
                              "peak": pk["hbm"], "unit": "GB/s", "frac": pm_bytes / (st["permute_kv"] * 1e-3) / 1e9 / pk["hbm"]},
         "occupancy": occupancy(wl, stats),
     }

@@ -23,13 +23,14 @@ struct FwdLayout {
 // under the other's pass.  One side stream + two events per device, created on first use; a call only enqueues on them.
 struct SideStream {
   cudaStream_t st = nullptr;
-  cudaEvent_t fork = nullptr, join = nullptr;
+  cudaEvent_t fork = nullptr, mid = nullptr, join = nullptr;
   bool tried = false, ok = false;
   std::mutex busy;   // held while a call enqueues its fork .. join sequence
   void create() {
     tried = true;
     ok = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess &&
          cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&mid, cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&join, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) cudaGetLastError();
   }
@@ -223,9 +224,52 @@ int forward_impl(const hva_shape* s, const hva_config* c, const void* Q, const v
   const size_t es = s->dtype == HVA_F32 ? 4 : 2;
   const bool two_streams = step_kind == HVA_ANCHOR && !hybrid && (size_t)BH * n * s->D * es >= F.scratch_bytes && side_stream() != nullptr;
   if (two_streams) {
-    HVA_TRY(hva_cluster_qk(s, c, Q, K, (int32_t*)(sb + F.assign[0]), (float*)(sb + F.mu[0]), (int32_t*)(sb + F.sizes[0]), (float*)(sb + F.sums[0]),
-                           (int32_t*)(sb + F.assign[1]), (float*)(sb + F.mu[1]), (int32_t*)(sb + F.sizes[1]), (float*)(sb + F.sums[1]),
-                           w + F.scratch, F.scratch_bytes, w + F.kp, (size_t)BH * n * s->D * es, stream));
+    // caller's stream: cluster Q ................. [wait K clustered] mask, merge, query half of the plan [wait side] attention
+    // side stream:     cluster K, key half of the plan (koff, perm_k: they depend on the K clustering alone), K' and V' gathers
+    // -- the gathers (HBM-bound) run under mask and merge (ALU / latency-bound).  Scratch on the side stream: the K' region for the
+    // clustering, the V' region for the key sort, each before it is written.  Fork / join by events: legal under stream capture.
+    SideStream* side = side_stream();
+    std::lock_guard<std::mutex> guard(side->busy);
+    cudaStream_t ss = side->st;
+    const size_t xbytes = (size_t)BH * n * s->D * es;
+    if (hva_plan_keys_ws_bytes(BH, n, F.Nk) > xbytes) return HVA_EWORKSPACE;
+    if (cudaEventRecord(side->fork, st) != cudaSuccess || cudaStreamWaitEvent(ss, side->fork, 0) != cudaSuccess) return HVA_ECUDA;
+    int rc = hva_cluster_ex(s, cell[0], win[0], c->iters, Q, nullptr, (int32_t*)(sb + F.assign[0]), (float*)(sb + F.mu[0]),
+                            (int32_t*)(sb + F.sizes[0]), (float*)(sb + F.sums[0]), nullptr, c->flags, nullptr, w + F.scratch, F.scratch_bytes, stream);
+    int rs = hva_cluster_ex(s, cell[1], win[1], c->iters, K, nullptr, (int32_t*)(sb + F.assign[1]), (float*)(sb + F.mu[1]),
+                            (int32_t*)(sb + F.sizes[1]), (float*)(sb + F.sums[1]), nullptr, c->flags, nullptr, w + F.kp, xbytes, ss);
+    if (rs == HVA_OK && cudaEventRecord(side->mid, ss) != cudaSuccess) rs = HVA_ECUDA;
+    if (rs == HVA_OK) rs = hva_plan_keys(BH, n, F.Nk, (int32_t*)(sb + F.assign[1]), (int32_t*)(sb + F.sizes[1]), plan, F.PL, w + F.vp, xbytes, ss);
+    const char* pbk = reinterpret_cast<const char*>(plan);
+    if (rs == HVA_OK) rs = hva_gather_kv(s, K, V, (const int32_t*)(pbk + F.PL.perm_k), w + F.kp, w + F.vp, ss);
+    if (rc == HVA_OK && rs == HVA_OK && cudaStreamWaitEvent(st, side->mid, 0) != cudaSuccess) rc = HVA_ECUDA;
+    if (rc == HVA_OK && rs == HVA_OK) {
+      const float scale2 = c->softmax_scale > 0.f ? c->softmax_scale : 1.0f / sqrtf((float)s->D);
+      uint8_t* mask = (uint8_t*)(w + F.mask);
+      uint8_t* gmask = (uint8_t*)(w + F.group_mask);
+      int32_t* group_of = (int32_t*)(w + F.group_of);
+      int32_t* n_groups = (int32_t*)(w + F.n_groups);
+      rc = hva_build_mask_ex(BH, F.Nq, F.Nk, s->D, (float*)(sb + F.mu[0]), (float*)(sb + F.mu[1]), (int32_t*)(sb + F.sizes[1]), scale2,
+                             c->top_p, c->min_kc, mask, c->flags, w + F.scratch, F.scratch_bytes, stream);
+      if (rc == HVA_OK)
+        rc = hva_merge_offset(bh0, BH, F.Nq, F.Nk, (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), mask, c->tile_q, c->tile_k,
+                              c->merge_rounds, c->max_q_tiles, c->seed, group_of, n_groups, gmask, c->flags, w + F.scratch, F.scratch_bytes, stream);
+      if (rc == HVA_OK)
+        rc = hva_plan_queries(BH, n, F.Nq, F.Nk, (int32_t*)(sb + F.assign[0]), (int32_t*)(sb + F.sizes[0]), (int32_t*)(sb + F.sizes[1]), group_of,
+                              gmask, c->tile_q, c->tile_k, plan, F.PL, w + F.scratch, F.scratch_bytes, st);
+    }
+    // join even after an error: the side stream must not stay forked (stream capture)
+    if (cudaEventRecord(side->join, ss) != cudaSuccess || cudaStreamWaitEvent(st, side->join, 0) != cudaSuccess) return HVA_ECUDA;
+    if (rc != HVA_OK) return rc;
+    if (rs != HVA_OK) return rs;
+    if (!F.fuse_q) HVA_TRY(hva_permute(s, Q, (const int32_t*)(pbk + F.PL.perm_q), w + F.qp, stream));
+    hva_config ca = *c;
+    if (F.fuse_q) ca.flags |= HVA_FLAG_Q_UNPERMUTED;
+    HVA_TRY(hva_sparse_attention(s, &ca, F.fuse_q ? Q : (const void*)(w + F.qp), w + F.kp, w + F.vp, plan, F.PL.total, F.Nq, F.Nk, O, 1, nullptr, 0,
+                                 stream));
+    if (stats_out && cudaMemcpyAsync(stats_out, pbk + F.PL.stats, sizeof(hva_stats) * BH, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+      return HVA_ECUDA;
+    return HVA_OK;
   }
   for (int t = 0; t < 2 && !two_streams; ++t) {
     int32_t* assign = (int32_t*)(sb + F.assign[t]);

@@ -74,6 +74,14 @@ struct HvaGrid;
 size_t hva_cluster_ws_bytes(const HvaGrid& g, int BH, int D);
 size_t hva_merge_ws_bytes(int BH, int Nq, int Nk);
 size_t hva_plan_ws_bytes(int BH, int n, int Nq, int Nk);
+// hva_build_plan in two halves (plan.cu): keys (koff, perm_k) from the K clustering alone; queries (everything else)
+int hva_gather_kv(const hva_shape* s, const void* K, const void* V, const int32_t* perm, void* Kp, void* Vp, cudaStream_t st);
+size_t hva_plan_keys_ws_bytes(int BH, int n, int Nk);
+int hva_plan_keys(int BH, int n, int Nk, const int* assign_k, const int* sizes_k, void* plan, const hva_plan_layout& L, void* ws,
+                  size_t ws_bytes, cudaStream_t st);
+int hva_plan_queries(int BH, int n, int Nq, int Nk, const int* assign_q, const int* sizes_q, const int* sizes_k, const int* group_of_cluster,
+                     const uint8_t* group_mask, int tile_q, int tile_k, void* plan, const hva_plan_layout& L, void* ws, size_t ws_bytes,
+                     cudaStream_t st);
 size_t hva_hybrid_ws_bytes(int BH, int n, int Nc, int m, int D);
 size_t hva_refresh_ws_bytes(int BH, int n, int Nc);
 // R-H3': mu, sums, sizes of every cluster recomputed from the current X and labels (plan.cu: label sort + segment means)

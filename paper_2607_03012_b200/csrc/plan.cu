@@ -60,11 +60,12 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
                                                                const int* __restrict__ sizes_k,
                                                                const int* __restrict__ group_of,
                                                                const uint8_t* __restrict__ group_mask, int tile_q,
-                                                               int tile_k, PlanPtrs P, int* __restrict__ qbase) {
+                                                               int tile_k, PlanPtrs P, int* __restrict__ qbase, int write_koff) {
   // blockIdx.y: the key-run extraction (the long part: one pass over the group's mask row per group) is split over the
   // gridDim.y CTAs of a head; the scans are cheap and every CTA does them, CTA 0 of the head writes their results
   const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool lead = blockIdx.y == 0;
+  const bool lead_k = lead && write_koff;     // hva_plan_keys() has written koff already (and K' may be being gathered with it)
   int* koff = P.koff + (size_t)bh * (Nk + 1);
   int* gid = P.gid + (size_t)bh * Nq;
   int* goff = P.goff + (size_t)bh * (Nq + 1);
@@ -89,9 +90,9 @@ __global__ void __launch_bounds__(1024) hva_plan_groups_kernel(int n, int Nq, in
   {
     const int j0 = 2 * tid, a = j0 < Nk ? s_sk[j0] : 0, b = j0 + 1 < Nk ? s_sk[j0 + 1] : 0;
     const int e = block_excl_scan(a + b, s_warp, &s_tot);
-    if (lead && j0 < Nk) koff[j0] = e;
-    if (lead && j0 + 1 < Nk) koff[j0 + 1] = e + a;
-    if (lead && tid == 0) koff[Nk] = s_tot;
+    if (lead_k && j0 < Nk) koff[j0] = e;
+    if (lead_k && j0 + 1 < Nk) koff[j0 + 1] = e + a;
+    if (lead_k && tid == 0) koff[Nk] = s_tot;
   }
   // active groups in ascending gid (a leader whose group has no rows is not active) and their Q' row offsets
   int ng;
@@ -417,7 +418,7 @@ extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, con
   if (gsmem > 48 * 1024 && cudaFuncSetAttribute(hva_plan_groups_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem) != cudaSuccess)
     return HVA_EUNSUPPORTED;
   hva_plan_groups_kernel<<<dim3(BH, kGroupSplit), 1024, gsmem, st>>>(n, Nq, Nk, sizes_q, sizes_k, group_of_cluster, group_mask, tile_q,
-                                                                 tile_k, P, qbase);
+                                                                 tile_k, P, qbase, 1);
   HVA_CHECK_LAUNCH();
   hva_plan_work_kernel<<<BH, 1024, 0, st>>>(Nq, tile_q, tile_k, P);
   HVA_CHECK_LAUNCH();
@@ -430,6 +431,79 @@ extern "C" int hva_build_plan(int32_t BH, int32_t n, int32_t Nq, int32_t Nk, con
   hva_sort_hist_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
   HVA_CHECK_LAUNCH();
   hva_sort_scan_kernel<<<dim3((Ncmax + 3) / 4, BH, 2), 128, 0, st>>>(ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
+}
+
+// ---- hva_build_plan in two halves for hva_forward: the key half (koff, perm_k) depends on the K clustering alone, so it and the
+// K', V' gathers run on the side stream while mask, merge and the query half run on the caller's.  Same kernels, same results.
+__global__ void __launch_bounds__(1024) hva_koff_kernel(int Nk, const int* __restrict__ sizes_k, int* __restrict__ koff_all) {
+  const int bh = blockIdx.x, tid = threadIdx.x;
+  __shared__ int s_warp[32];
+  __shared__ int s_tot;
+  int* koff = koff_all + (size_t)bh * (Nk + 1);
+  const int j0 = 2 * tid, a = j0 < Nk ? sizes_k[(size_t)bh * Nk + j0] : 0, b = j0 + 1 < Nk ? sizes_k[(size_t)bh * Nk + j0 + 1] : 0;
+  const int e = block_excl_scan(a + b, s_warp, &s_tot);
+  if (j0 < Nk) koff[j0] = e;
+  if (j0 + 1 < Nk) koff[j0 + 1] = e + a;
+  if (tid == 0) koff[Nk] = s_tot;
+}
+
+size_t hva_plan_keys_ws_bytes(int BH, int n, int Nk) {
+  const int ntile = (n + kTile - 1) / kTile;
+  return hva_align((size_t)BH * ntile * Nk * 4);
+}
+
+int hva_plan_keys(int BH, int n, int Nk, const int* assign_k, const int* sizes_k, void* plan, const hva_plan_layout& L, void* ws,
+                  size_t ws_bytes, cudaStream_t st) {
+  if (Nk > 2048) return HVA_EUNSUPPORTED;
+  if (ws_bytes < hva_plan_keys_ws_bytes(BH, n, Nk)) return HVA_EWORKSPACE;
+  PlanPtrs P = plan_ptrs(plan, L);
+  const int ntile = (n + kTile - 1) / kTile;
+  hva_koff_kernel<<<BH, 1024, 0, st>>>(Nk, sizes_k, P.koff);
+  HVA_CHECK_LAUNCH();
+  SortArgs A;
+  A.p[0] = SortPass{Nk, assign_k, reinterpret_cast<int*>(ws), P.koff, Nk + 1, P.perm_k, nullptr};
+  A.p[1] = A.p[0];
+  const dim3 gsort((ntile + kSortWarps - 1) / kSortWarps, BH, 1);
+  const size_t smem = (size_t)kSortWarps * Nk * sizeof(int);
+  hva_sort_hist_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scan_kernel<<<dim3((Nk + 3) / 4, BH, 1), 128, 0, st>>>(ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
+}
+
+// the query half: groups, key runs, work list, perm_q / inv_perm_q; koff is left alone.  ws: hva_plan_ws_bytes()
+int hva_plan_queries(int BH, int n, int Nq, int Nk, const int* assign_q, const int* sizes_q, const int* sizes_k, const int* group_of_cluster,
+                     const uint8_t* group_mask, int tile_q, int tile_k, void* plan, const hva_plan_layout& L, void* ws, size_t ws_bytes,
+                     cudaStream_t st) {
+  if (Nq > 2048 || Nk > 2048 || (n + tile_q - 1) / tile_q > 32767) return HVA_EUNSUPPORTED;
+  if (ws_bytes < hva_plan_ws_bytes(BH, n, Nq, Nk)) return HVA_EWORKSPACE;
+  PlanPtrs P = plan_ptrs(plan, L);
+  const int ntile = (n + kTile - 1) / kTile;
+  int* hist_q = reinterpret_cast<int*>(ws);
+  int* qbase = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + hva_align((size_t)BH * ntile * Nq * 4));
+  const size_t gsmem = sizeof(int) * (5 * (size_t)Nq + Nk + 1);
+  if (gsmem > 48 * 1024 && cudaFuncSetAttribute(hva_plan_groups_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem) != cudaSuccess)
+    return HVA_EUNSUPPORTED;
+  hva_plan_groups_kernel<<<dim3(BH, kGroupSplit), 1024, gsmem, st>>>(n, Nq, Nk, sizes_q, sizes_k, group_of_cluster, group_mask, tile_q,
+                                                                 tile_k, P, qbase, 0);
+  HVA_CHECK_LAUNCH();
+  hva_plan_work_kernel<<<BH, 1024, 0, st>>>(Nq, tile_q, tile_k, P);
+  HVA_CHECK_LAUNCH();
+  SortArgs A;
+  A.p[0] = SortPass{Nq, assign_q, hist_q, qbase, Nq, P.perm_q, P.inv_perm_q};
+  A.p[1] = A.p[0];
+  const dim3 gsort((ntile + kSortWarps - 1) / kSortWarps, BH, 1);
+  const size_t smem = (size_t)kSortWarps * Nq * sizeof(int);
+  hva_sort_hist_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
+  HVA_CHECK_LAUNCH();
+  hva_sort_scan_kernel<<<dim3((Nq + 3) / 4, BH, 1), 128, 0, st>>>(ntile, A);
   HVA_CHECK_LAUNCH();
   hva_sort_scatter_kernel<<<gsort, kSortWarps * 32, smem, st>>>(n, ntile, A);
   HVA_CHECK_LAUNCH();
@@ -491,10 +565,78 @@ static int permute_common(const hva_shape* s, const void* X, const int32_t* perm
 }
 
 extern "C" int hva_permute(const hva_shape* s, const void* X, const int32_t* perm, void* Xp, void* stream) {
-  return permute_common(s, X, perm, Xp, stream, 0);
+  if (!s || !X || !perm || !Xp) return HVA_EINVAL;
+  if (s->D != 64 && s->D != 128) return HVA_EINVAL;
+  if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
+  if ((size_t)s->B * s->heads * s->T * s->H * s->W >= 0x7fffffffull) return permute_common(s, X, perm, Xp, stream, 0);
+  return hva_gather_kv(s, X, nullptr, perm, Xp, nullptr, reinterpret_cast<cudaStream_t>(stream));
 }
 extern "C" int hva_unpermute(const hva_shape* s, const void* Xp, const int32_t* perm, void* X, void* stream) {
   return permute_common(s, Xp, perm, X, stream, 1);
+}
+
+// K' and V' in one background launch for hva_forward's side stream: the same gather as hva_permute (both tensors share perm_k), but as
+// two resident CTAs per SM with eight 16-byte loads in flight per thread instead of a grid that fills every thread slot -- it has
+// to run UNDER the mask and merge kernels of the caller's stream, which need those slots (a full-occupancy gather just ran before
+// them: no overlap).  The perm entries of the next iteration are fetched while the rows of the current one are in flight.
+template <int RC, bool kBoth>     // 16-byte chunks per row: 8, 16 or 32; kBoth: K and V (else V, Vp are unused)
+__global__ void __launch_bounds__(256) hva_gather_kv_kernel(unsigned rows_total, unsigned n, const uint4* __restrict__ K, const uint4* __restrict__ V,
+                                                            const int* __restrict__ perm, uint4* __restrict__ Kp, uint4* __restrict__ Vp) {
+  constexpr int RPW = 32 / RC, U = 4;                         // rows per warp instruction, instructions per iteration
+  const int lane = threadIdx.x & 31, sub = lane / RC, q = lane % RC;
+  const unsigned wg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+  unsigned src[U], src_next[U];
+  auto fetch = [&](unsigned base, unsigned (&out)[U]) {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const unsigned row = base + u * RPW + sub;
+      out[u] = row < rows_total ? (row / n) * n + (unsigned)__ldg(perm + row) : 0xffffffffu;
+    }
+  };
+  unsigned base = wg * (U * RPW);
+  const unsigned stride = nw * (U * RPW);
+  if (base < rows_total) fetch(base, src_next);
+  for (; base < rows_total; base += stride) {
+#pragma unroll
+    for (int u = 0; u < U; ++u) src[u] = src_next[u];
+    uint4 kv[U], vv[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (src[u] != 0xffffffffu) { kv[u] = __ldg(K + (size_t)src[u] * RC + q); if (kBoth) vv[u] = __ldg(V + (size_t)src[u] * RC + q); }
+    }
+    if (base + stride < rows_total && base + stride > base) fetch(base + stride, src_next);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (src[u] != 0xffffffffu) {
+        const size_t row = (size_t)base + u * RPW + sub;
+        Kp[row * RC + q] = kv[u]; if (kBoth) Vp[row * RC + q] = vv[u];
+      }
+    }
+  }
+}
+
+int hva_gather_kv(const hva_shape* s, const void* K, const void* V, const int32_t* perm, void* Kp, void* Vp, cudaStream_t st) {
+  const int n = s->T * s->H * s->W;
+  const size_t rows = (size_t)s->B * s->heads * n;
+  if (rows >= 0x7fffffffull) return HVA_EUNSUPPORTED;
+  const int rc = s->D * (s->dtype == HVA_F32 ? 4 : 2) / 16;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HVA_ECUDA;
+  const dim3 grid(2 * sms);                                   // one tensor alone (hva_permute): four CTAs per SM for the same bytes in flight
+  const uint4 *k4 = reinterpret_cast<const uint4*>(K), *v4 = reinterpret_cast<const uint4*>(V);
+  uint4 *kp4 = reinterpret_cast<uint4*>(Kp), *vp4 = reinterpret_cast<uint4*>(Vp);
+  const unsigned r = (unsigned)rows, nn = (unsigned)n;
+  if (V) {
+    if (rc == 8) hva_gather_kv_kernel<8, true><<<grid, 256, 0, st>>>(r, nn, k4, v4, perm, kp4, vp4);
+    else if (rc == 16) hva_gather_kv_kernel<16, true><<<grid, 256, 0, st>>>(r, nn, k4, v4, perm, kp4, vp4);
+    else if (rc == 32) hva_gather_kv_kernel<32, true><<<grid, 256, 0, st>>>(r, nn, k4, v4, perm, kp4, vp4);
+    else return HVA_EUNSUPPORTED;
+  } else if (rc == 8) hva_gather_kv_kernel<8, false><<<dim3(4 * sms), 256, 0, st>>>(r, nn, k4, v4, perm, kp4, vp4);
+  else if (rc == 16) hva_gather_kv_kernel<16, false><<<dim3(4 * sms), 256, 0, st>>>(r, nn, k4, v4, perm, kp4, vp4);
+  else if (rc == 32) hva_gather_kv_kernel<32, false><<<dim3(4 * sms), 256, 0, st>>>(r, nn, k4, v4, perm, kp4, vp4);
+  else return HVA_EUNSUPPORTED;
+  HVA_CHECK_LAUNCH();
+  return HVA_OK;
 }
 
 int hva_attention_dense_plan(int BH, int n, int tile_q, int tile_k, void* plan, const hva_plan_layout& L, cudaStream_t st) {
