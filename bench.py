@@ -325,9 +325,9 @@ def main():
                                      float(cfg.top_p), int(cfg.merge_rounds), custom),
            "clocks": clocks,
            "e2e": {"value": e2e_ms if strong else e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes},
-           # kernels of one hva_forward: per tensor init (writes the bf16 split too) + iters x (assign, finalize); mask; merge init (+ nterms) + R x (overlap,
+           # kernels of one hva_forward: per tensor init (writes the bf16 split too) + iters x (assign, finalize); mask; merge init (+ nterms) + R x (sides, overlap,
            # propose, apply) + rank + out; plan: key half (koff, hist, scan, scatter; side stream) + query half (groups, work, hist, scan, scatter); one K, V gather (Q is gathered inside the attention kernel); attention
-           "gpu_launches": args.steps * (2 * (1 + 2 * wl.iters) + 1 + (3 + 3 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 9 + 1 + 1)}
+           "gpu_launches": args.steps * (2 * (1 + 2 * wl.iters) + 1 + (3 + 4 * int(cfg.merge_rounds) + (1 if int(cfg.merge_rounds) > 0 else 0)) + 9 + 1 + 1)}
 
     # ---- per-stage times and rooflines (rank 0)
     if rank == 0 and not args.no_stages:

@@ -105,21 +105,64 @@ __global__ void __launch_bounds__(256) hva_merge_propose_kernel(MergeParams p, i
 // Alg. 1 lines 6-13 for round r with the pairwise overlaps I[A][B] precomputed on the tensor pipe (merge_tc.cu):
 // kappa(A u B) = kappa(A) + kappa(B) - I[A][B].  One warp per A in side 1, lanes over B (coalesced row of I); the warp's
 // best (dC, gid(B)) is the lexicographic minimum == first minimum in ascending gid(B) with strict '<' (line 13).
-__global__ void __launch_bounds__(256) hva_merge_propose_inter_kernel(MergeParams p, int r, const int* __restrict__ inter, int Nqp) {
+// The round's bipartition as two compact lists (Alg. 1 line 6): alive groups of side 1 ascending from the front of list[bh], alive
+// groups of side 0 ascending at its end; cnt[bh] = (nA, nB).  One CTA per (b, head), two groups per thread (N_q <= 2048).
+__global__ void __launch_bounds__(1024) hva_merge_sides_kernel(MergeParams p, int r, int* __restrict__ list, int* __restrict__ cnt) {
+  const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, Nq = p.Nq;
+  const size_t e0 = (size_t)bh * Nq;
+  __shared__ int s_a[32], s_b[32];
+  int fa[2], fb[2];
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const int g = 2 * tid + e;
+    const bool al = g < Nq && p.alive[e0 + g];
+    const uint32_t sd = hva_side_hash(p.seed, (uint32_t)(p.bh0 + bh), (uint32_t)r, (uint32_t)g);
+    fa[e] = al && sd == 1; fb[e] = al && sd == 0;
+  }
+  int ia = fa[0] + fa[1], ib = fb[0] + fb[1];        // inclusive warp scans, then the warps' totals
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int ya = __shfl_up_sync(0xffffffffu, ia, o), yb = __shfl_up_sync(0xffffffffu, ib, o);
+    if (lane >= o) { ia += ya; ib += yb; }
+  }
+  if (lane == 31) { s_a[warp] = ia; s_b[warp] = ib; }
+  __syncthreads();
+  int oa = 0, ob = 0, ta = 0, tb = 0;
+  for (int w = 0; w < 32; ++w) {
+    if (w < warp) { oa += s_a[w]; ob += s_b[w]; }
+    ta += s_a[w]; tb += s_b[w];
+  }
+  int pa = oa + ia - (fa[0] + fa[1]), pb = ob + ib - (fb[0] + fb[1]);   // exclusive positions of this thread's first group
+  int* la = list + e0;
+  int* lb = list + e0 + (Nq - tb);
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const int g = 2 * tid + e;
+    if (fa[e]) la[pa++] = g;
+    if (fb[e]) lb[pb++] = g;
+  }
+  if (tid == 0) { cnt[2 * bh] = ta; cnt[2 * bh + 1] = tb; }
+}
+
+__global__ void __launch_bounds__(256) hva_merge_propose_inter_kernel(MergeParams p, int r, const int* __restrict__ inter, int Nqp,
+                                                                      const int* __restrict__ list, const int* __restrict__ cnt) {
   const int bh = blockIdx.y, tid = threadIdx.x, lane = tid & 31, Nq = p.Nq;
   const size_t e0 = (size_t)bh * Nq;
-  const int A = blockIdx.x * 8 + (tid >> 5);
-  if (A >= Nq || !p.alive[e0 + A] || hva_side_hash(p.seed, (uint32_t)(p.bh0 + bh), (uint32_t)r, (uint32_t)A) != 1) return;
+  const int nA = cnt[2 * bh], nB = cnt[2 * bh + 1];
+  const int i = blockIdx.x * 8 + (tid >> 5);           // i-th group of side 1
+  if (i >= nA) return;
+  const int A = list[e0 + i];
+  const int* listB = list + e0 + (Nq - nB);
   const int sA = p.sq[e0 + A], kA = p.kap[e0 + A], rA = cdiv(sA, p.tile_q), cA = rA * cdiv(kA, p.tile_k);
-  const int* row = inter + ((size_t)bh * Nqp + A) * Nqp;
+  const int* row = inter + ((size_t)bh * Nqp + i) * Nqp;
   int best_dc = 0, best_B = 0x7fffffff;
-  for (int B = lane; B < Nq; B += 32) {
-    if (!p.alive[e0 + B] || hva_side_hash(p.seed, (uint32_t)(p.bh0 + bh), (uint32_t)r, (uint32_t)B) != 0) continue;
+  for (int j = lane; j < nB; j += 32) {
+    const int B = listB[j];
     const int sB = p.sq[e0 + B], kB = p.kap[e0 + B], rB = cdiv(sB, p.tile_q), cB = rB * cdiv(kB, p.tile_k);
     const int rU = cdiv(sA + sB, p.tile_q);
     if (p.max_q_tiles > 0 && rU > p.max_q_tiles) continue;
     if (rU >= rA + rB) continue;                                      // no row tile saved => dC >= 0 (R-M6)
-    const int dc = rU * cdiv(kA + kB - row[B], p.tile_k) - cA - cB;   // Eq. 10 in tile units
+    const int dc = rU * cdiv(kA + kB - row[j], p.tile_k) - cA - cB;   // Eq. 10 in tile units
     if (dc < best_dc) { best_dc = dc; best_B = B; }                   // ascending B per lane: strict '<' keeps the lower gid
   }
   for (int o = 16; o > 0; o >>= 1) {
@@ -132,7 +175,6 @@ __global__ void __launch_bounds__(256) hva_merge_propose_inter_kernel(MergeParam
   }
 }
 
-// Alg. 1 lines 15-16: accepted pairs are disjoint, applied in parallel.  One CTA per (b, head); warp per pair.
 __global__ void __launch_bounds__(1024) hva_merge_apply_kernel(MergeParams p) {
   const int bh = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, Nq = p.Nq, Wd = p.Wd;
   uint32_t* chi = p.chi + (size_t)bh * Nq * Wd;
@@ -201,7 +243,8 @@ __global__ void __launch_bounds__(256) hva_merge_out_kernel(MergeParams p) {
 // tensor-pipe overlap matrix (merge_tc.cu)
 size_t hva_merge_inter_bytes(int BH, int Nq);
 int hva_merge_nterms_launch(int BH, int Nk, const int* sizes_k, int* nterms, cudaStream_t st);
-int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, cudaStream_t st);
+int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, const int* list,
+                           const int* cnt, cudaStream_t st);
 
 
 size_t hva_merge_ws_bytes(int BH, int Nq, int Nk) {
@@ -241,6 +284,7 @@ int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int3
   const int Nqp = (Nq + 127) / 128 * 128;
   int* inter = reinterpret_cast<int*>(w);
   int* nterms = reinterpret_cast<int*>(w + hva_align((size_t)BH * Nqp * Nqp * 4));
+  int* side_cnt = reinterpret_cast<int*>(w + hva_align((size_t)BH * Nqp * Nqp * 4) + hva_align((size_t)BH * 4));
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const dim3 gw((Nq + 7) / 8, BH);
   hva_merge_init_kernel<<<gw, 256, 0, st>>>(p);
@@ -249,8 +293,10 @@ int hva_merge_offset(int32_t bh0, int32_t BH, int32_t Nq, int32_t Nk, const int3
   if (use_inter) HVA_TRY(hva_merge_nterms_launch(BH, Nk, sizes_k, nterms, st));
   for (int r = 1; r <= rounds; ++r) {
     if (use_inter) {
-      HVA_TRY(hva_merge_inter_launch(BH, Nq, Nk, p.chi, sizes_k, nterms, inter, st));
-      hva_merge_propose_inter_kernel<<<gw, 256, 0, st>>>(p, r, inter, Nqp);
+      hva_merge_sides_kernel<<<BH, 1024, 0, st>>>(p, r, p.side, side_cnt);
+      HVA_CHECK_LAUNCH();
+      HVA_TRY(hva_merge_inter_launch(BH, Nq, Nk, p.chi, sizes_k, nterms, inter, p.side, side_cnt, st));
+      hva_merge_propose_inter_kernel<<<gw, 256, 0, st>>>(p, r, inter, Nqp, p.side, side_cnt);
     } else {
       hva_merge_propose_kernel<<<gw, 256, smem, st>>>(p, r);
     }

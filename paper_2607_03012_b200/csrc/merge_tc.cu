@@ -20,15 +20,22 @@ struct InterParams {
   const uint32_t* chi;               // [BH, Nq, Wd] bit-packed key sets
   const int* sizes_k;                // [BH, Nk]
   const int* nterms;                 // [BH] base-256 digits needed for max_j s^k_j (1..3)
-  int* inter;                        // [BH, Nqp, Nqp]
+  int* inter;                        // [BH, Nqp, Nqp]: I[i][j] for the i-th group of side 1 (rows) and the j-th group of side 0 (columns)
+  const int* list;                   // [BH, Nq]: the round's alive groups of side 1 ascending from the front, of side 0 ascending at the end
+  const int* cnt;                    // [BH, 2]: how many of each
 };
 
 // 8 key bits -> 8 bf16 values (bit ? v[i] : 0) as one 16-byte chunk; v4 = the 8 bf16 values packed in four words
 // (a 256-entry shared-memory mask table was measured slower: bank conflicts)
+// Two bits select the two bf16 halves of a word with ONE byte permute: selector = 16 bits of a constant picked by the bit pair
+// (00 -> 0x4444: both halves from the zero operand, 01 -> 0x4410, 10 -> 0x3244, 11 -> 0x3210): 4 instructions per word where the
+// multiply-by-0xFFFF masks took 9 (the expansion is what this kernel's threads spend their time on)
+__device__ __forceinline__ uint32_t pick2(uint32_t v, uint32_t bits, int i) {
+  const unsigned long long sel = 0x3210324444104444ull;
+  return __byte_perm(v, 0u, (uint32_t)(sel >> (((bits >> (2 * i)) & 3u) << 4)));
+}
 __device__ __forceinline__ uint4 expand8(uint32_t bits, const uint4& v4) {
-  const uint32_t m0 = (bits & 1u) * 0xFFFFu | ((bits >> 1) & 1u) * 0xFFFF0000u, m1 = ((bits >> 2) & 1u) * 0xFFFFu | ((bits >> 3) & 1u) * 0xFFFF0000u;
-  const uint32_t m2 = ((bits >> 4) & 1u) * 0xFFFFu | ((bits >> 5) & 1u) * 0xFFFF0000u, m3 = ((bits >> 6) & 1u) * 0xFFFFu | ((bits >> 7) & 1u) * 0xFFFF0000u;
-  return make_uint4(v4.x & m0, v4.y & m1, v4.z & m2, v4.w & m3);
+  return make_uint4(pick2(v4.x, bits, 0), pick2(v4.y, bits, 1), pick2(v4.z, bits, 2), pick2(v4.w, bits, 3));
 }
 
 constexpr int kColBlocks = 2;          // 128-group column blocks per CTA: 256 TMEM columns and 48 KB of tiles, so that TWO CTAs share an SM and
@@ -38,7 +45,14 @@ constexpr int kRowsPerThread = ((1 + kColBlocks) * 128 + 255) / 256;      // (1 
 __global__ void __launch_bounds__(kThreadsG, 2) hva_merge_inter_kernel(InterParams p) {
   const int bh = blockIdx.z, mb = blockIdx.x, cg = blockIdx.y;          // rows [128 mb, +128), column blocks kColBlocks cg ...
   const int tid = threadIdx.x, warp = tid >> 5;
-  const int ncb = min(kColBlocks, p.Nqp / 128 - kColBlocks * cg);      // column blocks of this CTA
+  // Alg. 1 only pairs a group A of side 1 with a group B of side 0 (line 6): rows = the nA alive groups of side 1, columns = the nB
+  // of side 0, both compacted -- a quarter of the N_q x N_q pairs in the first round, fewer later.  The grid is sized for the worst
+  // case; CTAs past the counts leave at once.
+  const int nA = p.cnt[2 * bh], nB = p.cnt[2 * bh + 1];
+  if (128 * mb >= nA || 128 * kColBlocks * cg >= nB) return;
+  const int* listA = p.list + (size_t)bh * p.Nq;
+  const int* listB = listA + (p.Nq - nB);
+  const int ncb = min(kColBlocks, (nB + 127) / 128 - kColBlocks * cg);  // column blocks of this CTA
   const int nt = p.nterms[bh];
   extern __shared__ unsigned char raw[];
   unsigned char* smem = raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);
@@ -67,7 +81,7 @@ __global__ void __launch_bounds__(kThreadsG, 2) hva_merge_inter_kernel(InterPara
     grp[k] = -1; dst[k] = sA;
     if (tile < 1 + ncb) {
       const int gg = tile == 0 ? 128 * mb + r : 128 * (kColBlocks * cg + tile - 1) + r;
-      grp[k] = gg < p.Nq ? gg : -2;                                      // -2: row of zeros
+      grp[k] = tile == 0 ? (gg < nA ? listA[gg] : -2) : (gg < nB ? listB[gg] : -2);   // -2: row of zeros
       dst[k] = (tile == 0 ? sA : sB + (size_t)(tile - 1) * kTileB) + r * 128;
     }
   }
@@ -137,7 +151,7 @@ __global__ void __launch_bounds__(kThreadsG, 2) hva_merge_inter_kernel(InterPara
         for (int cc = 0; cc < 4; ++cc) {
           uint32_t v[32];
           tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + cb * 128 + cc * 32, v);
-          if (r < p.Nq) {
+          if (r < nA) {
             int* out = p.inter + ((size_t)bh * p.Nqp + r) * p.Nqp + 128 * (kColBlocks * cg + cb) + cc * 32;
 #pragma unroll
             for (int i = 0; i < 32; i += 4) {
@@ -175,7 +189,7 @@ __global__ void hva_merge_nterms_kernel(int Nk, const int* __restrict__ sizes_k,
 
 size_t hva_merge_inter_bytes(int BH, int Nq) {
   const size_t Nqp = ((size_t)Nq + 127) / 128 * 128;
-  return hva_align((size_t)BH * Nqp * Nqp * 4) + hva_align((size_t)BH * 4);
+  return hva_align((size_t)BH * Nqp * Nqp * 4) + hva_align((size_t)BH * 4) + hva_align((size_t)BH * 2 * 4);   // I, digits, side counts
 }
 
 int hva_merge_nterms_launch(int BH, int Nk, const int* sizes_k, int* nterms, cudaStream_t st) {
@@ -184,8 +198,9 @@ int hva_merge_nterms_launch(int BH, int Nk, const int* sizes_k, int* nterms, cud
   return HVA_OK;
 }
 
-int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, cudaStream_t st) {
-  InterParams p{Nq, Nk, (Nk + 31) / 32, (Nq + 127) / 128 * 128, chi, sizes_k, nterms, inter};
+int hva_merge_inter_launch(int BH, int Nq, int Nk, const uint32_t* chi, const int* sizes_k, const int* nterms, int* inter, const int* list,
+                           const int* cnt, cudaStream_t st) {
+  InterParams p{Nq, Nk, (Nk + 31) / 32, (Nq + 127) / 128 * 128, chi, sizes_k, nterms, inter, list, cnt};
   const size_t smem = 1024 + (1 + kColBlocks) * (size_t)kTileB + 8 * 16 + 64;
   // (per device and cheap: set on every call rather than behind a process-wide flag)
   if (cudaFuncSetAttribute(hva_merge_inter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return HVA_ECUDA;
