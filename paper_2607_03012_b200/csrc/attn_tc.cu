@@ -265,6 +265,19 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
       __syncwarp();
     };
     mbar_wait(&B->q_full, 0);
+    {
+      // rows of the Q tile past the end of the group (the loads over-read / repeat rows there) are cleared: their scores, probabilities
+      // and output rows are never used, and under the power cap a zero row costs the tensor pipe less than a live one
+      const int nval = row1 - row0;
+      if (nval < kBM) {
+        for (int e = lane; e < (kBM - nval) * 16; e += 32) {
+          const int rr = nval + (e >> 4), q = e & 15;
+          *reinterpret_cast<uint4*>(sQ + (q >> 3) * kHalfBytes + rr * 128 + ((q & 7) << 4)) = make_uint4(0u, 0u, 0u, 0u);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+      }
+    }
     issue_qk(0);
     if (jn > 1) issue_qk(1);
     for (int j = 0; j < jn; ++j) {
@@ -324,11 +337,31 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long tprev = clock64();
 #endif
+    // A warp whose 32 rows all lie past the end of the group (the padding of the group's last q-tile: 12 % of all rows at C4) has
+    // nothing to compute: its rows of P stay zero (written once per buffer, here, while both are free), and per key tile it only
+    // keeps the barrier phases in step.  The kernel runs at the board's power cap, so the exponentials it does not compute and the
+    // zero rows the PV MMA multiplies are clock for the valid rows.
+    const bool warp_dead = !__any_sync(0xffffffffu, row_ok);
+    if (warp_dead) {
+      uint32_t z[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) z[i] = 0u;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) tmem_st16(p_addr + c * 16, z);     // this set's P_b (64 columns); ordered before PV by the set's p_ready arrivals
+      tmem_st_wait();
+      tc_fence_before();
+    }
     for (int j = b; j < jn; j += 2) {
       const int rows_valid = min(kBN, kappa - j * kBN);
       AMARK(0);
       mbar_wait(&B->s_full[b], (j >> 1) & 1);
       AMARK(1);
+      if (warp_dead) {
+        mbar_arrive(&B->s_free[b]);
+        if (j >= 2) mbar_wait(&B->p_free[b], ((j - 2) >> 1) & 1);
+        mbar_arrive(&B->p_ready[b]);
+        continue;
+      }
       tc_fence_after();
       tmem_ld32_nowait(s_addr, v0);
       tmem_ld32_nowait(s_addr + 32, v1);
@@ -419,7 +452,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) hva_attn_tc_kernel(const __grid
     if (p.probe && tid == 0) for (int k = 0; k < 8; ++k) atomicAdd(p.probe + 8 + k, tacc[k]);
 #endif
     // final reference of the row, partial sums of the two sets
-    while (seq[r] != jn) { }
+    if (!warp_dead) while (seq[r] != jn) { }
     __threadfence_block();
     {
       const float m_fin = mref[r];
