@@ -438,20 +438,6 @@ extern "C" int hva_cluster_ex(const hva_shape* s, const int32_t cell[3], const i
   if (s->dtype != HVA_F32 && s->dtype != HVA_BF16) return HVA_EUNSUPPORTED;
   HvaGrid g = hva_make_grid(s, cell, win);
   int BH = s->B * s->heads;
-#ifdef HVA_HEAD_GROUP
-  if (BH > HVA_HEAD_GROUP && s->B == 1) {   // EXPERIMENT: all iterations of a few heads back to back (X of a head stays in L2)
-    const size_t es = s->dtype == HVA_F32 ? 4 : 2;
-    for (int h0 = 0; h0 < BH; h0 += HVA_HEAD_GROUP) {
-      hva_shape sub = *s;
-      sub.heads = std::min(HVA_HEAD_GROUP, BH - h0);
-      const size_t o = (size_t)h0;
-      HVA_TRY(hva_cluster_ex(&sub, cell, win, iters, (const char*)X + o * g.n * s->D * es, mu_init ? mu_init + o * g.Nc * s->D : nullptr,
-                             assign + o * g.n, mu + o * g.Nc * s->D, sizes + o * g.Nc, sums ? sums + o * g.Nc * s->D : nullptr,
-                             lowe ? lowe + o * g.n : nullptr, flags, probe, ws, ws_bytes, stream));
-    }
-    return HVA_OK;
-  }
-#endif
   if ((size_t)g.nwin * hva_assign_tc_csplit(g) > 1024 || (size_t)BH * g.Nc * g.nwin * hva_assign_tc_csplit(g) >= (1ull << 32)) return HVA_EUNSUPPORTED;
   if (ws_bytes < hva_cluster_ws_bytes(g, BH, s->D)) return HVA_EWORKSPACE;
   ClusterWs cw;
