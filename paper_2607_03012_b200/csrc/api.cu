@@ -385,13 +385,34 @@ extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const v
     return rc;
   }
   std::lock_guard<std::mutex> hold(pipe->busy);
-  // chunk boundaries: the first chunk's H2D copy and the last chunk's D2H copy are the only transfers no kernel covers, so
-  // both end chunks are small (heads / 12) and the heads between them go in three equal parts
-  const int nchunk = 5;
-  int bound[8];
+  // Chunk sizes.  The H2D copies run back to back from t = 0; chunk k's kernels can start when its copy has landed and chunk k-1's
+  // kernels are done.  With a = copy time and b = r a = kernel time per head, nothing waits iff  c_k <= c_1 + (r - 1) S_{k-1}
+  // (S = heads before chunk k): the chunks grow geometrically from a small first one, and the last one is small again because its
+  // D2H copy is the one transfer nothing covers.  r is estimated from the problem size (attention ~ n^2 per head, copies ~ n; 0.45
+  // of the tile pairs executed, 1.2 PFLOP/s, 55 GB/s); the smallest c_1 whose schedule fits 8 chunks is taken.
+  int nchunk = 0;
+  int bound[9];
   {
-    const int edge = s->heads / 12 > 0 ? s->heads / 12 : 1, mid = s->heads - 2 * edge;
-    bound[0] = 0; bound[1] = edge; bound[2] = edge + mid / 3; bound[3] = edge + (2 * mid) / 3; bound[4] = edge + mid; bound[5] = s->heads;
+    const double n_tok = (double)s->T * s->H * s->W;
+    double r = n_tok * 0.45 * 3.1e-5 * (2.0 / (double)es);
+    r = r < 1.05 ? 1.05 : (r > 3.0 ? 3.0 : r);
+    for (int c1 = 1; c1 <= s->heads && nchunk == 0; ++c1) {
+      int sizes[8], k = 0, S = 0;
+      const int last = std::min(c1, s->heads - c1);          // heads >= 8 here
+      sizes[k++] = c1; S = c1;
+      while (S < s->heads - last && k < 7) {
+        int cap = (int)std::floor((double)c1 + (r - 1.0) * (double)S);
+        if (cap < 1) cap = 1;
+        const int take = std::min(cap, s->heads - last - S);
+        sizes[k++] = take; S += take;
+      }
+      if (S != s->heads - last) continue;                     // does not fit 8 chunks: a larger first chunk
+      sizes[k++] = last;
+      bound[0] = 0;
+      for (int i = 0; i < k; ++i) bound[i + 1] = bound[i] + sizes[i];
+      nchunk = k;
+    }
+    if (nchunk == 0) { nchunk = 1; bound[0] = 0; bound[1] = s->heads; }
   }
   int rc = HVA_OK;
   // the copy streams start after whatever the caller has queued on `st`
