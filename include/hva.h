@@ -283,10 +283,13 @@ int hva_forward(const hva_shape* s, const hva_config* c, const void* Q, const vo
 
 /* Same as hva_forward with HOST Q,K,V,O (pinned or pageable); allocates nothing: `dev_qkvo` is a
  * caller-owned DEVICE staging buffer of 4*B*heads*n*D elements.  Heads are independent, so with B = 1, >= 8 heads and no
- * hybrid state the call runs in 5 chunks of heads (two small end chunks of heads/12 heads, three equal parts between them:
- * only the first chunk's H2D copy and the last chunk's D2H copy are not covered by kernels): the copies of the neighbouring
- * chunks (two library-owned copy streams, both PCIe directions; pinned host buffers needed for the overlap) run under the
- * kernels of the current one.  Chunked and unchunked calls give the same bits (the merge hash is keyed by the global head).
+ * hybrid state the call runs in up to 16 chunks of heads whose sizes grow geometrically from a one-head first chunk (so that
+ * a chunk's H2D copy has landed before the kernels of the chunk before it are done) and end with a small one: only the first
+ * chunk's H2D copy and the last chunk's D2H copy are not covered by kernels.  The copies (two library-owned copy streams, both
+ * PCIe directions; pinned host buffers needed for the overlap) run under the kernels; consecutive chunks run on two library-owned
+ * compute streams with one half of `ws` each when a half holds the largest chunk (the small stages of chunk k+1 then fill in under
+ * the attention kernel of chunk k), else on `stream`; all of them start after what the caller has queued on `stream` and are
+ * drained before the call returns.  Chunked and unchunked calls give the same bits (the merge hash is keyed by the global head).
  * Arguments are validated before anything is enqueued; on any error the stream and the copy streams are drained before
  * returning.  The copy streams are per device; concurrent host calls on the same device are serialised by the library.
  * Synchronises the stream. */

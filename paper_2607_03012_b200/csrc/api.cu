@@ -324,16 +324,18 @@ namespace {
 // is allocated).  The table is guarded by a mutex; a call holds its device's set for its whole duration, so concurrent host
 // calls on one device are serialised (documented in hva.h).
 struct HostPipe {
-  cudaStream_t h2d = nullptr, d2h = nullptr;
-  cudaEvent_t in_done[8] = {}, out_ready[8] = {}, start = nullptr;
+  cudaStream_t h2d = nullptr, d2h = nullptr, comp[2] = {nullptr, nullptr};   // copy streams; compute streams of the even / odd chunks
+  cudaEvent_t in_done[16] = {}, out_ready[16] = {}, start = nullptr;
   bool tried = false, ok = false;
   std::mutex busy;
   void create() {
     tried = true;
     ok = cudaStreamCreateWithFlags(&h2d, cudaStreamNonBlocking) == cudaSuccess &&
-         cudaStreamCreateWithFlags(&d2h, cudaStreamNonBlocking) == cudaSuccess;
+         cudaStreamCreateWithFlags(&d2h, cudaStreamNonBlocking) == cudaSuccess &&
+         cudaStreamCreateWithFlags(&comp[0], cudaStreamNonBlocking) == cudaSuccess &&
+         cudaStreamCreateWithFlags(&comp[1], cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&start, cudaEventDisableTiming) == cudaSuccess;
-    for (int i = 0; i < 8 && ok; ++i)
+    for (int i = 0; i < 16 && ok; ++i)
       ok = cudaEventCreateWithFlags(&in_done[i], cudaEventDisableTiming) == cudaSuccess &&
            cudaEventCreateWithFlags(&out_ready[i], cudaEventDisableTiming) == cudaSuccess;
   }
@@ -389,24 +391,25 @@ extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const v
   // kernels are done.  With a = copy time and b = r a = kernel time per head, nothing waits iff  c_k <= c_1 + (r - 1) S_{k-1}
   // (S = heads before chunk k): the chunks grow geometrically from a small first one, and the last one is small again because its
   // D2H copy is the one transfer nothing covers.  r is estimated from the problem size (attention ~ n^2 per head, copies ~ n; 0.45
-  // of the tile pairs executed, 1.2 PFLOP/s, 55 GB/s); the smallest c_1 whose schedule fits 8 chunks is taken.
+  // of the tile pairs executed, 1.2 PFLOP/s, 55 GB/s); the smallest c_1 whose schedule fits 16 chunks is taken
+  // (with the chunks alternating between two compute streams, below, a chunk's fixed costs are hidden, so many chunks are cheap).
   int nchunk = 0;
-  int bound[9];
+  int bound[17];
   {
     const double n_tok = (double)s->T * s->H * s->W;
     double r = n_tok * 0.45 * 3.1e-5 * (2.0 / (double)es);
     r = r < 1.05 ? 1.05 : (r > 3.0 ? 3.0 : r);
     for (int c1 = 1; c1 <= s->heads && nchunk == 0; ++c1) {
-      int sizes[8], k = 0, S = 0;
+      int sizes[16], k = 0, S = 0;
       const int last = std::min(c1, s->heads - c1);          // heads >= 8 here
       sizes[k++] = c1; S = c1;
-      while (S < s->heads - last && k < 7) {
+      while (S < s->heads - last && k < 15) {
         int cap = (int)std::floor((double)c1 + (r - 1.0) * (double)S);
         if (cap < 1) cap = 1;
         const int take = std::min(cap, s->heads - last - S);
         sizes[k++] = take; S += take;
       }
-      if (S != s->heads - last) continue;                     // does not fit 8 chunks: a larger first chunk
+      if (S != s->heads - last) continue;                     // does not fit 16 chunks: a larger first chunk
       sizes[k++] = last;
       bound[0] = 0;
       for (int i = 0; i < k; ++i) bound[i + 1] = bound[i] + sizes[i];
@@ -415,31 +418,46 @@ extern "C" int hva_forward_host(const hva_shape* s, const hva_config* c, const v
     if (nchunk == 0) { nchunk = 1; bound[0] = 0; bound[1] = s->heads; }
   }
   int rc = HVA_OK;
-  // the copy streams start after whatever the caller has queued on `st`
+  // Consecutive chunks run on two compute streams with one half of the workspace each, so that the small, latency-bound stages of
+  // chunk k+1 (clustering, mask, merge, plan: ~0.5 ms whatever the head count) fill in under the attention kernel of chunk k
+  // instead of following it; a stream's order keeps chunk k+2 off the half chunk k still uses.  If a half cannot hold the largest
+  // chunk, everything runs on the caller's stream with the whole workspace.
+  size_t half = (ws_bytes / 2) & ~(size_t)255, need = 0;
+  for (int i = 0; i < nchunk; ++i) {
+    hva_shape sc = *s;
+    sc.heads = bound[i + 1] - bound[i];
+    need = std::max(need, hva_workspace_bytes(&sc, c));
+  }
+  const bool two = nchunk > 1 && need > 0 && need <= half;
+  cudaStream_t cs[2] = {two ? pipe->comp[0] : st, two ? pipe->comp[1] : st};
+  // the library's streams start after whatever the caller has queued on `st`
   if (cudaEventRecord(pipe->start, st) != cudaSuccess || cudaStreamWaitEvent(pipe->h2d, pipe->start, 0) != cudaSuccess ||
-      cudaStreamWaitEvent(pipe->d2h, pipe->start, 0) != cudaSuccess)
+      cudaStreamWaitEvent(pipe->d2h, pipe->start, 0) != cudaSuccess ||
+      (two && (cudaStreamWaitEvent(cs[0], pipe->start, 0) != cudaSuccess || cudaStreamWaitEvent(cs[1], pipe->start, 0) != cudaSuccess)))
     rc = HVA_ECUDA;
   const char* src[3] = {(const char*)hQ, (const char*)hK, (const char*)hV};
   for (int i = 0; i < nchunk && rc == HVA_OK; ++i) {
     const int h0 = bound[i], h1 = bound[i + 1], nh = h1 - h0;
     const size_t off = (size_t)h0 * head_bytes, cb = (size_t)nh * head_bytes;
+    cudaStream_t ci = cs[i & 1];
     for (int t = 0; t < 3 && rc == HVA_OK; ++t)
       if (cudaMemcpyAsync(d + t * bytes + off, src[t] + off, cb, cudaMemcpyHostToDevice, pipe->h2d) != cudaSuccess) rc = HVA_ECUDA;
-    if (rc == HVA_OK && (cudaEventRecord(pipe->in_done[i], pipe->h2d) != cudaSuccess || cudaStreamWaitEvent(st, pipe->in_done[i], 0) != cudaSuccess))
+    if (rc == HVA_OK && (cudaEventRecord(pipe->in_done[i], pipe->h2d) != cudaSuccess || cudaStreamWaitEvent(ci, pipe->in_done[i], 0) != cudaSuccess))
       rc = HVA_ECUDA;
     if (rc != HVA_OK) break;
     hva_shape sc = *s;
     sc.heads = nh;
-    rc = forward_impl(&sc, c, d + off, d + bytes + off, d + 2 * bytes + off, d + 3 * bytes + off, step_kind, nullptr, nullptr, ws,
-                      ws_bytes, stream, h0);
+    rc = forward_impl(&sc, c, d + off, d + bytes + off, d + 2 * bytes + off, d + 3 * bytes + off, step_kind, nullptr, nullptr,
+                      two ? (char*)ws + (i & 1) * half : (char*)ws, two ? half : ws_bytes, ci, h0);
     if (rc != HVA_OK) break;
-    if (cudaEventRecord(pipe->out_ready[i], st) != cudaSuccess || cudaStreamWaitEvent(pipe->d2h, pipe->out_ready[i], 0) != cudaSuccess ||
+    if (cudaEventRecord(pipe->out_ready[i], ci) != cudaSuccess || cudaStreamWaitEvent(pipe->d2h, pipe->out_ready[i], 0) != cudaSuccess ||
         cudaMemcpyAsync((char*)hO + off, d + 3 * bytes + off, cb, cudaMemcpyDeviceToHost, pipe->d2h) != cudaSuccess)
       rc = HVA_ECUDA;
   }
   // drain all three streams, also on error: no copy into or out of the caller's buffers is left in flight
   const bool s0 = cudaStreamSynchronize(pipe->h2d) == cudaSuccess, s1 = cudaStreamSynchronize(st) == cudaSuccess,
-             s2 = cudaStreamSynchronize(pipe->d2h) == cudaSuccess;
-  if (rc == HVA_OK && !(s0 && s1 && s2)) rc = HVA_ECUDA;
+             s2 = cudaStreamSynchronize(pipe->d2h) == cudaSuccess, s3 = cudaStreamSynchronize(pipe->comp[0]) == cudaSuccess,
+             s4 = cudaStreamSynchronize(pipe->comp[1]) == cudaSuccess;
+  if (rc == HVA_OK && !(s0 && s1 && s2 && s3 && s4)) rc = HVA_ECUDA;
   return rc;
 }
