@@ -651,3 +651,23 @@ def test_cluster_qk_two_streams_equals_two_cluster_calls():
                                 b._p(k["assign"]), b._p(k["mu"]), b._p(k["sizes"]), b._p(k["sums"]), b._p(ws), C.c_size_t(ws.numel()),
                                 b._p(ws), C.c_size_t(ws.numel()), b._stream())
     assert rc == -1
+
+
+@pytest.mark.parametrize("dtype,D", [("bf16", 64), ("bf16", 128), ("f32", 64), ("f32", 128)])
+def test_permute_row_gather_all_row_widths(dtype, D):
+    """hva_permute / hva_unpermute against torch indexing for every row width the gather kernel is instantiated for (8, 16 and 32
+    16-byte chunks per row), a row count that is not a multiple of the rows one warp moves per iteration, and per-head random
+    permutations (bit-exact: byte copies)."""
+    b = _b()
+    heads, T, H, W = 3, 3, 7, 11                      # n = 231 rows per head
+    n = T * H * W
+    g = torch.Generator().manual_seed(100 + D + (0 if dtype == "bf16" else 1))
+    tdt = torch.bfloat16 if dtype == "bf16" else torch.float32
+    X = torch.randn((1, heads, n, D), generator=g, dtype=torch.float32).to(tdt).cuda().contiguous()
+    perm = torch.stack([torch.randperm(n, generator=g) for _ in range(heads)]).to(torch.int32).cuda().contiguous()
+    shape = b.make_shape((1, heads, T, H, W, D), dtype=dtype)
+    Xp = b.hva_permute(shape, X, perm)
+    torch.cuda.synchronize()
+    ref = torch.stack([X[0, h][perm[h].long()] for h in range(heads)]).unsqueeze(0)
+    assert torch.equal(Xp, ref)
+    assert torch.equal(b.hva_unpermute(shape, Xp, perm), X)
