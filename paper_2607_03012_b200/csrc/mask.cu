@@ -194,11 +194,13 @@ __device__ __forceinline__ int mask_key_j(unsigned long long k) { return 2047 - 
 
 constexpr int kWarpRows = 8;
 
-template <int D, int E>
+// E keys per lane and sorted run, R runs per lane (R = 2: 1024 < N_k <= 2048, two runs of 32: the selection below works on sorted
+// runs, so a lane never holds more than 32 keys in registers)
+template <int D, int E, int R>
 __global__ void __launch_bounds__(256, 2) hva_mask_warp_kernel(int Nq, int Nk, const float* __restrict__ mu_q,
                                                             const float* __restrict__ mu_k, const int* __restrict__ sizes_k,
                                                             double scale, double top_p, int kmin, uint8_t* __restrict__ mask) {
-  constexpr int P = 32 * E;
+  constexpr int P = 32 * E * R;
   const int i0 = blockIdx.x * kWarpRows, bh = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* s_q = reinterpret_cast<double*>(smem_raw);         // [kWarpRows][D]
@@ -247,92 +249,109 @@ __global__ void __launch_bounds__(256, 2) hva_mask_warp_kernel(int Nq, int Nk, c
   __syncthreads();
   if (warp >= nrows) return;
   uint8_t* mrow = mask + ((size_t)bh * Nq + i0 + warp) * Nk;
-  const double* sc = s_sc + (size_t)warp * P;
-  WarpSort<E> ws;
+  double* sc = s_sc + (size_t)warp * P;
   double smax = -1.0 / 0.0;
-  double wv[E];
 #pragma unroll
-  for (int i = 0; i < E; ++i) {                              // initial placement is arbitrary: key j = 32 i + lane (conflict-free)
-    const int jj = 32 * i + lane;
-    wv[i] = jj < Nk ? sc[jj] : -1.0 / 0.0;
-    smax = fmax(smax, wv[i]);
+  for (int q = 0; q < E * R; ++q) {                          // key j = 32 q + lane (conflict-free, and an interleaved sample of the row)
+    const int jj = 32 * q + lane;
+    if (jj < Nk) smax = fmax(smax, sc[jj]);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
-#pragma unroll
-  for (int i = 0; i < E; ++i) {                              // w_j = s^k_j exp(S_j - max); pads get the smallest key of all (0, j >= N_k)
-    const int jj = 32 * i + lane;
-    ws.k[i] = jj < Nk ? mask_key((double)sizes_k[(size_t)bh * Nk + jj] * exp(wv[i] - smax), jj) : (unsigned long long)(2047 - jj);
-  }
   // Selection instead of a full sort of the row (round 2: 55 bitonic stages, two thirds of the kernel's instructions).  The cut is
   // the LARGEST key c with  sum_{k >= c} w_k >= p Z  and  #{k >= c} >= kmin  (Eq. 3 + min-kc: the same prefix as "sort, then first
-  // cum >= p Z"; keys are unique, so "k >= c" is the sorted prefix that ends at c).  Each lane sorts only its own E keys (registers, no
-  // shuffles) and parks them in shared memory, skey[i][lane]; then a quickselect on the key VALUE: the pivot is the middle key of
-  // the longest still-undecided lane segment (keys j = 32 i + lane are an interleaved sample of the row, so it splits every lane's
-  // segment about in half), every lane counts its keys >= pivot by binary search and adds the weights of the keys that moved, and the
-  // warp decides.  ~12-15 rounds of ~90 instructions.  The sums are associated differently from a sequential cumulative sum (R-K3's
-  // 1e-9 Z exemption covers that, as it did the scan's).
-  ws.sort_lane();
-  unsigned long long* skey = reinterpret_cast<unsigned long long*>(s_sc + (size_t)warp * P);   // the row's scores are consumed
+  // cum >= p Z"; keys are unique, so "k >= c" is the sorted prefix that ends at c).  Each lane sorts its own keys in runs of E
+  // (registers, no shuffles) and parks them in shared memory -- in place: slot 32 q + lane held the score of the key the lane read
+  // from it; then a quickselect on the key VALUE: the pivot is the middle key of the longest still-undecided run (a lane's keys
+  // are an interleaved sample of the row, so it splits every run about in half), every lane counts its keys >= pivot by binary
+  // search and adds the weights of the keys that moved, and the warp decides.  ~12-15 rounds of ~90 instructions.  The sums are
+  // associated differently from a sequential cumulative sum (R-K3's 1e-9 Z exemption covers that, as it did the scan's).
+  unsigned long long* skey = reinterpret_cast<unsigned long long*>(sc);
   double run = 0.0;
 #pragma unroll
-  for (int i = 0; i < E; ++i) run += mask_key_w(ws.k[i]);
+  for (int u = 0; u < R; ++u) {
+    WarpSort<E> ws;
+#pragma unroll
+    for (int i = 0; i < E; ++i) {                            // w_j = s^k_j exp(S_j - max); pads get the smallest keys of all (0, j >= N_k)
+      const int jj = 32 * (u * E + i) + lane;
+      ws.k[i] = jj < Nk ? mask_key((double)sizes_k[(size_t)bh * Nk + jj] * exp(sc[jj] - smax), jj) : (unsigned long long)(2047 - jj);
+    }
+    ws.sort_lane();
+#pragma unroll
+    for (int i = 0; i < E; ++i) { run += mask_key_w(ws.k[i]); skey[(u * E + i) * 32 + lane] = ws.k[i]; }
+  }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) run += __shfl_xor_sync(0xffffffffu, run, o);   // same bits in every lane (commutative tree)
   const double thr = top_p * run;
   __syncwarp();
-#pragma unroll
-  for (int i = 0; i < E; ++i) skey[i * 32 + lane] = ws.k[i];
-  __syncwarp();
   const unsigned long long U0 = (unsigned long long)(2047 - Nk);   // below every real key, at or above every pad: "everything"
   unsigned long long U = U0;                                     // largest key known to satisfy the condition
-  int a = 0;                                                     // keys [0, a) of this lane are >= L, the smallest key known to fail
-  int b = lane < Nk ? (Nk - lane + 31) >> 5 : 0;                 // keys [a, b) are undecided (the lane's real keys come first)
+  int a[R], b[R];                                                // run u: keys [0, a) are >= L (the smallest key known to fail), [a, b) undecided
+#pragma unroll
+  for (int u = 0; u < R; ++u) {                                  // the run's real keys come first
+    a[u] = 0;
+    const int first = 32 * u * E + lane;                         // j of the run's first slot
+    b[u] = first < Nk ? min(E, (Nk - first + 31) >> 5) : 0;
+  }
   double S_hi = 0.0;                                             // sum of the weights of all keys >= L
   int N_hi = 0;
   for (;;) {
-    const unsigned best = __reduce_max_sync(0xffffffffu, ((unsigned)(b - a) << 5) | (unsigned)lane);
-    if ((best >> 5) == 0) break;
-    const int src = (int)(best & 31u);
-    const unsigned long long mine = b > a ? skey[((a + b) >> 1) * 32 + lane] : 0ull;
-    const unsigned long long pv = __shfl_sync(0xffffffffu, mine, src);
-    int lo = a, hi = b;                                          // c = number of this lane's keys >= pv
+    unsigned mine_len = 0;
 #pragma unroll
-    for (int it = 0; it < 6; ++it) {
-      if (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if (skey[mid * 32 + lane] >= pv) lo = mid + 1; else hi = mid;
-      }
-    }
-    const int c = lo;
+    for (int u = 0; u < R; ++u) mine_len = max(mine_len, ((unsigned)(b[u] - a[u]) << 6) | ((unsigned)u << 5) | (unsigned)lane);
+    const unsigned best = __reduce_max_sync(0xffffffffu, mine_len);
+    if ((best >> 6) == 0) break;
+    const int src = (int)(best & 31u), su = (int)((best >> 5) & 1u);
+    unsigned long long mine = 0ull;
+#pragma unroll
+    for (int u = 0; u < R; ++u)
+      if (u == su && b[u] > a[u]) mine = skey[(u * E + ((a[u] + b[u]) >> 1)) * 32 + lane];
+    const unsigned long long pv = __shfl_sync(0xffffffffu, mine, src);
+    int c[R], moved = 0;
     double sum = 0.0;
-    for (int idx = a; idx < c; ++idx) sum += mask_key_w(skey[idx * 32 + lane]);
+#pragma unroll
+    for (int u = 0; u < R; ++u) {
+      int lo = a[u], hi = b[u];                                  // c = number of this run's keys >= pv
+#pragma unroll
+      for (int it = 0; it < 6; ++it) {
+        if (lo < hi) {
+          const int mid = (lo + hi) >> 1;
+          if (skey[(u * E + mid) * 32 + lane] >= pv) lo = mid + 1; else hi = mid;
+        }
+      }
+      c[u] = lo;
+      for (int idx = a[u]; idx < lo; ++idx) sum += mask_key_w(skey[(u * E + idx) * 32 + lane]);
+      moved += lo - a[u];
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-    const int cn = __reduce_add_sync(0xffffffffu, c - a);
+    const int cn = __reduce_add_sync(0xffffffffu, moved);
     const double S = S_hi + sum;
     const int N = N_hi + cn;
     if (S >= thr && N >= kmin) {     // warp-uniform: S, N are the same bits in every lane
       U = pv;
-      b = c - (lane == src ? 1 : 0);                             // undecided: the keys above pv
+#pragma unroll
+      for (int u = 0; u < R; ++u) b[u] = c[u] - ((lane == src && u == su) ? 1 : 0);   // undecided: the keys above pv
     } else {
-      a = c; S_hi = S; N_hi = N;                                 // pv fails and becomes L
+#pragma unroll
+      for (int u = 0; u < R; ++u) a[u] = c[u];                   // pv fails and becomes L
+      S_hi = S; N_hi = N;
     }
   }
 #pragma unroll
-  for (int i = 0; i < E; ++i) {
-    const unsigned long long k = skey[i * 32 + lane];
+  for (int q = 0; q < E * R; ++q) {
+    const unsigned long long k = skey[q * 32 + lane];
     const int jj = mask_key_j(k);
     if (jj < Nk) mrow[jj] = k >= U ? 1 : 0;
   }
 }
 
-template <int D, int E>
+template <int D, int E, int R>
 int launch_mask_warp(int BH, int Nq, int Nk, const float* mu_q, const float* mu_k, const int* sizes_k, double scale, double top_p,
                      int kmin, uint8_t* mask, cudaStream_t st) {
-  const size_t smem = (size_t)kWarpRows * D * 8 + (size_t)kWarpRows * 32 * E * 8;
-  if (cudaFuncSetAttribute(hva_mask_warp_kernel<D, E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return HVA_ECUDA;
-  hva_mask_warp_kernel<D, E><<<dim3((Nq + kWarpRows - 1) / kWarpRows, BH), 256, smem, st>>>(Nq, Nk, mu_q, mu_k, sizes_k, scale, top_p, kmin, mask);
+  const size_t smem = (size_t)kWarpRows * D * 8 + (size_t)kWarpRows * 32 * E * R * 8;
+  if (cudaFuncSetAttribute(hva_mask_warp_kernel<D, E, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return HVA_ECUDA;
+  hva_mask_warp_kernel<D, E, R><<<dim3((Nq + kWarpRows - 1) / kWarpRows, BH), 256, smem, st>>>(Nq, Nk, mu_q, mu_k, sizes_k, scale, top_p, kmin, mask);
   HVA_CHECK_LAUNCH();
   return HVA_OK;
 }
@@ -358,12 +377,13 @@ extern "C" int hva_build_mask_ex(int32_t BH, int32_t Nq, int32_t Nk, int32_t D, 
   int kmin = (int)ceil((double)min_kc * (double)Nk);
   size_t smem = (size_t)P * 12 + (size_t)kRowsPerCta * Nk * 8 + (size_t)kRowsPerCta * D * 8 + kMaskThreads * 8 + 16;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (top_p < 1.f && Nk <= 1024 && !(flags & HVA_FLAG_MASK_BLOCKSORT)) {   // warp-per-row register sort
+  if (top_p < 1.f && !(flags & HVA_FLAG_MASK_BLOCKSORT)) {   // warp per row: selection on lane-sorted runs (N_k <= 2048 here)
 #define HVA_MASK_WARP(DD)                                                                                                             \
     do {                                                                                                                              \
-      if (Nk <= 256) return launch_mask_warp<DD, 8>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st);  \
-      if (Nk <= 512) return launch_mask_warp<DD, 16>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st); \
-      return launch_mask_warp<DD, 32>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st);                \
+      if (Nk <= 256) return launch_mask_warp<DD, 8, 1>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st);  \
+      if (Nk <= 512) return launch_mask_warp<DD, 16, 1>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st); \
+      if (Nk <= 1024) return launch_mask_warp<DD, 32, 1>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st); \
+      return launch_mask_warp<DD, 32, 2>(BH, Nq, Nk, mu_q, mu_k, sizes_k, (double)scale, (double)top_p, kmin, mask, st);             \
     } while (0)
     if (D == 64) HVA_MASK_WARP(64);
     HVA_MASK_WARP(128);
