@@ -356,3 +356,33 @@ def test_mask_merge_plan_paper_cluster_counts():
             for k in ("perm_q", "inv_perm_q", "perm_k", "koff"):
                 assert np.array_equal(getattr(plan, k)[hi].cpu().numpy(), po[k]), k
             assert np.array_equal(plan.goff[hi].cpu().numpy()[:len(gids) + 1], po["goff"])
+
+
+def test_c4_forward_is_deterministic_and_ignores_stale_workspace():
+    """The whole C4 call three times on the same inputs, the workspace filled with random bytes in between: the output, the mask, the
+    merge result and every meaningful array of the plan are the same bits each time (no floating-point atomics, no dependence on
+    what a previous call -- or anybody else -- left in the workspace, no race between the two streams the call runs on)."""
+    b = _b()
+    wl = inputs.CONFIGS["C4"]
+    Q, K, V = _device_inputs("C4")
+    shape, cfg = b.make_shape(wl), b.make_config(wl)
+    fwd = b.Forward(shape, cfg)
+    ref = None
+    for it in range(3):
+        O = torch.empty_like(Q)
+        fwd(Q, K, V, O)
+        torch.cuda.synchronize()
+        views = fwd.ws_views()
+        pl, ng = views["plan"], views["n_groups"]
+        snap = [O.clone()] + [v.clone() for v in views.values() if torch.is_tensor(v)]
+        snap += [getattr(pl, k).clone() for k in ("perm_q", "inv_perm_q", "perm_k", "koff", "stats")]
+        for h in range(0, pl.BH, 5):
+            g, wc = int(ng[h]), int(pl.work_cnt[h])
+            snap += [pl.gid[h, :g].clone(), pl.goff[h, :g + 1].clone(), pl.kappa[h, :g].clone(), pl.run_cnt[h, :g].clone(),
+                     pl.work[h, :wc].clone()]
+        if ref is None:
+            ref = snap
+        else:
+            for i, (x, y) in enumerate(zip(ref, snap)):
+                assert torch.equal(x, y), (it, i)
+        fwd.ws.random_(0, 255)
